@@ -1,0 +1,122 @@
+/*
+ * oat.h -- C ABI of liboat.so: the matched projector pair H / H^T of the
+ * interpolation-based discrete-to-discrete imaging model of 3-D optoacoustic
+ * tomography (arxiv/paper_1304_2017), as hand-written CUDA kernels for sm_100a.
+ *
+ * Citations are PAPER.md line numbers (+ equation / algorithm).
+ *
+ *   H   = D G      projection      (Eq. 11 L116 without H^e; G = Eq. 12 L121 and
+ *                                   Appendix Eq. 35-39; D = Eq. 13 L125 / Eq. 3)
+ *   H^T = G^T D^T  backprojection  (L168; D^T = Eq. 22; G^T = Eq. 23, Alg. 6)
+ *
+ * The discretisation implemented is "OAT-DISC v1".
+ *
+ * Conventions
+ *   - units: mm and microseconds.
+ *   - volume x: nz*ny*nx fp32, x fastest, voxel n = (iz*ny + iy)*nx + ix (Alg. 6 L601 order);
+ *     node (ix,iy,iz) sits at origin + spacing*(ix,iy,iz)             (L203, Eq. 9).
+ *   - data y: Q*K fp32, index m = q*K + k, time fastest                (Eq. 5).
+ *   - pointers named d_* are DEVICE pointers owned by the caller (e.g. torch tensors);
+ *     pointers named h_* are HOST pointers owned by the caller.  The library never frees or
+ *     reallocates them.  The geometry handle owns its own device tables and scratch buffers.
+ *   - every function returns 0 (OAT_OK) or a negative error code, never throws, never exits;
+ *     oat_last_error() gives a thread-local message for the last failure on this thread.
+ *   - `cuda_stream` is a cudaStream_t (NULL = the legacy default stream).  Calls are
+ *     asynchronous on that stream unless stated otherwise.  One handle must not be used from two
+ *     streams at the same time (its scratch buffers are shared).
+ *   - there is no CPU fallback: without a CUDA device every call fails with OAT_ERR_CUDA.
+ */
+#ifndef OAT_H
+#define OAT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OAT_OK 0
+#define OAT_ERR_INVALID (-1) /* bad argument / descriptor */
+#define OAT_ERR_ALLOC (-2)   /* host or device allocation failed */
+#define OAT_ERR_CUDA (-3)    /* CUDA runtime error (message has the CUDA string) */
+
+/* Problem statement of the paper: reconstruction cuboid (L203), point-like transducers (L114),
+ * speed of sound, first sample time t_min, sampling interval, number of samples (L203, L255). */
+typedef struct {
+    int32_t nx, ny, nz;      /* nodes per axis (N_x, N_y, N_z), each >= 1 */
+    double spacing;          /* Delta_s > 0 */
+    double origin[3];        /* (x_min, y_min, z_min): position of node (0,0,0) */
+    int32_t n_trans;         /* Q >= 0 */
+    const double *trans_xyz; /* HOST, Q x 3 row-major, copied at create */
+    double c;                /* c_0 > 0 */
+    double t0;               /* t_min >= 0: time of sample k = 0 */
+    double dt;               /* Delta_t > 0 */
+    int32_t nt;              /* K >= 1 */
+    double surf_step;        /* h: surface patch size of Eq. (37); 0 => spacing */
+    int32_t kband;           /* B: consecutive time samples sharing one angular rule (reading G11);
+                                0 => 32; 1 = the paper's per-sample rule; must be <= 32 */
+    double gain;             /* kappa = beta/(4 pi C_p) of Eq. (3); 0 => 1 */
+} oat_geometry_desc;
+
+typedef struct oat_geometry oat_geometry;
+
+/* Validates the descriptor (sizes, positive steps, finite positions, no transducer at the grid
+ * centre -- the local frame of Appendix L349 is undefined there), computes per-transducer frames
+ * and per-band ring tables in fp64 on the host, uploads them to `device`, allocates scratch.
+ * *out is set only on success. */
+int oat_geometry_create(const oat_geometry_desc *desc, int device, oat_geometry **out);
+
+/* Frees device and host tables.  NULL is a no-op.  The caller must have synchronised its streams. */
+void oat_geometry_destroy(oat_geometry *geom);
+
+/* Pure queries (negative on NULL). */
+int64_t oat_num_voxels(const oat_geometry *geom);  /* nx*ny*nz */
+int64_t oat_num_samples(const oat_geometry *geom); /* Q*K */
+/* Number of quadrature samples of OAT-DISC v1 that fall inside the zero-padded node box (the
+ * "interpolation samples" of the throughput metric).  Counted on the GPU on first use by a
+ * traversal-only kernel (synchronises the device once), then cached. */
+int64_t oat_num_surface_samples(oat_geometry *geom);
+
+/* y = H x.  d_x: nz*ny*nx fp32 (read), d_y: Q*K fp32 (OVERWRITTEN).  x and y must not alias. */
+int oat_project(oat_geometry *geom, const float *d_x, float *d_y, void *cuda_stream);
+
+/* x = H^T y.  d_y: Q*K fp32 (read), d_x: nz*ny*nx fp32 (OVERWRITTEN; the library zeroes it). */
+int oat_backproject(oat_geometry *geom, const float *d_y, float *d_x, void *cuda_stream);
+
+/* Adjoint test: lhs = <Hx, y>, rhs = <x, H^T y> with fp64 reductions on internal scratch,
+ * rel = |lhs - rhs| / max(|lhs|, |rhs|).  Synchronises `cuda_stream` before returning. */
+int oat_adjoint_check(oat_geometry *geom, const float *d_x, const float *d_y,
+                      double *lhs, double *rhs, double *rel, void *cuda_stream);
+
+/* Same operators with HOST buffers: pinned-or-pageable host memory in, host memory out; the
+ * host->device and device->host copies are part of the call, which returns after the result has
+ * landed in h_y / h_x (used for the end-to-end figure of bench.py). */
+int oat_project_host(oat_geometry *geom, const float *h_x, float *h_y);
+int oat_backproject_host(oat_geometry *geom, const float *h_y, float *h_x);
+
+/* Row C1: n_iter steps of CGLS (= linear CG on H^T H x = H^T y, L265) from
+ * x = 0 with fp32 vectors and fp64 dot products; one H and one H^T per iteration (L273).
+ * d_y: Q*K (read), d_x: nz*ny*nx (OVERWRITTEN with the iterate after n_iter steps).
+ * h_res / h_grad: HOST arrays of n_iter+1 doubles (may be NULL) receiving ||y - H x_i|| / ||y||
+ * and ||H^T (y - H x_i)|| for i = 0..n_iter.  Synchronises the stream every iteration. */
+int oat_cgls(oat_geometry *geom, const float *d_y, float *d_x, int n_iter,
+             double *h_res, double *h_grad, void *cuda_stream);
+
+/* Kernel-variant selection for measurements ("chosen by ncu", north_star).  key = "project" or
+ * "backproject"; the meaning of `variant` is listed in DESIGN.md §5.  Unknown => OAT_ERR_INVALID. */
+int oat_set_variant(oat_geometry *geom, const char *key, int variant);
+
+/* Number of kernels the last oat_project / oat_backproject on this handle launched. */
+int oat_last_launch_count(const oat_geometry *geom);
+
+/* Device time (ms, CUDA events on the call's stream) of the dominant kernel of the last
+ * oat_project / oat_backproject; synchronises that stream.  Negative if none was recorded. */
+float oat_last_kernel_ms(oat_geometry *geom);
+
+const char *oat_last_error(void);
+const char *oat_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OAT_H */

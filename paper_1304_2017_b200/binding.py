@@ -1,0 +1,254 @@
+"""Thin ctypes binding of liboat.so -- same names as include/oat.h, argument
+marshalling only.  PyTorch supplies device memory and streams; every step of
+the path runs in the library's CUDA kernels.  There is no CPU fallback: if the
+library cannot be loaded or no CUDA device exists, calls raise ``OatError``.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+_LIB_PATH = Path(__file__).resolve().parent / "csrc" / "liboat.so"
+_lib = None
+
+OAT_OK, OAT_ERR_INVALID, OAT_ERR_ALLOC, OAT_ERR_CUDA = 0, -1, -2, -3
+
+EXPORTS = [
+    "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
+    "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
+    "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
+    "oat_last_launch_count", "oat_last_kernel_ms", "oat_last_error", "oat_version",
+]
+
+
+class OatError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"liboat error {code}: {msg}")
+        self.code = code
+
+
+class oat_geometry_desc(ctypes.Structure):
+    _fields_ = [
+        ("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("nz", ctypes.c_int32),
+        ("spacing", ctypes.c_double),
+        ("origin", ctypes.c_double * 3),
+        ("n_trans", ctypes.c_int32),
+        ("trans_xyz", ctypes.POINTER(ctypes.c_double)),
+        ("c", ctypes.c_double), ("t0", ctypes.c_double), ("dt", ctypes.c_double),
+        ("nt", ctypes.c_int32),
+        ("surf_step", ctypes.c_double),
+        ("kband", ctypes.c_int32),
+        ("gain", ctypes.c_double),
+    ]
+
+
+def load():
+    """Load liboat.so (built in-tree by paper_1304_2017_b200.build); fail loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise OatError(OAT_ERR_CUDA, f"{_LIB_PATH} is missing: run `python -m paper_1304_2017_b200.build` "
+                                     "(nvcc, sm_100a). There is no CPU fallback.")
+    lib = ctypes.CDLL(str(_LIB_PATH))
+    vp, fp, dp = ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double)
+    lib.oat_geometry_create.argtypes = [ctypes.POINTER(oat_geometry_desc), ctypes.c_int, ctypes.POINTER(vp)]
+    lib.oat_geometry_create.restype = ctypes.c_int
+    lib.oat_geometry_destroy.argtypes = [vp]
+    lib.oat_geometry_destroy.restype = None
+    for n in ("oat_num_voxels", "oat_num_samples", "oat_num_surface_samples"):
+        getattr(lib, n).argtypes = [vp]
+        getattr(lib, n).restype = ctypes.c_int64
+    for n in ("oat_project", "oat_backproject"):
+        getattr(lib, n).argtypes = [vp, fp, fp, vp]
+        getattr(lib, n).restype = ctypes.c_int
+    lib.oat_adjoint_check.argtypes = [vp, fp, fp, dp, dp, dp, vp]
+    lib.oat_adjoint_check.restype = ctypes.c_int
+    for n in ("oat_project_host", "oat_backproject_host"):
+        getattr(lib, n).argtypes = [vp, fp, fp]
+        getattr(lib, n).restype = ctypes.c_int
+    lib.oat_cgls.argtypes = [vp, fp, fp, ctypes.c_int, dp, dp, vp]
+    lib.oat_cgls.restype = ctypes.c_int
+    lib.oat_set_variant.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
+    lib.oat_set_variant.restype = ctypes.c_int
+    lib.oat_last_launch_count.argtypes = [vp]
+    lib.oat_last_launch_count.restype = ctypes.c_int
+    lib.oat_last_kernel_ms.argtypes = [vp]
+    lib.oat_last_kernel_ms.restype = ctypes.c_float
+    lib.oat_last_error.restype = ctypes.c_char_p
+    lib.oat_version.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def oat_last_error() -> str:
+    return load().oat_last_error().decode()
+
+
+def oat_version() -> str:
+    return load().oat_version().decode()
+
+
+def _check(rc):
+    if rc != 0:
+        raise OatError(rc, oat_last_error())
+
+
+def make_desc(w):
+    """Descriptor from any object with the problem-statement attributes (e.g. workloads.Workload).
+    Returns (desc, keepalive)."""
+    tr = np.ascontiguousarray(np.asarray(w.trans_xyz, dtype=np.float64).reshape(-1, 3))
+    d = oat_geometry_desc()
+    d.nx, d.ny, d.nz = int(w.nx), int(w.ny), int(w.nz)
+    d.spacing = float(w.spacing)
+    d.origin = (ctypes.c_double * 3)(*[float(v) for v in w.origin])
+    d.n_trans = int(tr.shape[0])
+    d.trans_xyz = tr.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+    d.c, d.t0, d.dt = float(w.c), float(w.t0), float(w.dt)
+    d.nt = int(w.nt)
+    d.surf_step = float(getattr(w, "surf_step", 0.0))
+    d.kband = int(getattr(w, "kband", 0))
+    d.gain = float(getattr(w, "gain", 0.0))
+    return d, tr
+
+
+class Geometry:
+    """Owner of an ``oat_geometry*`` handle."""
+
+    def __init__(self, handle, device, n_trans, nt, shape):
+        self.handle, self.device, self.n_trans, self.nt, self.shape = handle, device, n_trans, nt, shape
+
+    def close(self):
+        if self.handle:
+            load().oat_geometry_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def oat_geometry_create(w, device: int = 0) -> Geometry:
+    d, keep = make_desc(w)
+    h = ctypes.c_void_p()
+    _check(load().oat_geometry_create(ctypes.byref(d), int(device), ctypes.byref(h)))
+    return Geometry(h, int(device), d.n_trans, d.nt, (d.nz, d.ny, d.nx))
+
+
+def oat_geometry_destroy(g: Geometry):
+    g.close()
+
+
+def oat_num_voxels(g) -> int:
+    return int(load().oat_num_voxels(g.handle))
+
+
+def oat_num_samples(g) -> int:
+    return int(load().oat_num_samples(g.handle))
+
+
+def oat_num_surface_samples(g) -> int:
+    v = int(load().oat_num_surface_samples(g.handle))
+    if v < 0:
+        raise OatError(OAT_ERR_CUDA, oat_last_error())
+    return v
+
+
+def _dev_ptr(t, n, what, g):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise OatError(OAT_ERR_INVALID, f"{what} must be a CUDA tensor")
+    if t.dtype != torch.float32 or not t.is_contiguous() or t.numel() != n:
+        raise OatError(OAT_ERR_INVALID, f"{what} must be contiguous float32 with {n} elements")
+    if t.device.index != g.device:
+        raise OatError(OAT_ERR_INVALID, f"{what} is on cuda:{t.device.index}, geometry on cuda:{g.device}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def oat_project(g, x, y=None, stream=None):
+    """y = H x on the current torch stream; x: (nz,ny,nx) float32 CUDA tensor."""
+    import torch
+    if y is None:
+        y = torch.empty((g.n_trans, g.nt), dtype=torch.float32, device=x.device)
+    _check(load().oat_project(g.handle, _dev_ptr(x, oat_num_voxels(g), "x", g),
+                              _dev_ptr(y, oat_num_samples(g), "y", g), _stream(stream)))
+    return y
+
+
+def oat_backproject(g, y, x=None, stream=None):
+    """x = H^T y on the current torch stream; y: (Q,K) float32 CUDA tensor."""
+    import torch
+    if x is None:
+        x = torch.empty(g.shape, dtype=torch.float32, device=y.device)
+    _check(load().oat_backproject(g.handle, _dev_ptr(y, oat_num_samples(g), "y", g),
+                                  _dev_ptr(x, oat_num_voxels(g), "x", g), _stream(stream)))
+    return x
+
+
+def oat_adjoint_check(g, x, y, stream=None):
+    """(lhs, rhs, rel) with lhs = <Hx, y>, rhs = <x, H^T y>."""
+    lhs, rhs, rel = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(load().oat_adjoint_check(g.handle, _dev_ptr(x, oat_num_voxels(g), "x", g),
+                                    _dev_ptr(y, oat_num_samples(g), "y", g),
+                                    ctypes.byref(lhs), ctypes.byref(rhs), ctypes.byref(rel), _stream(stream)))
+    return lhs.value, rhs.value, rel.value
+
+
+def _host_ptr(a, n, what):
+    """Host float32 buffer: a numpy array or a CPU torch tensor (pinned or pageable)."""
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float32 or not a.flags["C_CONTIGUOUS"] or a.size != n:
+            raise OatError(OAT_ERR_INVALID, f"{what} must be C-contiguous float32 with {n} elements")
+        return ctypes.c_void_p(a.ctypes.data)
+    import torch
+    if isinstance(a, torch.Tensor) and not a.is_cuda and a.dtype == torch.float32 and a.is_contiguous() and a.numel() == n:
+        return ctypes.c_void_p(a.data_ptr())
+    raise OatError(OAT_ERR_INVALID, f"{what} must be a host float32 buffer with {n} elements")
+
+
+def oat_project_host(g, h_x, h_y):
+    _check(load().oat_project_host(g.handle, _host_ptr(h_x, oat_num_voxels(g), "h_x"),
+                                   _host_ptr(h_y, oat_num_samples(g), "h_y")))
+    return h_y
+
+
+def oat_backproject_host(g, h_y, h_x):
+    _check(load().oat_backproject_host(g.handle, _host_ptr(h_y, oat_num_samples(g), "h_y"),
+                                       _host_ptr(h_x, oat_num_voxels(g), "h_x")))
+    return h_x
+
+
+def oat_cgls(g, y, n_iter, x=None, stream=None):
+    """n_iter CGLS steps from x = 0; returns (x, res, grad) with the two curves of length n_iter+1."""
+    import torch
+    if x is None:
+        x = torch.empty(g.shape, dtype=torch.float32, device=y.device)
+    res = np.zeros(n_iter + 1, dtype=np.float64)
+    grad = np.zeros(n_iter + 1, dtype=np.float64)
+    dp = ctypes.POINTER(ctypes.c_double)
+    _check(load().oat_cgls(g.handle, _dev_ptr(y, oat_num_samples(g), "y", g), _dev_ptr(x, oat_num_voxels(g), "x", g),
+                           int(n_iter), res.ctypes.data_as(dp), grad.ctypes.data_as(dp), _stream(stream)))
+    return x, res, grad
+
+
+def oat_set_variant(g, key: str, variant: int):
+    _check(load().oat_set_variant(g.handle, key.encode(), int(variant)))
+
+
+def oat_last_launch_count(g) -> int:
+    return int(load().oat_last_launch_count(g.handle))
+
+
+def oat_last_kernel_ms(g) -> float:
+    return float(load().oat_last_kernel_ms(g.handle))

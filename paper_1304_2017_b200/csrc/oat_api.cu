@@ -1,0 +1,492 @@
+// C ABI of liboat.so (include/oat.h): descriptor validation, host fp64 pre-computation of
+// per-transducer frames and per-band ring tables (step A1 of SURVEY.md §8(a)), scratch
+// management, and the operator entry points.  All hot work is in oat_kernels.cu.
+#include "../../include/oat.h"
+#include "oat_internal.h"
+
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                          \
+    do {                                                                                        \
+        cudaError_t e_ = (expr);                                                                \
+        if (e_ != cudaSuccess)                                                                  \
+            return fail(e_ == cudaErrorMemoryAllocation ? OAT_ERR_ALLOC : OAT_ERR_CUDA,         \
+                        "%s failed: %s", #expr, cudaGetErrorString(e_));                        \
+    } while (0)
+
+const double kPi = 3.14159265358979323846;
+
+}  // namespace
+
+struct oat_geometry {
+    oat_geometry_desc desc;
+    int device = 0;
+    double h = 0, kappa = 1;
+    OatDev dev;                               // kernel parameter block (device pointers inside)
+    // device tables
+    double *d_frame = nullptr;
+    OatBand *d_band = nullptr;
+    OatRing *d_ring = nullptr;
+    int *d_qb_rings = nullptr;
+    long long *d_item_prefix = nullptr;
+    // scratch
+    float *d_xpad = nullptr;                  // padded volume (gather source / scatter target)
+    double *d_g = nullptr;                    // Q*K SRT accumulator
+    float *d_y2 = nullptr, *d_x2 = nullptr;   // adjoint check / CGLS / host entry points (lazy)
+    float *d_x3 = nullptr, *d_y3 = nullptr, *d_x4 = nullptr;   // CGLS vectors (lazy)
+    double *d_scal = nullptr;                 // a few fp64 scalars (dots)
+    unsigned long long *d_counter = nullptr;
+    double *h_scal = nullptr;                 // pinned mirror of d_scal
+    long long n_surface_samples = -1;
+    int variant_project = 0, variant_backproject = 0;
+    int last_launches = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool ev_valid = false;
+    size_t n_vox = 0, n_dat = 0, n_pad = 0;
+};
+
+namespace {
+
+void free_all(oat_geometry *g)
+{
+    if (!g) return;
+    cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
+    cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
+    cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
+    cudaFree(g->d_counter);
+    if (g->h_scal) cudaFreeHost(g->h_scal);
+    if (g->ev0) cudaEventDestroy(g->ev0);
+    if (g->ev1) cudaEventDestroy(g->ev1);
+    delete g;
+}
+
+// Largest polar angle (about the axis transducer -> grid centre) at which a ray segment with
+// radius in [ra, rb] can meet the ball of radius R around the centre at distance L (S9; the paper's
+// theta'_max, Alg. 4, extended to a radius interval).  < 0: cannot meet.
+double band_theta_max(double L, double R, double ra, double rb)
+{
+    if (ra >= L + R || rb <= L - R) return -1.0;
+    if (ra <= R - L) return kPi;                          // a shell lies wholly inside the ball
+    // cos(theta_max(rho)) = f(rho) = (L^2 + rho^2 - R^2) / (2 rho L); minimise f over [ra, rb]
+    double rs = ra;
+    if (L > R) { rs = sqrt(L * L - R * R); if (rs < ra) rs = ra; if (rs > rb) rs = rb; }
+    const double cm = (L * L + rs * rs - R * R) / (2.0 * rs * L);
+    if (cm >= 1.0) return -1.0;
+    if (cm <= -1.0) return kPi;
+    return acos(cm);
+}
+
+template <class T>
+int upload(T **dst, const std::vector<T> &src)
+{
+    const size_t bytes = sizeof(T) * (src.size() ? src.size() : 1);
+    CUDA_TRY(cudaMalloc((void **)dst, bytes));
+    if (!src.empty()) CUDA_TRY(cudaMemcpy(*dst, src.data(), sizeof(T) * src.size(), cudaMemcpyHostToDevice));
+    return OAT_OK;
+}
+
+int ensure(float **p, size_t n)
+{
+    if (*p) return OAT_OK;
+    CUDA_TRY(cudaMalloc((void **)p, sizeof(float) * (n ? n : 1)));
+    return OAT_OK;
+}
+
+int build_geometry(oat_geometry *G)
+{
+    const oat_geometry_desc &d = G->desc;
+    const int B = d.kband > 0 ? d.kband : 32;
+    const int K = d.nt, Q = d.n_trans;
+    const int NB = (K + B - 1) / B;
+    G->h = d.surf_step > 0 ? d.surf_step : d.spacing;
+    G->kappa = d.gain != 0 ? d.gain : 1.0;
+    const double ds = d.spacing, h = G->h;
+    const int n[3] = {d.nx, d.ny, d.nz};
+    double C[3], r2 = 0;
+    for (int a = 0; a < 3; ++a) {
+        C[a] = d.origin[a] + ds * 0.5 * (n[a] - 1);
+        const double half = ds * (0.5 * (n[a] - 1) + 1.0);
+        r2 += half * half;
+    }
+    const double r_pad = sqrt(r2);
+
+    // ---- bands and rings (S2), fp64, same closed-form rule as the oracle (reading G19)
+    std::vector<OatBand> bands(NB);
+    std::vector<OatRing> rings;
+    for (int b = 0; b < NB; ++b) {
+        OatBand &bd = bands[b];
+        bd.k0 = b * B;
+        bd.nk = (K - bd.k0 < B) ? K - bd.k0 : B;
+        const int kref = bd.k0 + bd.nk - 1;
+        const double rho_ref = d.c * (d.t0 + kref * d.dt);
+        bd.s_mid = d.c * (d.t0 + (bd.k0 + 0.5 * (B - 1)) * d.dt) / ds;
+        bd.ring_ofs = (int)rings.size();
+        bd.n_rings = 0;
+        bd.dtheta = 0;
+        int kfirst = bd.k0;                                // first sample with rho > 0
+        while (kfirst <= kref && !(d.c * (d.t0 + kfirst * d.dt) > 0)) ++kfirst;
+        bd.s_lo = (float)(d.c * (d.t0 + kfirst * d.dt) / ds);
+        bd.s_hi = (float)(rho_ref / ds);
+        long long cum = 0;
+        if (rho_ref > 0 && kfirst <= kref) {
+            const double dtheta = h / rho_ref;             // Eq. 37
+            bd.dtheta = dtheta;
+            for (int i = 1;; ++i) {
+                const double theta = i * dtheta;           // Eq. 38
+                if (!(theta < kPi)) break;
+                OatRing r;
+                r.st = sin(theta);
+                r.ct = cos(theta);
+                double Nd = ceil(2.0 * kPi * rho_ref * r.st / h);
+                if (Nd < 1) Nd = 1;
+                if (cum + (long long)Nd > 0x7fffffffLL) return fail(OAT_ERR_INVALID, "too many directions in one band (surf_step too small)");
+                r.N = (int)Nd;
+                r.omega = (float)(r.st * dtheta * (2.0 * kPi / Nd));
+                r.cum = (int)cum;
+                r.pad = 0;
+                cum += r.N;
+                rings.push_back(r);
+                ++bd.n_rings;
+            }
+        }
+        OatRing sentinel;
+        sentinel.st = 0; sentinel.ct = 1; sentinel.omega = 0; sentinel.N = 1; sentinel.cum = (int)cum; sentinel.pad = 0;
+        rings.push_back(sentinel);
+    }
+
+    // ---- frames (S1) and the per-(q, band) ring bound (S9) + work-item prefix
+    std::vector<double> frame((size_t)Q * 12);
+    std::vector<int> qb_rings((size_t)Q * NB);
+    std::vector<long long> prefix((size_t)Q * NB + 1);
+    long long items = 0;
+    for (int q = 0; q < Q; ++q) {
+        const double *rq = d.trans_xyz + 3 * (size_t)q;
+        double v[3] = {C[0] - rq[0], C[1] - rq[1], C[2] - rq[2]};
+        const double L = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+        if (!(L > 0) || !isfinite(L)) return fail(OAT_ERR_INVALID, "transducer %d is at the grid centre or not finite", q);
+        double ez[3] = {v[0] / L, v[1] / L, v[2] / L};
+        double ey[3] = {ez[1], -ez[0], 0.0};               // e_z x z^
+        const double an = sqrt(ey[0] * ey[0] + ey[1] * ey[1]);
+        if (an < 1e-12) { ey[0] = 0; ey[1] = 1; ey[2] = 0; }
+        else { ey[0] /= an; ey[1] /= an; }
+        const double ex[3] = {ey[1] * ez[2] - ey[2] * ez[1], ey[2] * ez[0] - ey[0] * ez[2], ey[0] * ez[1] - ey[1] * ez[0]};
+        double *f = &frame[(size_t)q * 12];
+        for (int a = 0; a < 3; ++a) {
+            f[a] = ex[a]; f[3 + a] = ey[a]; f[6 + a] = ez[a];
+            f[9 + a] = (rq[a] - d.origin[a]) / ds + 1.0;   // padded fractional node coordinates
+        }
+        for (int b = 0; b < NB; ++b) {
+            const OatBand &bd = bands[b];
+            int nr = 0;
+            if (bd.n_rings > 0) {
+                const double th = band_theta_max(L, r_pad, (double)bd.s_lo * ds * (1 - 1e-6), (double)bd.s_hi * ds * (1 + 1e-6));
+                if (th >= 0) {
+                    const double cnt = floor(th / bd.dtheta) + 1.0;     // rings with theta_i <= th, +1 margin
+                    nr = cnt < bd.n_rings ? (int)cnt : bd.n_rings;
+                }
+            }
+            qb_rings[(size_t)q * NB + b] = nr;
+            prefix[(size_t)q * NB + b] = items;
+            const long long cand = rings[bd.ring_ofs + nr].cum;
+            items += (cand + OAT_CH - 1) / OAT_CH;
+        }
+    }
+    prefix[(size_t)Q * NB] = items;
+
+    // ---- upload
+    int rc;
+    if ((rc = upload(&G->d_frame, frame))) return rc;
+    if ((rc = upload(&G->d_band, bands))) return rc;
+    if ((rc = upload(&G->d_ring, rings))) return rc;
+    if ((rc = upload(&G->d_qb_rings, qb_rings))) return rc;
+    if ((rc = upload(&G->d_item_prefix, prefix))) return rc;
+
+    OatDev &P = G->dev;
+    P.nx = d.nx; P.ny = d.ny; P.nz = d.nz;
+    P.px = ((d.nx + 2 + 7) / 8) * 8;                       // rows start on 32-byte sectors
+    P.py = d.ny + 2; P.pz = d.nz + 2;
+    P.pxy = (long long)P.px * P.py;
+    P.Q = Q; P.K = K; P.B = B; P.NB = NB;
+    P.c = d.c; P.t0 = d.t0; P.dt = d.dt; P.kappa = G->kappa;
+    P.step = d.c * d.dt / ds;
+    P.frame = G->d_frame; P.band = G->d_band; P.ring = G->d_ring;
+    P.qb_rings = G->d_qb_rings; P.item_prefix = G->d_item_prefix;
+    P.n_items = items;
+
+    G->n_vox = (size_t)d.nx * d.ny * d.nz;
+    G->n_dat = (size_t)Q * K;
+    G->n_pad = (size_t)P.pz * P.pxy;
+    CUDA_TRY(cudaMalloc((void **)&G->d_xpad, sizeof(float) * G->n_pad));
+    CUDA_TRY(cudaMalloc((void **)&G->d_g, sizeof(double) * (G->n_dat ? G->n_dat : 1)));
+    CUDA_TRY(cudaMalloc((void **)&G->d_scal, sizeof(double) * 8));
+    CUDA_TRY(cudaMalloc((void **)&G->d_counter, sizeof(unsigned long long)));
+    CUDA_TRY(cudaMallocHost((void **)&G->h_scal, sizeof(double) * 8));
+    CUDA_TRY(cudaEventCreate(&G->ev0));
+    CUDA_TRY(cudaEventCreate(&G->ev1));
+    return OAT_OK;
+}
+
+int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
+{
+    const OatDev &P = G->dev;
+    G->last_launches = 0;
+    oat_launch_pad(P, d_x, G->d_xpad, st); ++G->last_launches;
+    CUDA_TRY(cudaMemsetAsync(G->d_g, 0, sizeof(double) * (G->n_dat ? G->n_dat : 1), st));
+    CUDA_TRY(cudaEventRecord(G->ev0, st));
+    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(0, P, G->d_xpad, nullptr, nullptr, G->d_g, nullptr, st)); ++G->last_launches; }
+    CUDA_TRY(cudaEventRecord(G->ev1, st));
+    G->ev_valid = true;
+    if (G->n_dat > 0) { oat_launch_diff(P, G->d_g, d_y, st); ++G->last_launches; }
+    CUDA_TRY(cudaGetLastError());
+    return OAT_OK;
+}
+
+int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t st)
+{
+    const OatDev &P = G->dev;
+    G->last_launches = 0;
+    CUDA_TRY(cudaMemsetAsync(G->d_xpad, 0, sizeof(float) * G->n_pad, st));
+    CUDA_TRY(cudaEventRecord(G->ev0, st));
+    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(1, P, nullptr, G->d_xpad, d_y, nullptr, nullptr, st)); ++G->last_launches; }
+    CUDA_TRY(cudaEventRecord(G->ev1, st));
+    G->ev_valid = true;
+    oat_launch_unpad(P, G->d_xpad, d_x, st); ++G->last_launches;
+    CUDA_TRY(cudaGetLastError());
+    return OAT_OK;
+}
+
+int dot_sync(oat_geometry *G, const float *a, const float *b, size_t n, double *out, cudaStream_t st)
+{
+    CUDA_TRY(cudaMemsetAsync(G->d_scal, 0, sizeof(double), st));
+    oat_launch_dot(a, b, (long long)n, G->d_scal, st);
+    CUDA_TRY(cudaMemcpyAsync(G->h_scal, G->d_scal, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    *out = G->h_scal[0];
+    return OAT_OK;
+}
+
+int check_handle(const oat_geometry *g)
+{
+    if (!g) return fail(OAT_ERR_INVALID, "geometry handle is NULL");
+    cudaError_t e = cudaSetDevice(g->device);
+    if (e != cudaSuccess) return fail(OAT_ERR_CUDA, "cudaSetDevice(%d) failed: %s", g->device, cudaGetErrorString(e));
+    return OAT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int oat_geometry_create(const oat_geometry_desc *desc, int device, oat_geometry **out)
+{
+    if (!desc || !out) return fail(OAT_ERR_INVALID, "desc and out must not be NULL");
+    if (desc->nx < 1 || desc->ny < 1 || desc->nz < 1) return fail(OAT_ERR_INVALID, "grid sizes must be >= 1");
+    if ((long long)desc->nx * desc->ny * desc->nz > (1LL << 40)) return fail(OAT_ERR_INVALID, "grid too large");
+    if (desc->n_trans < 0 || desc->nt < 1) return fail(OAT_ERR_INVALID, "n_trans must be >= 0 and nt >= 1");
+    if (!(desc->spacing > 0) || !(desc->c > 0) || !(desc->dt > 0) || !(desc->t0 >= 0))
+        return fail(OAT_ERR_INVALID, "spacing, c, dt must be > 0 and t0 >= 0");
+    if (!isfinite(desc->spacing) || !isfinite(desc->c) || !isfinite(desc->dt) || !isfinite(desc->t0))
+        return fail(OAT_ERR_INVALID, "non-finite scalar in descriptor");
+    if (desc->surf_step < 0 || !isfinite(desc->surf_step)) return fail(OAT_ERR_INVALID, "surf_step must be >= 0");
+    if (desc->kband < 0 || desc->kband > 32) return fail(OAT_ERR_INVALID, "kband must be in 0..32");
+    if (!isfinite(desc->gain)) return fail(OAT_ERR_INVALID, "gain must be finite");
+    if (desc->n_trans > 0 && !desc->trans_xyz) return fail(OAT_ERR_INVALID, "trans_xyz is NULL");
+    for (int a = 0; a < 3; ++a)
+        if (!isfinite(desc->origin[a])) return fail(OAT_ERR_INVALID, "origin must be finite");
+    for (long long i = 0; i < 3LL * desc->n_trans; ++i)
+        if (!isfinite(desc->trans_xyz[i])) return fail(OAT_ERR_INVALID, "transducer %lld has a non-finite coordinate", i / 3);
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev <= 0)
+        return fail(OAT_ERR_CUDA, "no CUDA device (%s); liboat has no CPU fallback", e != cudaSuccess ? cudaGetErrorString(e) : "count = 0");
+    if (device < 0 || device >= ndev) return fail(OAT_ERR_INVALID, "device %d out of range (0..%d)", device, ndev - 1);
+    CUDA_TRY(cudaSetDevice(device));
+
+    oat_geometry *G = new (std::nothrow) oat_geometry();
+    if (!G) return fail(OAT_ERR_ALLOC, "out of host memory");
+    G->desc = *desc;
+    G->device = device;
+    std::vector<double> tr_copy;
+    try {
+        tr_copy.assign(desc->trans_xyz, desc->trans_xyz + 3 * (size_t)desc->n_trans);
+    } catch (...) { delete G; return fail(OAT_ERR_ALLOC, "out of host memory"); }
+    G->desc.trans_xyz = tr_copy.data();
+    int rc;
+    try { rc = build_geometry(G); }
+    catch (const std::bad_alloc &) { rc = fail(OAT_ERR_ALLOC, "out of host memory while building tables"); }
+    G->desc.trans_xyz = nullptr;                           // the copy lives on the device (frames) only
+    if (rc) { free_all(G); return rc; }
+    *out = G;
+    return OAT_OK;
+}
+
+void oat_geometry_destroy(oat_geometry *geom)
+{
+    if (!geom) return;
+    cudaSetDevice(geom->device);
+    free_all(geom);
+}
+
+int64_t oat_num_voxels(const oat_geometry *g) { return g ? (int64_t)g->n_vox : -1; }
+int64_t oat_num_samples(const oat_geometry *g) { return g ? (int64_t)g->n_dat : -1; }
+
+int64_t oat_num_surface_samples(oat_geometry *g)
+{
+    if (check_handle(g)) return -1;
+    if (g->n_surface_samples >= 0) return g->n_surface_samples;
+    if (cudaMemset(g->d_counter, 0, sizeof(unsigned long long)) != cudaSuccess) return -1;
+    if (oat_launch_ray(2, g->dev, nullptr, nullptr, nullptr, nullptr, g->d_counter, 0) != cudaSuccess) return -1;
+    unsigned long long v = 0;
+    if (cudaMemcpy(&v, g->d_counter, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) {
+        fail(OAT_ERR_CUDA, "sample count kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return -1;
+    }
+    g->n_surface_samples = (long long)v;
+    return g->n_surface_samples;
+}
+
+int oat_project(oat_geometry *g, const float *d_x, float *d_y, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_x || (!d_y && g->n_dat)) return fail(OAT_ERR_INVALID, "d_x / d_y must not be NULL");
+    return project_impl(g, d_x, d_y, (cudaStream_t)stream);
+}
+
+int oat_backproject(oat_geometry *g, const float *d_y, float *d_x, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_x || (!d_y && g->n_dat)) return fail(OAT_ERR_INVALID, "d_x / d_y must not be NULL");
+    return backproject_impl(g, d_y, d_x, (cudaStream_t)stream);
+}
+
+int oat_adjoint_check(oat_geometry *g, const float *d_x, const float *d_y, double *lhs, double *rhs, double *rel, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_x || !d_y || !lhs || !rhs || !rel) return fail(OAT_ERR_INVALID, "NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = ensure(&g->d_y2, g->n_dat))) return rc;
+    if ((rc = ensure(&g->d_x2, g->n_vox))) return rc;
+    if ((rc = project_impl(g, d_x, g->d_y2, st))) return rc;
+    if ((rc = dot_sync(g, g->d_y2, d_y, g->n_dat, lhs, st))) return rc;
+    if ((rc = backproject_impl(g, d_y, g->d_x2, st))) return rc;
+    if ((rc = dot_sync(g, d_x, g->d_x2, g->n_vox, rhs, st))) return rc;
+    const double m = fmax(fabs(*lhs), fabs(*rhs));
+    *rel = m > 0 ? fabs(*lhs - *rhs) / m : 0.0;
+    return OAT_OK;
+}
+
+int oat_project_host(oat_geometry *g, const float *h_x, float *h_y)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!h_x || (!h_y && g->n_dat)) return fail(OAT_ERR_INVALID, "h_x / h_y must not be NULL");
+    if ((rc = ensure(&g->d_y2, g->n_dat))) return rc;
+    if ((rc = ensure(&g->d_x2, g->n_vox))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(g->d_x2, h_x, sizeof(float) * g->n_vox, cudaMemcpyHostToDevice, 0));
+    if ((rc = project_impl(g, g->d_x2, g->d_y2, 0))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(h_y, g->d_y2, sizeof(float) * g->n_dat, cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(cudaStreamSynchronize(0));
+    return OAT_OK;
+}
+
+int oat_backproject_host(oat_geometry *g, const float *h_y, float *h_x)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!h_x || (!h_y && g->n_dat)) return fail(OAT_ERR_INVALID, "h_x / h_y must not be NULL");
+    if ((rc = ensure(&g->d_y2, g->n_dat))) return rc;
+    if ((rc = ensure(&g->d_x2, g->n_vox))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(g->d_y2, h_y, sizeof(float) * g->n_dat, cudaMemcpyHostToDevice, 0));
+    if ((rc = backproject_impl(g, g->d_y2, g->d_x2, 0))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(h_x, g->d_x2, sizeof(float) * g->n_vox, cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(cudaStreamSynchronize(0));
+    return OAT_OK;
+}
+
+// Row C1: CGLS (reading G15).  r = y - Hx; s = H^T r; p = s; loop { q = Hp; alpha = |s|^2/|q|^2;
+// x += alpha p; r -= alpha q; s = H^T r; beta = |s|^2_new/|s|^2_old; p = s + beta p }
+int oat_cgls(oat_geometry *g, const float *d_y, float *d_x, int n_iter, double *h_res, double *h_grad, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_y || !d_x || n_iter < 0) return fail(OAT_ERR_INVALID, "bad argument to oat_cgls");
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = ensure(&g->d_y2, g->n_dat))) return rc;     // r
+    if ((rc = ensure(&g->d_y3, g->n_dat))) return rc;     // q
+    if ((rc = ensure(&g->d_x3, g->n_vox))) return rc;     // s
+    if ((rc = ensure(&g->d_x4, g->n_vox))) return rc;     // p
+    float *r = g->d_y2, *qv = g->d_y3, *s = g->d_x3, *p = g->d_x4;
+    CUDA_TRY(cudaMemsetAsync(d_x, 0, sizeof(float) * g->n_vox, st));
+    CUDA_TRY(cudaMemcpyAsync(r, d_y, sizeof(float) * g->n_dat, cudaMemcpyDeviceToDevice, st));
+    if ((rc = backproject_impl(g, r, s, st))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(p, s, sizeof(float) * g->n_vox, cudaMemcpyDeviceToDevice, st));
+    double gamma, ynorm2, rr;
+    if ((rc = dot_sync(g, s, s, g->n_vox, &gamma, st))) return rc;
+    if ((rc = dot_sync(g, d_y, d_y, g->n_dat, &ynorm2, st))) return rc;
+    const double ynorm = sqrt(ynorm2);
+    if (h_res) h_res[0] = ynorm > 0 ? 1.0 : 0.0;
+    if (h_grad) h_grad[0] = sqrt(gamma);
+    for (int it = 0; it < n_iter; ++it) {
+        double qq;
+        if ((rc = project_impl(g, p, qv, st))) return rc;
+        if ((rc = dot_sync(g, qv, qv, g->n_dat, &qq, st))) return rc;
+        if (qq > 0 && gamma > 0) {
+            const double alpha = gamma / qq;
+            oat_launch_axpy((float)alpha, p, d_x, (long long)g->n_vox, st);
+            oat_launch_axpy((float)-alpha, qv, r, (long long)g->n_dat, st);
+            if ((rc = backproject_impl(g, r, s, st))) return rc;
+            double gamma_new;
+            if ((rc = dot_sync(g, s, s, g->n_vox, &gamma_new, st))) return rc;
+            const double beta = gamma_new / gamma;
+            gamma = gamma_new;
+            oat_launch_xpay(s, (float)beta, p, (long long)g->n_vox, st);
+        }
+        if (h_res) {
+            if ((rc = dot_sync(g, r, r, g->n_dat, &rr, st))) return rc;
+            h_res[it + 1] = ynorm > 0 ? sqrt(rr) / ynorm : 0.0;
+        }
+        if (h_grad) h_grad[it + 1] = sqrt(gamma);
+    }
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return OAT_OK;
+}
+
+int oat_set_variant(oat_geometry *g, const char *key, int variant)
+{
+    if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");
+    if (!strcmp(key, "project")) { if (variant != 0) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
+    if (!strcmp(key, "backproject")) { if (variant != 0) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
+    return fail(OAT_ERR_INVALID, "unknown variant key '%s'", key);
+}
+
+int oat_last_launch_count(const oat_geometry *g) { return g ? g->last_launches : -1; }
+
+float oat_last_kernel_ms(oat_geometry *g)
+{
+    if (check_handle(g) || !g->ev_valid) return -1.f;
+    if (cudaEventSynchronize(g->ev1) != cudaSuccess) return -1.f;
+    float ms = -1.f;
+    if (cudaEventElapsedTime(&ms, g->ev0, g->ev1) != cudaSuccess) return -1.f;
+    return ms;
+}
+
+const char *oat_last_error(void) { return g_err; }
+const char *oat_version(void) { return "oat-b200 0.1 (OAT-DISC v1; sm_100a)"; }
+
+}  // extern "C"

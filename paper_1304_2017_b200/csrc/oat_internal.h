@@ -1,0 +1,65 @@
+// Internal declarations of liboat.so (not part of the C ABI; see include/oat.h).
+//
+// Data layout in HBM:
+//   frame   Q x 12 fp64   e_x, e_y, e_z (Appendix, reading S1) and base' = (r_q - o)/ds + 1,
+//                         the transducer position in PADDED fractional node coordinates
+//   band    NB            per band of B time samples: reference radius, dtheta, ring-table slice
+//   ring    sum(n_rings+1) per band, rings i = 1..n_rings with theta_i = i*dtheta < pi, plus a
+//                         sentinel whose `cum` is the band's total direction count
+//   qb_rings Q x NB       number of leading rings that can reach the padded box (S9 cull)
+//   item_prefix Q*NB+1    exclusive prefix of work items (chunks of OAT_CH candidate directions)
+//   xpad    (nz+2)(ny+2)(px) fp32  volume zero-padded by one node on every side = Eq. (12)'s
+//                         "nodes outside the grid do not exist" (reading G5), row pitch px
+//   g       Q x K fp64    SRT accumulator (forward) before the time difference
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define OAT_CH 8192        // candidate directions per work item
+#define OAT_SB 1024        // candidates per shared-memory sub-batch
+#define OAT_NT 256         // threads per block of the ray kernels
+#define OAT_NW (OAT_NT / 32)
+
+struct OatBand {
+    double s_mid;      // radius of the band's anchor (k0 + (B-1)/2) in voxel units: rho/ds
+    double dtheta;     // h / rho_ref (Eq. 37), rho_ref = radius of the band's last sample (S2)
+    float s_lo, s_hi;  // radii (voxel units) of the first / last sample with rho > 0
+    int ring_ofs;      // first ring of this band in the ring table
+    int n_rings;       // rings with theta_i < pi
+    int k0, nk;        // first sample and number of samples (ragged last band: nk < B)
+};
+
+struct __align__(16) OatRing {
+    double st, ct;     // sin(theta_i), cos(theta_i)
+    float omega;       // solid-angle weight sin(theta_i) dtheta dphi_i (S2)
+    int N;             // azimuth count N_{b,i} = max(1, ceil(2 pi rho_ref sin(theta_i) / h))
+    int cum;           // directions in rings before this one
+    int pad;
+};
+
+struct OatDev {
+    int nx, ny, nz;            // nodes
+    int px, py, pz;            // padded dims: px = row pitch >= nx+2, py = ny+2, pz = nz+2
+    long long pxy;             // px*py
+    int Q, K, B, NB;
+    double c, t0, dt, kappa;
+    double step;               // c*dt/ds: voxels per time sample along a ray
+    const double *frame;
+    const OatBand *band;
+    const OatRing *ring;
+    const int *qb_rings;
+    const long long *item_prefix;
+    long long n_items;
+};
+
+// launchers (oat_kernels.cu); all asynchronous on `st`
+void oat_launch_pad(const OatDev &P, const float *x, float *xpad, cudaStream_t st);
+void oat_launch_unpad(const OatDev &P, const float *xpad, float *x, cudaStream_t st);
+// mode 0: g += G x (gathers from xpad); 1: xacc += G^T D^T y (scatter); 2: count in-box samples
+cudaError_t oat_launch_ray(int mode, const OatDev &P, const float *xpad, float *xacc, const float *y,
+                           double *g, unsigned long long *counter, cudaStream_t st);
+void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st);
+// vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)
+void oat_launch_dot(const float *a, const float *b, long long n, double *out, cudaStream_t st);
+void oat_launch_axpy(float alpha, const float *x, float *y, long long n, cudaStream_t st);   // y += alpha x
+void oat_launch_xpay(const float *x, float beta, float *y, long long n, cudaStream_t st);    // y = x + beta y

@@ -1,0 +1,248 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the thin binding) against the fp64
+oracle, element by element, on the same seeded inputs.
+
+Tolerances (north_star): rel-L2 <= 1e-4 for H and for H^T, adjoint mismatch <= 1e-4.
+The path computes in fp32 with an fp64 final combine; the oracle in fp64.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from oracle import oat_oracle as orc
+    from paper_1304_2017_b200 import binding as oat, build, workloads as wl
+    build.build()
+    assert torch.cuda.is_available()
+    return torch, orc, oat, wl
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    nb = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / nb) if nb > 0 else float(np.linalg.norm(a))
+
+
+def gpu_project(torch, oat, w, x, g=None):
+    own = g is None
+    g = g or oat.oat_geometry_create(w)
+    y = oat.oat_project(g, torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).cuda())
+    torch.cuda.synchronize()
+    out = y.cpu().numpy()
+    if own:
+        g.close()
+    return out
+
+
+def gpu_backproject(torch, oat, w, y, g=None):
+    own = g is None
+    g = g or oat.oat_geometry_create(w)
+    x = oat.oat_backproject(g, torch.from_numpy(np.ascontiguousarray(y, dtype=np.float32)).cuda())
+    torch.cuda.synchronize()
+    out = x.cpu().numpy()
+    if own:
+        g.close()
+    return out
+
+
+def check_pair(env, w, x=None, y=None, tol=TOL):
+    torch, orc, oat, wl = env
+    x = w.phantom() if x is None else x
+    y = w.data_noise() if y is None else y
+    g = oat.oat_geometry_create(w)
+    hx = gpu_project(torch, oat, w, x, g)
+    hty = gpu_backproject(torch, oat, w, y, g)
+    ref_hx = orc.project(w, x.astype(np.float64))
+    ref_hty = orc.backproject(w, y.astype(np.float64))
+    e1, e2 = rel_l2(hx, ref_hx), rel_l2(hty, ref_hty)
+    assert e1 <= tol, f"H rel-L2 {e1:.3e}"
+    assert e2 <= tol, f"H^T rel-L2 {e2:.3e}"
+    # element by element: no single output is off by more than a few 1e-4 of the vector's scale
+    assert np.max(np.abs(hx - ref_hx)) <= 10 * tol * np.max(np.abs(ref_hx))
+    assert np.max(np.abs(hty - ref_hty)) <= 10 * tol * np.max(np.abs(ref_hty))
+    lhs, rhs, rel = oat.oat_adjoint_check(g, torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda())
+    assert rel <= tol, f"adjoint mismatch {rel:.3e}"
+    assert abs(lhs - float(np.vdot(ref_hx, y))) <= 10 * tol * abs(lhs) + 1e-12
+    # in-box sample count (integer work): equal up to samples that sit exactly on the padded-box faces
+    cnt, ref_cnt = oat.oat_num_surface_samples(g), orc.count_samples(w)
+    assert abs(cnt - ref_cnt) <= max(2, 1e-6 * ref_cnt), (cnt, ref_cnt)
+    g.close()
+    return e1, e2, rel
+
+
+# ------------------------------------------------------------------ small, ragged, several band widths
+@pytest.mark.parametrize("kband,nt", [(32, 70), (8, 37), (1, 20), (5, 33)])
+def test_small_problems(env, kband, nt):
+    torch, orc, oat, wl = env
+    w = wl.small(n=14, q=5, nt=nt, kband=kband)            # nt not a multiple of kband: ragged last band
+    check_pair(env, w)
+
+
+def test_non_cubic_grid_and_offset_origin(env):
+    torch, orc, oat, wl = env
+    tr = np.array([[25.0, 3.0, -4.0], [-6.0, -22.0, 9.0], [2.0, 5.0, 27.0], [-14.0, 11.0, -19.0]])
+    w = wl.Workload("noncubic", 21, 13, 9, 0.4, (-3.7, -2.1, -1.3), tr, c=1.5, t0=9.0, dt=0.06, nt=150,
+                    surf_step=0.3, kband=32, gain=0.5)
+    rng = np.random.default_rng(4)
+    x = rng.random((w.nz, w.ny, w.nx)).astype(np.float32)
+    check_pair(env, w, x=x)
+
+
+def test_config1_tiny_full(env):
+    """BASELINE.json config 1: one H, one H^T, adjoint test with seeded N(0,1) y."""
+    torch, orc, oat, wl = env
+    w = wl.config(1)
+    e1, e2, rel = check_pair(env, w)
+    print(f"config1: H {e1:.2e}  H^T {e2:.2e}  adjoint {rel:.2e}")
+
+
+def test_dense_columns_and_rows_match_oracle(env):
+    """P5 on the GPU: columns H e_n and rows H^T e_m of a tiny problem against the oracle's."""
+    torch, orc, oat, wl = env
+    tr = np.array([[6.0, 1.0, 2.0], [-1.5, -5.0, 4.0]])
+    w = wl.Workload("tiny", 5, 4, 3, 0.5, (-1.0, -0.75, -0.5), tr, c=1.5, t0=2.6, dt=0.1, nt=22,
+                    surf_step=0.4, kband=4, gain=1.0)
+    g = oat.oat_geometry_create(w)
+    N, m = w.n_voxels, w.n_trans * w.nt
+    cols = np.stack([gpu_project(torch, oat, w, np.eye(N, dtype=np.float32)[n].reshape(w.nz, w.ny, w.nx), g).ravel() for n in range(N)], axis=1)
+    rows = np.stack([gpu_backproject(torch, oat, w, np.eye(m, dtype=np.float32)[i].reshape(w.n_trans, w.nt), g).ravel() for i in range(m)], axis=0)
+    M = np.stack([orc.project(w, np.eye(N)[n].reshape(w.nz, w.ny, w.nx)).ravel() for n in range(N)], axis=1)
+    scale = np.abs(M).max()
+    assert np.abs(cols - M).max() <= 1e-5 * scale
+    assert np.abs(rows - M).max() <= 1e-5 * scale
+    g.close()
+
+
+# ------------------------------------------------------------------ edge cases
+def test_shells_that_miss_the_grid_and_empty_inputs(env):
+    torch, orc, oat, wl = env
+    tr = np.array([[30.0, 0.0, 0.0]])
+    w = wl.Workload("miss", 8, 8, 8, 0.5, (-1.75, -1.75, -1.75), tr, c=1.5, t0=0.0, dt=0.5, nt=12, surf_step=0.5, kband=32)
+    x = np.ones((8, 8, 8), dtype=np.float32)
+    assert np.all(gpu_project(torch, oat, w, x) == 0.0)
+    assert np.all(gpu_backproject(torch, oat, w, np.ones((1, 12), dtype=np.float32)) == 0.0)
+    w0 = wl.Workload("noq", 8, 8, 8, 0.5, (-1.75, -1.75, -1.75), np.zeros((0, 3)), c=1.5, t0=1.0, dt=0.5, nt=12, surf_step=0.5)
+    g = oat.oat_geometry_create(w0)
+    assert oat.oat_num_samples(g) == 0 and oat.oat_num_voxels(g) == 512
+    xb = oat.oat_backproject(g, torch.zeros((0, 12), device="cuda"))
+    torch.cuda.synchronize()
+    assert xb.shape == (8, 8, 8) and float(xb.abs().max()) == 0.0
+    assert oat.oat_num_surface_samples(g) == 0
+    g.close()
+
+
+def test_transducer_inside_the_grid_t0_zero_and_single_sample(env):
+    torch, orc, oat, wl = env
+    tr = np.array([[0.6, -0.3, 0.2], [9.0, 0.0, 0.0]])
+    w = wl.Workload("inside", 16, 16, 16, 0.5, (-3.75, -3.75, -3.75), tr, c=1.5, t0=0.0, dt=0.2, nt=40, surf_step=0.25, kband=8)
+    rng = np.random.default_rng(8)
+    check_pair(env, w, x=rng.random((16, 16, 16)).astype(np.float32))
+    w1 = wl.Workload("nt1", 10, 10, 10, 0.5, (-2.25, -2.25, -2.25), np.array([[7.0, 1.0, 0.5]]), c=1.5, t0=4.5, dt=0.1, nt=1, surf_step=0.5, kband=32)
+    # K = 1: D has only zero-extended neighbours, so H x = 0 exactly and H^T y = 0
+    assert np.all(gpu_project(torch, oat, w1, np.ones((10, 10, 10), dtype=np.float32)) == 0.0)
+    assert np.all(gpu_backproject(torch, oat, w1, np.ones((1, 1), dtype=np.float32)) == 0.0)
+
+
+def test_argument_errors(env):
+    torch, orc, oat, wl = env
+    w = wl.small()
+    g = oat.oat_geometry_create(w)
+    with pytest.raises(oat.OatError):
+        oat.oat_project(g, torch.zeros(5, device="cuda"))
+    with pytest.raises(oat.OatError):
+        oat.oat_project(g, torch.zeros((w.nz, w.ny, w.nx), dtype=torch.float64, device="cuda"))
+    with pytest.raises(oat.OatError):
+        oat.oat_backproject(g, torch.zeros((w.n_trans, w.nt)))            # host tensor
+    with pytest.raises(oat.OatError):
+        oat.oat_geometry_create(wl.Workload("c", 8, 8, 8, 0.5, (-1.75,) * 3, np.zeros((1, 3)), c=1.5, t0=1, dt=0.1, nt=4, surf_step=0.5))
+    with pytest.raises(oat.OatError):
+        oat.oat_set_variant(g, "project", 99)
+    # repeated create / destroy
+    for _ in range(5):
+        oat.oat_geometry_create(w).close()
+    g.close()
+
+
+def test_stream_ordering_and_overwrite(env):
+    """y is overwritten (not accumulated); calls on a side stream are ordered with its other work."""
+    torch, orc, oat, wl = env
+    w = wl.small(n=12, q=3, nt=40, kband=8)
+    g = oat.oat_geometry_create(w)
+    x = torch.from_numpy(w.phantom()).cuda()
+    y1 = oat.oat_project(g, x).clone()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        y2 = torch.full((w.n_trans, w.nt), 7.0, device="cuda")
+        x2 = x * 2.0                                                       # produced on s, consumed by the call on s
+        oat.oat_project(g, x2, y2)
+        y2h = (y2 / 2.0)
+    s.synchronize()
+    assert torch.allclose(y2h, y1, rtol=1e-5, atol=1e-6 * float(y1.abs().max()))
+    xb = torch.full((w.nz, w.ny, w.nx), 3.0, device="cuda")
+    ydat = torch.from_numpy(w.data_noise()).cuda()
+    oat.oat_backproject(g, ydat, xb)
+    xb2 = oat.oat_backproject(g, ydat)
+    torch.cuda.synchronize()
+    assert torch.allclose(xb, xb2, rtol=1e-4, atol=1e-5 * float(xb2.abs().max()))
+    g.close()
+
+
+def test_host_entry_points(env):
+    torch, orc, oat, wl = env
+    w = wl.small(n=12, q=3, nt=40, kband=8)
+    g = oat.oat_geometry_create(w)
+    x = w.phantom(); y = w.data_noise()
+    hy = np.empty((w.n_trans, w.nt), dtype=np.float32)
+    hx = torch.empty((w.nz, w.ny, w.nx), dtype=torch.float32).pin_memory()
+    oat.oat_project_host(g, x, hy)
+    oat.oat_backproject_host(g, y, hx)
+    assert rel_l2(hy, orc.project(w, x.astype(np.float64))) <= TOL
+    assert rel_l2(hx.numpy(), orc.backproject(w, y.astype(np.float64))) <= TOL
+    g.close()
+
+
+# ------------------------------------------------------------------ larger configs
+def test_config2_transducer_subset(env):
+    """BASELINE.json config 2 on a seeded subset of 16 transducers (rows of H are independent;
+    H^T is a sum over transducers)."""
+    torch, orc, oat, wl = env
+    w = wl.config(2)
+    idx, ws = w.seeded_subset(16)
+    x = w.phantom()
+    y = ws.data_noise()
+    g = oat.oat_geometry_create(ws)
+    hx = gpu_project(torch, oat, ws, x, g)
+    hty = gpu_backproject(torch, oat, ws, y, g)
+    g.close()
+    e1 = rel_l2(hx, orc.project(ws, x.astype(np.float64)))
+    e2 = rel_l2(hty, orc.backproject(ws, y.astype(np.float64)))
+    print(f"config2[16]: H {e1:.2e}  H^T {e2:.2e}")
+    assert e1 <= TOL and e2 <= TOL
+
+
+def test_config4_cgls_first_iterations(env):
+    """Row C1: first 3 CGLS iterations on a config-2-shaped problem (reduced transducer count so the
+    oracle finishes in seconds) against the oracle's CGLS; residual curve must match."""
+    torch, orc, oat, wl = env
+    w = wl.config(4)
+    idx, ws = w.seeded_subset(6)
+    xt = w.phantom()
+    ytrue = orc.project(ws, xt.astype(np.float64))
+    rng = np.random.default_rng(4)
+    y = (ytrue + rng.standard_normal(ytrue.shape) * 0.05 * np.abs(ytrue).max()).astype(np.float32)
+    g = oat.oat_geometry_create(ws)
+    x, res, grad = oat.oat_cgls(g, torch.from_numpy(y).cuda(), 3)
+    xo, reso, grado = orc.cgls(ws, y.astype(np.float64), 3)
+    assert np.allclose(res, reso, rtol=2e-4, atol=1e-7)
+    assert np.allclose(grad, grado, rtol=2e-3)
+    assert rel_l2(x.cpu().numpy(), xo) <= 5e-4
+    assert np.all(np.diff(res) <= 1e-6)
+    g.close()
