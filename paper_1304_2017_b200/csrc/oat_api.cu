@@ -57,7 +57,10 @@ struct oat_geometry {
     unsigned long long *d_counter = nullptr;
     double *h_scal = nullptr;                 // pinned mirror of d_scal
     long long n_surface_samples = -1;
-    int variant_project = 0, variant_backproject = 0;
+    int variant_project = 0, variant_backproject = 1;
+    cudaArray_t atlas = nullptr;              // slice atlas for the texture-gather projection (lazy)
+    cudaTextureObject_t tex = 0;
+    cudaSurfaceObject_t surf = 0;
     int last_launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool ev_valid = false;
@@ -73,6 +76,9 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
     cudaFree(g->d_counter);
+    if (g->tex) cudaDestroyTextureObject(g->tex);
+    if (g->surf) cudaDestroySurfaceObject(g->surf);
+    if (g->atlas) cudaFreeArray(g->atlas);
     if (g->h_scal) cudaFreeHost(g->h_scal);
     if (g->ev0) cudaEventDestroy(g->ev0);
     if (g->ev1) cudaEventDestroy(g->ev1);
@@ -231,10 +237,12 @@ int build_geometry(oat_geometry *G)
     P.frame = G->d_frame; P.band = G->d_band; P.ring = G->d_ring;
     P.qb_rings = G->d_qb_rings; P.item_prefix = G->d_item_prefix;
     P.n_items = items;
+    P.tex = 0; P.atlas_shift = 0; P.atlas_mask = 0;
 
     G->n_vox = (size_t)d.nx * d.ny * d.nz;
     G->n_dat = (size_t)Q * K;
     G->n_pad = (size_t)P.pz * P.pxy;
+    if (G->n_pad >= (1ULL << 31)) return fail(OAT_ERR_INVALID, "padded grid has more than 2^31 nodes");
     CUDA_TRY(cudaMalloc((void **)&G->d_xpad, sizeof(float) * G->n_pad));
     CUDA_TRY(cudaMalloc((void **)&G->d_g, sizeof(double) * (G->n_dat ? G->n_dat : 1)));
     CUDA_TRY(cudaMalloc((void **)&G->d_scal, sizeof(double) * 8));
@@ -245,14 +253,55 @@ int build_geometry(oat_geometry *G)
     return OAT_OK;
 }
 
+// Slice atlas for the texture-gather variant: the pz slices of the padded volume tiled into one 2-D
+// CUDA array (2-D because texture gather, tld4, exists for 2-D textures only), 2^shift slices per row.
+int ensure_atlas(oat_geometry *G)
+{
+    if (G->tex) return OAT_OK;
+    OatDev &P = G->dev;
+    int shift = 0;
+    while ((1 << (2 * shift)) < P.pz) ++shift;            // cols = 2^shift >= sqrt(pz)
+    const int cols = 1 << shift, rows = (P.pz + cols - 1) / cols;
+    int maxw = 0, maxh = 0;
+    CUDA_TRY(cudaDeviceGetAttribute(&maxw, cudaDevAttrMaxTexture2DGatherWidth, G->device));
+    CUDA_TRY(cudaDeviceGetAttribute(&maxh, cudaDevAttrMaxTexture2DGatherHeight, G->device));
+    if ((long long)cols * P.px > maxw || (long long)rows * P.py > maxh)
+        return fail(OAT_ERR_INVALID, "grid too large for the texture-gather variant (atlas %lld x %lld > %d x %d)",
+                    (long long)cols * P.px, (long long)rows * P.py, maxw, maxh);
+    cudaChannelFormatDesc fmt = cudaCreateChannelDesc<float>();
+    CUDA_TRY(cudaMallocArray(&G->atlas, &fmt, (size_t)cols * P.px, (size_t)rows * P.py,
+                             cudaArrayTextureGather | cudaArraySurfaceLoadStore));
+    cudaResourceDesc res;
+    memset(&res, 0, sizeof(res));
+    res.resType = cudaResourceTypeArray;
+    res.res.array.array = G->atlas;
+    cudaTextureDesc td;
+    memset(&td, 0, sizeof(td));
+    td.addressMode[0] = td.addressMode[1] = cudaAddressModeClamp;
+    td.filterMode = cudaFilterModePoint;
+    td.readMode = cudaReadModeElementType;
+    td.normalizedCoords = 0;
+    CUDA_TRY(cudaCreateTextureObject(&G->tex, &res, &td, nullptr));
+    CUDA_TRY(cudaCreateSurfaceObject(&G->surf, &res));
+    P.tex = G->tex;
+    P.atlas_shift = shift;
+    P.atlas_mask = cols - 1;
+    return OAT_OK;
+}
+
 int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    oat_launch_pad(P, d_x, G->d_xpad, st); ++G->last_launches;
+    if (G->variant_project == 1) {
+        int rc = ensure_atlas(G); if (rc) return rc;
+        oat_launch_pad_atlas(P, d_x, G->surf, st); ++G->last_launches;
+    } else {
+        oat_launch_pad(P, d_x, G->d_xpad, st); ++G->last_launches;
+    }
     CUDA_TRY(cudaMemsetAsync(G->d_g, 0, sizeof(double) * (G->n_dat ? G->n_dat : 1), st));
     CUDA_TRY(cudaEventRecord(G->ev0, st));
-    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(0, P, G->d_xpad, nullptr, nullptr, G->d_g, nullptr, st)); ++G->last_launches; }
+    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(0, G->variant_project, P, G->d_xpad, nullptr, nullptr, G->d_g, nullptr, st)); ++G->last_launches; }
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
     if (G->n_dat > 0) { oat_launch_diff(P, G->d_g, d_y, st); ++G->last_launches; }
@@ -266,7 +315,7 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
     G->last_launches = 0;
     CUDA_TRY(cudaMemsetAsync(G->d_xpad, 0, sizeof(float) * G->n_pad, st));
     CUDA_TRY(cudaEventRecord(G->ev0, st));
-    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(1, P, nullptr, G->d_xpad, d_y, nullptr, nullptr, st)); ++G->last_launches; }
+    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(1, G->variant_backproject, P, nullptr, G->d_xpad, d_y, nullptr, nullptr, st)); ++G->last_launches; }
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
     oat_launch_unpad(P, G->d_xpad, d_x, st); ++G->last_launches;
@@ -354,7 +403,7 @@ int64_t oat_num_surface_samples(oat_geometry *g)
     if (check_handle(g)) return -1;
     if (g->n_surface_samples >= 0) return g->n_surface_samples;
     if (cudaMemset(g->d_counter, 0, sizeof(unsigned long long)) != cudaSuccess) return -1;
-    if (oat_launch_ray(2, g->dev, nullptr, nullptr, nullptr, nullptr, g->d_counter, 0) != cudaSuccess) return -1;
+    if (oat_launch_ray(2, 0, g->dev, nullptr, nullptr, nullptr, nullptr, g->d_counter, 0) != cudaSuccess) return -1;
     unsigned long long v = 0;
     if (cudaMemcpy(&v, g->d_counter, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) {
         fail(OAT_ERR_CUDA, "sample count kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -470,8 +519,8 @@ int oat_cgls(oat_geometry *g, const float *d_y, float *d_x, int n_iter, double *
 int oat_set_variant(oat_geometry *g, const char *key, int variant)
 {
     if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");
-    if (!strcmp(key, "project")) { if (variant != 0) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
-    if (!strcmp(key, "backproject")) { if (variant != 0) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
+    if (!strcmp(key, "project")) { if (variant != 0 && variant != 1) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
+    if (!strcmp(key, "backproject")) { if (variant != 0 && variant != 1) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
     return fail(OAT_ERR_INVALID, "unknown variant key '%s'", key);
 }
 

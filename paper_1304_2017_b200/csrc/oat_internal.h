@@ -50,13 +50,16 @@ struct OatDev {
     const int *qb_rings;
     const long long *item_prefix;
     long long n_items;
+    cudaTextureObject_t tex;   // slice atlas of the padded volume (project variant 1), 0 if unused
+    int atlas_shift, atlas_mask;   // slice z sits at column (z & mask), row (z >> shift) of the atlas
 };
 
 // launchers (oat_kernels.cu); all asynchronous on `st`
 void oat_launch_pad(const OatDev &P, const float *x, float *xpad, cudaStream_t st);
 void oat_launch_unpad(const OatDev &P, const float *xpad, float *x, cudaStream_t st);
 // mode 0: g += G x (gathers from xpad); 1: xacc += G^T D^T y (scatter); 2: count in-box samples
-cudaError_t oat_launch_ray(int mode, const OatDev &P, const float *xpad, float *xacc, const float *y,
+void oat_launch_pad_atlas(const OatDev &P, const float *x, cudaSurfaceObject_t surf, cudaStream_t st);
+cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
                            double *g, unsigned long long *counter, cudaStream_t st);
 void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st);
 // vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)

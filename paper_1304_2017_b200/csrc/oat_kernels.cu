@@ -55,7 +55,7 @@ __device__ __forceinline__ bool lane_sample(const OatDev &P, const Entry &e, flo
     return ((unsigned)s.ix <= (unsigned)P.nx) & ((unsigned)s.iy <= (unsigned)P.ny) & ((unsigned)s.iz <= (unsigned)P.nz);
 }
 
-template <int MODE>
+template <int MODE, int VAR>
 __global__ void __launch_bounds__(OAT_NT, 2)
 oat_ray_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict__ xacc,
                const float *__restrict__ y, double *__restrict__ g, unsigned long long *__restrict__ counter)
@@ -173,15 +173,27 @@ oat_ray_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict
                 Sample s;
                 const bool in = lane_sample(P, e, delta, s) && active;
                 if (MODE == 2) { cnt += in ? 1u : 0u; continue; }
-                if (!in) continue;
-                const size_t idx = ((size_t)s.iz * P.py + s.iy) * P.px + s.ix;
                 if (MODE == 0) {
-                    const float *p = xpad + idx;
-                    const float v000 = __ldg(p), v100 = __ldg(p + 1);
-                    const float v010 = __ldg(p + P.px), v110 = __ldg(p + P.px + 1);
-                    const float *p1 = p + P.pxy;
-                    const float v001 = __ldg(p1), v101 = __ldg(p1 + 1);
-                    const float v011 = __ldg(p1 + P.px), v111 = __ldg(p1 + P.px + 1);
+                    if (!in) continue;
+                    float v000, v100, v010, v110, v001, v101, v011, v111;
+                    if (VAR == 0) {                       // 8 scalar loads from the padded linear volume
+                        const float *p = xpad + ((size_t)s.iz * P.py + s.iy) * P.px + s.ix;
+                        v000 = __ldg(p); v100 = __ldg(p + 1);
+                        v010 = __ldg(p + P.px); v110 = __ldg(p + P.px + 1);
+                        const float *p1 = p + P.pxy;
+                        v001 = __ldg(p1); v101 = __ldg(p1 + 1);
+                        v011 = __ldg(p1 + P.px); v111 = __ldg(p1 + P.px + 1);
+                    } else {                              // 2 texture gathers (tld4) from the slice atlas
+                        const int z1 = s.iz + 1;
+                        const float tx = (float)s.ix + 1.0f, ty = (float)s.iy + 1.0f;   // between texel centres: exact 2x2 footprint
+                        const float ax0 = (float)((s.iz & P.atlas_mask) * P.px), ay0 = (float)((s.iz >> P.atlas_shift) * P.py);
+                        const float ax1 = (float)((z1 & P.atlas_mask) * P.px), ay1 = (float)((z1 >> P.atlas_shift) * P.py);
+                        const float4 lo = tex2Dgather<float4>(P.tex, tx + ax0, ty + ay0, 0);
+                        const float4 hi = tex2Dgather<float4>(P.tex, tx + ax1, ty + ay1, 0);
+                        // gather order: x = (i, j+1), y = (i+1, j+1), z = (i+1, j), w = (i, j)
+                        v000 = lo.w; v100 = lo.z; v010 = lo.x; v110 = lo.y;
+                        v001 = hi.w; v101 = hi.z; v011 = hi.x; v111 = hi.y;
+                    }
                     const float a00 = fmaf(s.fx, v100 - v000, v000);
                     const float a10 = fmaf(s.fx, v110 - v010, v010);
                     const float a01 = fmaf(s.fx, v101 - v001, v001);
@@ -189,19 +201,49 @@ oat_ray_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict
                     const float b0 = fmaf(s.fy, a10 - a00, a00);
                     const float b1 = fmaf(s.fy, a11 - a01, a01);
                     acc = fmaf(e.a.w, fmaf(s.fz, b1 - b0, b0), acc);
-                } else {
-                    float *p = xacc + idx;
-                    const float wz1 = s.fz * (coef * e.a.w), wz0 = coef * e.a.w - wz1;
+                } else if (MODE == 1) {
+                    if (VAR == 0) { if (!in) continue; }
+                    else if (!__any_sync(0xffffffffu, in)) continue;
+                    const size_t idx = ((size_t)s.iz * P.py + s.iy) * P.px + s.ix;
+                    const float cw = in ? coef * e.a.w : 0.f;
+                    const float wz1 = s.fz * cw, wz0 = cw - wz1;
                     const float gx = 1.f - s.fx, gy = 1.f - s.fy;
-                    atomicAdd(p, gx * gy * wz0);
-                    atomicAdd(p + 1, s.fx * gy * wz0);
-                    atomicAdd(p + P.px, gx * s.fy * wz0);
-                    atomicAdd(p + P.px + 1, s.fx * s.fy * wz0);
-                    float *p1 = p + P.pxy;
-                    atomicAdd(p1, gx * gy * wz1);
-                    atomicAdd(p1 + 1, s.fx * gy * wz1);
-                    atomicAdd(p1 + P.px, gx * s.fy * wz1);
-                    atomicAdd(p1 + P.px + 1, s.fx * s.fy * wz1);
+                    float w[8] = {gx * gy * wz0, s.fx * gy * wz0, gx * s.fy * wz0, s.fx * s.fy * wz0,
+                                  gx * gy * wz1, s.fx * gy * wz1, gx * s.fy * wz1, s.fx * s.fy * wz1};
+                    bool writer = in;
+                    if (VAR == 1) {
+                        // Lanes step along one ray, so lanes that fall into the same cell are CONSECUTIVE:
+                        // sum each run into its first lane (segmented suffix sum by shuffles) and let only
+                        // run heads issue the 8 atomics (~3x fewer L2 atomic operations).
+                        const unsigned cell = in ? (unsigned)idx : (0xfffffff0u - (unsigned)lane);
+                        const unsigned prev = __shfl_up_sync(0xffffffffu, cell, 1);
+                        const bool head = (lane == 0) || (cell != prev);
+                        const unsigned heads = __ballot_sync(0xffffffffu, head);
+                        const unsigned above = (lane == 31) ? 0u : (heads & ~((2u << lane) - 1u));
+                        const int run_end = above ? (__ffs(above) - 2) : 31;
+                        const unsigned maxrun = __reduce_max_sync(0xffffffffu, head ? (unsigned)(run_end - lane + 1) : 0u);
+                        for (unsigned d = 1; d < maxrun; d <<= 1) {
+                            const bool take = (lane + (int)d) <= run_end;
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) {
+                                const float o = __shfl_down_sync(0xffffffffu, w[c], d);
+                                if (take) w[c] += o;
+                            }
+                        }
+                        writer = in && head;
+                    }
+                    if (writer) {
+                        float *p = xacc + idx;
+                        atomicAdd(p, w[0]);
+                        atomicAdd(p + 1, w[1]);
+                        atomicAdd(p + P.px, w[2]);
+                        atomicAdd(p + P.px + 1, w[3]);
+                        float *p1 = p + P.pxy;
+                        atomicAdd(p1, w[4]);
+                        atomicAdd(p1 + 1, w[5]);
+                        atomicAdd(p1 + P.px, w[6]);
+                        atomicAdd(p1 + P.px + 1, w[7]);
+                    }
                 }
             }
             __syncthreads();                              // list is rebuilt next round
@@ -237,6 +279,21 @@ __global__ void oat_pad_kernel(const OatDev P, const float *__restrict__ x, floa
         if (xx >= 1 && xx <= P.nx && yy >= 1 && yy <= P.ny && zz >= 1 && zz <= P.nz)
             v = x[((size_t)(zz - 1) * P.ny + (yy - 1)) * P.nx + (xx - 1)];
         xpad[i] = v;
+    }
+}
+
+// same padded volume written into the 2-D slice atlas (slice z at column z & mask, row z >> shift)
+__global__ void oat_pad_atlas_kernel(const OatDev P, const float *__restrict__ x, cudaSurfaceObject_t surf)
+{
+    const long long n = (long long)P.pz * P.pxy;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int xx = (int)(i % P.px);
+        const long long r = i / P.px;
+        const int yy = (int)(r % P.py), zz = (int)(r / P.py);
+        float v = 0.f;
+        if (xx >= 1 && xx <= P.nx && yy >= 1 && yy <= P.ny && zz >= 1 && zz <= P.nz)
+            v = x[((size_t)(zz - 1) * P.ny + (yy - 1)) * P.nx + (xx - 1)];
+        surf2Dwrite(v, surf, (int)sizeof(float) * ((zz & P.atlas_mask) * P.px + xx), (zz >> P.atlas_shift) * P.py + yy);
     }
 }
 
@@ -309,31 +366,44 @@ void oat_launch_pad(const OatDev &P, const float *x, float *xpad, cudaStream_t s
     oat_pad_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, xpad);
 }
 
+void oat_launch_pad_atlas(const OatDev &P, const float *x, cudaSurfaceObject_t surf, cudaStream_t st)
+{
+    const long long n = (long long)P.pz * P.pxy;
+    oat_pad_atlas_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, surf);
+}
+
 void oat_launch_unpad(const OatDev &P, const float *xpad, float *x, cudaStream_t st)
 {
     const long long n = (long long)P.nx * P.ny * P.nz;
     oat_unpad_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, xpad, x);
 }
 
-cudaError_t oat_launch_ray(int mode, const OatDev &P, const float *xpad, float *xacc, const float *y,
-                           double *g, unsigned long long *counter, cudaStream_t st)
+template <int MODE, int VAR>
+static cudaError_t launch_ray_t(const OatDev &P, const float *xpad, float *xacc, const float *y, double *g,
+                                unsigned long long *counter, cudaStream_t st)
 {
-    if (P.n_items <= 0) return cudaSuccess;
     const size_t smem = sizeof(Entry) * OAT_SB;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e;
-        if ((e = cudaFuncSetAttribute(oat_ray_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) return e;
-        if ((e = cudaFuncSetAttribute(oat_ray_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) return e;
-        if ((e = cudaFuncSetAttribute(oat_ray_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) return e;
+        cudaError_t e = cudaFuncSetAttribute(oat_ray_kernel<MODE, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e) return e;
         attr_set = true;
     }
     const long long cap = 0x7fffffffLL;
     const unsigned grid = (unsigned)(P.n_items < cap ? P.n_items : cap);
-    if (mode == 0) oat_ray_kernel<0><<<grid, OAT_NT, smem, st>>>(P, xpad, xacc, y, g, counter);
-    else if (mode == 1) oat_ray_kernel<1><<<grid, OAT_NT, smem, st>>>(P, xpad, xacc, y, g, counter);
-    else oat_ray_kernel<2><<<grid, OAT_NT, smem, st>>>(P, xpad, xacc, y, g, counter);
+    oat_ray_kernel<MODE, VAR><<<grid, OAT_NT, smem, st>>>(P, xpad, xacc, y, g, counter);
     return cudaGetLastError();
+}
+
+cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
+                           double *g, unsigned long long *counter, cudaStream_t st)
+{
+    if (P.n_items <= 0) return cudaSuccess;
+    if (mode == 0) return variant == 1 ? launch_ray_t<0, 1>(P, xpad, xacc, y, g, counter, st)
+                                       : launch_ray_t<0, 0>(P, xpad, xacc, y, g, counter, st);
+    if (mode == 1) return variant == 0 ? launch_ray_t<1, 0>(P, xpad, xacc, y, g, counter, st)
+                                       : launch_ray_t<1, 1>(P, xpad, xacc, y, g, counter, st);
+    return launch_ray_t<2, 0>(P, xpad, xacc, y, g, counter, st);
 }
 
 void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st)

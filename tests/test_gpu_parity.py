@@ -246,3 +246,21 @@ def test_config4_cgls_first_iterations(env):
     assert rel_l2(x.cpu().numpy(), xo) <= 5e-4
     assert np.all(np.diff(res) <= 1e-6)
     g.close()
+
+
+# ------------------------------------------------------------------ kernel variants
+@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 1), ("backproject", 0), ("backproject", 1)])
+def test_every_kernel_variant_matches_the_oracle(env, key, variant):
+    """each selectable kernel variant computes the same operator."""
+    torch, orc, oat, wl = env
+    w = wl.small(n=18, q=5, nt=75, kband=32)
+    x, y = w.phantom(), w.data_noise()
+    g = oat.oat_geometry_create(w)
+    oat.oat_set_variant(g, key, variant)
+    if key == "project":
+        e = rel_l2(gpu_project(torch, oat, w, x, g), orc.project(w, x.astype(np.float64)))
+    else:
+        e = rel_l2(gpu_backproject(torch, oat, w, y, g), orc.backproject(w, y.astype(np.float64)))
+    _, _, rel = oat.oat_adjoint_check(g, torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda())
+    g.close()
+    assert e <= TOL and rel <= TOL, (key, variant, e, rel)
