@@ -50,6 +50,8 @@ struct oat_geometry {
     long long *d_item_prefix = nullptr;
     // scratch
     float *d_xpad = nullptr;                  // padded volume (gather source / scatter target)
+    float4 *d_quads = nullptr;                // 4 parity-shifted quad arrays (variant 2, lazy)
+    size_t n_quads = 0;
     double *d_g = nullptr;                    // Q*K SRT accumulator
     float *d_y2 = nullptr, *d_x2 = nullptr;   // adjoint check / CGLS / host entry points (lazy)
     float *d_x3 = nullptr, *d_y3 = nullptr, *d_x4 = nullptr;   // CGLS vectors (lazy)
@@ -57,7 +59,7 @@ struct oat_geometry {
     unsigned long long *d_counter = nullptr;
     double *h_scal = nullptr;                 // pinned mirror of d_scal
     long long n_surface_samples = -1;
-    int variant_project = 0, variant_backproject = 1;
+    int variant_project = 1, variant_backproject = 2;   // measured best
     cudaArray_t atlas = nullptr;              // slice atlas for the texture-gather projection (lazy)
     cudaTextureObject_t tex = 0;
     cudaSurfaceObject_t surf = 0;
@@ -75,7 +77,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
-    cudaFree(g->d_counter);
+    cudaFree(g->d_counter); cudaFree(g->d_quads);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
     if (g->atlas) cudaFreeArray(g->atlas);
@@ -238,10 +240,13 @@ int build_geometry(oat_geometry *G)
     P.qb_rings = G->d_qb_rings; P.item_prefix = G->d_item_prefix;
     P.n_items = items;
     P.tex = 0; P.atlas_shift = 0; P.atlas_mask = 0;
+    P.qx = (d.nx + 2) / 2 + 1; P.qy = (d.ny + 2) / 2 + 1;
+    P.qplane = (long long)P.qx * P.qy;
 
     G->n_vox = (size_t)d.nx * d.ny * d.nz;
     G->n_dat = (size_t)Q * K;
     G->n_pad = (size_t)P.pz * P.pxy;
+    G->n_quads = 4 * (size_t)P.pz * (size_t)P.qplane;
     if (G->n_pad >= (1ULL << 31)) return fail(OAT_ERR_INVALID, "padded grid has more than 2^31 nodes");
     CUDA_TRY(cudaMalloc((void **)&G->d_xpad, sizeof(float) * G->n_pad));
     CUDA_TRY(cudaMalloc((void **)&G->d_g, sizeof(double) * (G->n_dat ? G->n_dat : 1)));
@@ -289,11 +294,23 @@ int ensure_atlas(oat_geometry *G)
     return OAT_OK;
 }
 
+int ensure_quads(oat_geometry *G)
+{
+    if (G->d_quads) return OAT_OK;
+    CUDA_TRY(cudaMalloc((void **)&G->d_quads, sizeof(float4) * G->n_quads));
+    return OAT_OK;
+}
+
 int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    if (G->variant_project == 1) {
+    const float *src = G->d_xpad;
+    if (G->variant_project == 2) {
+        int rc = ensure_quads(G); if (rc) return rc;
+        oat_launch_pad_quads(P, d_x, G->d_quads, st); ++G->last_launches;
+        src = reinterpret_cast<const float *>(G->d_quads);
+    } else if (G->variant_project == 1) {
         int rc = ensure_atlas(G); if (rc) return rc;
         oat_launch_pad_atlas(P, d_x, G->surf, st); ++G->last_launches;
     } else {
@@ -301,7 +318,7 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     }
     CUDA_TRY(cudaMemsetAsync(G->d_g, 0, sizeof(double) * (G->n_dat ? G->n_dat : 1), st));
     CUDA_TRY(cudaEventRecord(G->ev0, st));
-    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(0, G->variant_project, P, G->d_xpad, nullptr, nullptr, G->d_g, nullptr, st)); ++G->last_launches; }
+    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(0, G->variant_project, P, src, nullptr, nullptr, G->d_g, nullptr, st)); ++G->last_launches; }
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
     if (G->n_dat > 0) { oat_launch_diff(P, G->d_g, d_y, st); ++G->last_launches; }
@@ -313,12 +330,22 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    CUDA_TRY(cudaMemsetAsync(G->d_xpad, 0, sizeof(float) * G->n_pad, st));
+    const bool quads = G->variant_backproject == 2;
+    float *acc = G->d_xpad;
+    if (quads) {
+        int rc = ensure_quads(G); if (rc) return rc;
+        acc = reinterpret_cast<float *>(G->d_quads);
+        CUDA_TRY(cudaMemsetAsync(G->d_quads, 0, sizeof(float4) * G->n_quads, st));
+    } else {
+        CUDA_TRY(cudaMemsetAsync(G->d_xpad, 0, sizeof(float) * G->n_pad, st));
+    }
     CUDA_TRY(cudaEventRecord(G->ev0, st));
-    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(1, G->variant_backproject, P, nullptr, G->d_xpad, d_y, nullptr, nullptr, st)); ++G->last_launches; }
+    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(1, G->variant_backproject, P, nullptr, acc, d_y, nullptr, nullptr, st)); ++G->last_launches; }
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
-    oat_launch_unpad(P, G->d_xpad, d_x, st); ++G->last_launches;
+    if (quads) oat_launch_unquad(P, G->d_quads, d_x, st);
+    else oat_launch_unpad(P, G->d_xpad, d_x, st);
+    ++G->last_launches;
     CUDA_TRY(cudaGetLastError());
     return OAT_OK;
 }
@@ -519,8 +546,8 @@ int oat_cgls(oat_geometry *g, const float *d_y, float *d_x, int n_iter, double *
 int oat_set_variant(oat_geometry *g, const char *key, int variant)
 {
     if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");
-    if (!strcmp(key, "project")) { if (variant != 0 && variant != 1) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
-    if (!strcmp(key, "backproject")) { if (variant != 0 && variant != 1) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
+    if (!strcmp(key, "project")) { if (variant < 0 || variant > 2) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
+    if (!strcmp(key, "backproject")) { if (variant < 0 || variant > 2) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
     return fail(OAT_ERR_INVALID, "unknown variant key '%s'", key);
 }
 

@@ -39,21 +39,72 @@ struct Sample {
     float fx, fy, fz;
 };
 
+// floor() without the quarter-rate conversion pipe: adding 1.5*2^23 with round-toward-minus-infinity
+// leaves floor(t) in the low mantissa bits (|t| < 2^22), so the integer cell index is one integer add
+// away from the float's bit pattern and floor(t) as a float is one exact subtraction away.
+#define OAT_MAGIC 12582912.0f
+#define OAT_MAGIC_BITS 0x4B400000
+
 __device__ __forceinline__ bool lane_sample(const OatDev &P, const Entry &e, float delta, Sample &s)
 {
     const float tx = fmaf(delta, e.u.x, e.a.x);
     const float ty = fmaf(delta, e.u.y, e.a.y);
     const float tz = fmaf(delta, e.u.z, e.a.z);
-    const float flx = floorf(tx), fly = floorf(ty), flz = floorf(tz);
-    s.ix = (int)flx + e.i.x;
-    s.iy = (int)fly + e.i.y;
-    s.iz = (int)flz + e.i.z;
-    s.fx = tx - flx;
-    s.fy = ty - fly;
-    s.fz = tz - flz;
+    const float rx = __fadd_rd(tx, OAT_MAGIC), ry = __fadd_rd(ty, OAT_MAGIC), rz = __fadd_rd(tz, OAT_MAGIC);
+    s.ix = __float_as_int(rx) + e.i.x;                   // e.i.* carry the -OAT_MAGIC_BITS bias
+    s.iy = __float_as_int(ry) + e.i.y;
+    s.iz = __float_as_int(rz) + e.i.z;
+    s.fx = tx - (rx - OAT_MAGIC);
+    s.fy = ty - (ry - OAT_MAGIC);
+    s.fz = tz - (rz - OAT_MAGIC);
     // padded cell n' in [0, N] <=> xi in [-1, N): the sample touches at least one existing node (S4)
     return ((unsigned)s.ix <= (unsigned)P.nx) & ((unsigned)s.iy <= (unsigned)P.ny) & ((unsigned)s.iz <= (unsigned)P.nz);
 }
+
+__device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float c, float d)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
+// index of the quad that holds the in-plane corners of padded cell (ix, iy) in plane iz
+__device__ __forceinline__ unsigned quad_index(const OatDev &P, int ix, int iy, int iz)
+{
+    const int par = (ix & 1) | ((iy & 1) << 1);          // 4*pz*qplane < 2^31 is checked at create
+    return (unsigned)(((par * P.pz + iz) * P.qy + (iy >> 1)) * P.qx + (ix >> 1));
+}
+
+// the 8 corner values of the sample's cell (v[cz*4 + cy*2 + cx]); lanes that are not in the box read
+// cell 0 (valid memory) so that the loads of several list entries can be issued back to back
+template <int VAR>
+__device__ __forceinline__ void fetch8(const OatDev &P, const float *__restrict__ xpad, const Sample &s, bool in, float v[8])
+{
+    const int ix = in ? s.ix : 0, iy = in ? s.iy : 0, iz = in ? s.iz : 0;
+    if (VAR == 0) {                                       // 8 scalar loads from the padded linear volume
+        const float *p = xpad + (unsigned)((iz * P.py + iy) * P.px + ix);
+        v[0] = __ldg(p); v[1] = __ldg(p + 1);
+        v[2] = __ldg(p + P.px); v[3] = __ldg(p + P.px + 1);
+        const float *p1 = p + P.pxy;
+        v[4] = __ldg(p1); v[5] = __ldg(p1 + 1);
+        v[6] = __ldg(p1 + P.px); v[7] = __ldg(p1 + P.px + 1);
+    } else if (VAR == 2) {                                // 2 x LDG.128 from the parity-shifted quad arrays
+        const float4 *qp = reinterpret_cast<const float4 *>(xpad) + quad_index(P, ix, iy, iz);
+        const float4 lo = __ldg(qp), hi = __ldg(qp + P.qplane);
+        v[0] = lo.x; v[1] = lo.y; v[2] = lo.z; v[3] = lo.w;
+        v[4] = hi.x; v[5] = hi.y; v[6] = hi.z; v[7] = hi.w;
+    } else {                                              // 2 texture gathers (tld4) from the slice atlas
+        const int z1 = iz + 1;
+        const float tx = (float)ix + 1.0f, ty = (float)iy + 1.0f;   // between texel centres: exact 2x2 footprint
+        const float ax0 = (float)((iz & P.atlas_mask) * P.px), ay0 = (float)((iz >> P.atlas_shift) * P.py);
+        const float ax1 = (float)((z1 & P.atlas_mask) * P.px), ay1 = (float)((z1 >> P.atlas_shift) * P.py);
+        const float4 lo = tex2Dgather<float4>(P.tex, tx + ax0, ty + ay0, 0);
+        const float4 hi = tex2Dgather<float4>(P.tex, tx + ax1, ty + ay1, 0);
+        // gather order: x = (i, j+1), y = (i+1, j+1), z = (i+1, j), w = (i, j)
+        v[0] = lo.w; v[1] = lo.z; v[2] = lo.x; v[3] = lo.y;
+        v[4] = hi.w; v[5] = hi.z; v[6] = hi.x; v[7] = hi.y;
+    }
+}
+
+#define OAT_U 2    // list entries in flight per warp (independent dependency chains)
 
 template <int MODE, int VAR>
 __global__ void __launch_bounds__(OAT_NT, 2)
@@ -161,88 +212,93 @@ oat_ray_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict
                 }
                 e.a = make_float4(af[0], af[1], af[2], R.omega);
                 e.u = make_float4(uu[0], uu[1], uu[2], 0.f);
-                e.i = make_int4(ai[0], ai[1], ai[2], 0);
+                e.i = make_int4(ai[0] - OAT_MAGIC_BITS, ai[1] - OAT_MAGIC_BITS, ai[2] - OAT_MAGIC_BITS, 0);
                 const int slot = atomicAdd(&s_count, 1);
                 list[slot] = e;
             }
             __syncthreads();
             // ------------------------------------------------------------ consume
             const int n_list = s_count;
-            for (int ei = warp; ei < n_list; ei += OAT_NW) {
-                const Entry e = list[ei];
-                Sample s;
-                const bool in = lane_sample(P, e, delta, s) && active;
-                if (MODE == 2) { cnt += in ? 1u : 0u; continue; }
-                if (MODE == 0) {
-                    if (!in) continue;
-                    float v000, v100, v010, v110, v001, v101, v011, v111;
-                    if (VAR == 0) {                       // 8 scalar loads from the padded linear volume
-                        const float *p = xpad + ((size_t)s.iz * P.py + s.iy) * P.px + s.ix;
-                        v000 = __ldg(p); v100 = __ldg(p + 1);
-                        v010 = __ldg(p + P.px); v110 = __ldg(p + P.px + 1);
-                        const float *p1 = p + P.pxy;
-                        v001 = __ldg(p1); v101 = __ldg(p1 + 1);
-                        v011 = __ldg(p1 + P.px); v111 = __ldg(p1 + P.px + 1);
-                    } else {                              // 2 texture gathers (tld4) from the slice atlas
-                        const int z1 = s.iz + 1;
-                        const float tx = (float)s.ix + 1.0f, ty = (float)s.iy + 1.0f;   // between texel centres: exact 2x2 footprint
-                        const float ax0 = (float)((s.iz & P.atlas_mask) * P.px), ay0 = (float)((s.iz >> P.atlas_shift) * P.py);
-                        const float ax1 = (float)((z1 & P.atlas_mask) * P.px), ay1 = (float)((z1 >> P.atlas_shift) * P.py);
-                        const float4 lo = tex2Dgather<float4>(P.tex, tx + ax0, ty + ay0, 0);
-                        const float4 hi = tex2Dgather<float4>(P.tex, tx + ax1, ty + ay1, 0);
-                        // gather order: x = (i, j+1), y = (i+1, j+1), z = (i+1, j), w = (i, j)
-                        v000 = lo.w; v100 = lo.z; v010 = lo.x; v110 = lo.y;
-                        v001 = hi.w; v101 = hi.z; v011 = hi.x; v111 = hi.y;
-                    }
-                    const float a00 = fmaf(s.fx, v100 - v000, v000);
-                    const float a10 = fmaf(s.fx, v110 - v010, v010);
-                    const float a01 = fmaf(s.fx, v101 - v001, v001);
-                    const float a11 = fmaf(s.fx, v111 - v011, v011);
-                    const float b0 = fmaf(s.fy, a10 - a00, a00);
-                    const float b1 = fmaf(s.fy, a11 - a01, a01);
-                    acc = fmaf(e.a.w, fmaf(s.fz, b1 - b0, b0), acc);
-                } else if (MODE == 1) {
-                    if (VAR == 0) { if (!in) continue; }
-                    else if (!__any_sync(0xffffffffu, in)) continue;
-                    const size_t idx = ((size_t)s.iz * P.py + s.iy) * P.px + s.ix;
-                    const float cw = in ? coef * e.a.w : 0.f;
-                    const float wz1 = s.fz * cw, wz0 = cw - wz1;
-                    const float gx = 1.f - s.fx, gy = 1.f - s.fy;
-                    float w[8] = {gx * gy * wz0, s.fx * gy * wz0, gx * s.fy * wz0, s.fx * s.fy * wz0,
-                                  gx * gy * wz1, s.fx * gy * wz1, gx * s.fy * wz1, s.fx * s.fy * wz1};
-                    bool writer = in;
-                    if (VAR == 1) {
-                        // Lanes step along one ray, so lanes that fall into the same cell are CONSECUTIVE:
-                        // sum each run into its first lane (segmented suffix sum by shuffles) and let only
-                        // run heads issue the 8 atomics (~3x fewer L2 atomic operations).
-                        const unsigned cell = in ? (unsigned)idx : (0xfffffff0u - (unsigned)lane);
-                        const unsigned prev = __shfl_up_sync(0xffffffffu, cell, 1);
-                        const bool head = (lane == 0) || (cell != prev);
-                        const unsigned heads = __ballot_sync(0xffffffffu, head);
-                        const unsigned above = (lane == 31) ? 0u : (heads & ~((2u << lane) - 1u));
-                        const int run_end = above ? (__ffs(above) - 2) : 31;
-                        const unsigned maxrun = __reduce_max_sync(0xffffffffu, head ? (unsigned)(run_end - lane + 1) : 0u);
-                        for (unsigned d = 1; d < maxrun; d <<= 1) {
-                            const bool take = (lane + (int)d) <= run_end;
+            for (int e0 = warp; e0 < n_list; e0 += OAT_NW * OAT_U) {
+                Sample s[OAT_U];
+                bool in[OAT_U];
+                float om[OAT_U];
 #pragma unroll
-                            for (int c = 0; c < 8; ++c) {
-                                const float o = __shfl_down_sync(0xffffffffu, w[c], d);
-                                if (take) w[c] += o;
-                            }
-                        }
-                        writer = in && head;
+                for (int u = 0; u < OAT_U; ++u) {
+                    const int ei = e0 + u * OAT_NW;
+                    const bool valid = ei < n_list;
+                    const Entry e = list[valid ? ei : e0];
+                    in[u] = lane_sample(P, e, delta, s[u]) && active && valid;
+                    om[u] = e.a.w;
+                }
+                if (MODE == 2) {
+#pragma unroll
+                    for (int u = 0; u < OAT_U; ++u) cnt += in[u] ? 1u : 0u;
+                } else if (MODE == 0) {
+                    float v[OAT_U][8];
+#pragma unroll
+                    for (int u = 0; u < OAT_U; ++u) fetch8<VAR>(P, xpad, s[u], in[u], v[u]);
+#pragma unroll
+                    for (int u = 0; u < OAT_U; ++u) {
+                        const float a00 = fmaf(s[u].fx, v[u][1] - v[u][0], v[u][0]);
+                        const float a10 = fmaf(s[u].fx, v[u][3] - v[u][2], v[u][2]);
+                        const float a01 = fmaf(s[u].fx, v[u][5] - v[u][4], v[u][4]);
+                        const float a11 = fmaf(s[u].fx, v[u][7] - v[u][6], v[u][6]);
+                        const float b0 = fmaf(s[u].fy, a10 - a00, a00);
+                        const float b1 = fmaf(s[u].fy, a11 - a01, a01);
+                        acc = fmaf(in[u] ? om[u] : 0.f, fmaf(s[u].fz, b1 - b0, b0), acc);
                     }
-                    if (writer) {
-                        float *p = xacc + idx;
-                        atomicAdd(p, w[0]);
-                        atomicAdd(p + 1, w[1]);
-                        atomicAdd(p + P.px, w[2]);
-                        atomicAdd(p + P.px + 1, w[3]);
-                        float *p1 = p + P.pxy;
-                        atomicAdd(p1, w[4]);
-                        atomicAdd(p1 + 1, w[5]);
-                        atomicAdd(p1 + P.px, w[6]);
-                        atomicAdd(p1 + P.px + 1, w[7]);
+                } else {
+#pragma unroll
+                    for (int u = 0; u < OAT_U; ++u) {
+                        const unsigned idx = (VAR == 2) ? quad_index(P, s[u].ix, s[u].iy, s[u].iz)
+                                                        : (unsigned)((s[u].iz * P.py + s[u].iy) * P.px + s[u].ix);
+                        const float cw = in[u] ? coef * om[u] : 0.f;
+                        const float wz1 = s[u].fz * cw, wz0 = cw - wz1;
+                        const float gx = 1.f - s[u].fx, gy = 1.f - s[u].fy;
+                        const float w00 = gx * gy, w10 = s[u].fx * gy, w01 = gx * s[u].fy, w11 = s[u].fx * s[u].fy;
+                        float w[8] = {w00 * wz0, w10 * wz0, w01 * wz0, w11 * wz0, w00 * wz1, w10 * wz1, w01 * wz1, w11 * wz1};
+                        bool writer = in[u];
+                        if (VAR >= 1) {
+                            // Lanes step along one ray, so lanes that fall into the same cell are CONSECUTIVE:
+                            // sum each run into its first lane (segmented suffix sum by shuffles) and let only
+                            // run heads issue the atomics (~3x fewer L2 atomic operations).
+                            const unsigned cell = in[u] ? idx : (0xfffffff0u - (unsigned)lane);
+                            const unsigned prev = __shfl_up_sync(0xffffffffu, cell, 1);
+                            const bool head = (lane == 0) || (cell != prev);
+                            const unsigned heads = __ballot_sync(0xffffffffu, head);
+                            const unsigned above = (lane == 31) ? 0u : (heads & ~((2u << lane) - 1u));
+                            const int run_end = above ? (__ffs(above) - 2) : 31;
+                            const unsigned maxrun = __reduce_max_sync(0xffffffffu, (head && in[u]) ? (unsigned)(run_end - lane + 1) : 0u);
+#pragma unroll
+                            for (int d = 1; d < 32; d <<= 1) {
+                                if (maxrun > (unsigned)d) {                    // warp-uniform
+                                    const float keep = (lane + d <= run_end) ? 1.f : 0.f;
+#pragma unroll
+                                    for (int c = 0; c < 8; ++c) w[c] = fmaf(keep, __shfl_down_sync(0xffffffffu, w[c], d), w[c]);
+                                }
+                            }
+                            writer = in[u] && head;
+                        }
+                        if (VAR == 2) {
+                            // one aligned 16-byte vector reduction per plane: 2 L2 sector operations per run
+                            if (writer) {
+                                float4 *qp = reinterpret_cast<float4 *>(xacc) + idx;
+                                red_add_v4(qp, w[0], w[1], w[2], w[3]);
+                                red_add_v4(qp + P.qplane, w[4], w[5], w[6], w[7]);
+                            }
+                        } else if (writer) {
+                            float *p = xacc + idx;
+                            atomicAdd(p, w[0]);
+                            atomicAdd(p + 1, w[1]);
+                            atomicAdd(p + P.px, w[2]);
+                            atomicAdd(p + P.px + 1, w[3]);
+                            float *p1 = p + P.pxy;
+                            atomicAdd(p1, w[4]);
+                            atomicAdd(p1 + 1, w[5]);
+                            atomicAdd(p1 + P.px, w[6]);
+                            atomicAdd(p1 + P.px + 1, w[7]);
+                        }
                     }
                 }
             }
@@ -279,6 +335,50 @@ __global__ void oat_pad_kernel(const OatDev P, const float *__restrict__ x, floa
         if (xx >= 1 && xx <= P.nx && yy >= 1 && yy <= P.ny && zz >= 1 && zz <= P.nz)
             v = x[((size_t)(zz - 1) * P.ny + (yy - 1)) * P.nx + (xx - 1)];
         xpad[i] = v;
+    }
+}
+
+// quad arrays from x: array p holds quads with origin (2a + (p&1), 2b + (p>>1)) in padded coordinates
+__global__ void oat_pad_quads_kernel(const OatDev P, const float *__restrict__ x, float4 *__restrict__ quads)
+{
+    const long long n = 4LL * P.pz * P.qplane;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int a = (int)(i % P.qx);
+        long long r = i / P.qx;
+        const int b = (int)(r % P.qy); r /= P.qy;
+        const int z = (int)(r % P.pz);
+        const int par = (int)(r / P.pz);
+        const int x0 = 2 * a + (par & 1), y0 = 2 * b + (par >> 1);
+        float v[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int X = x0 + (c & 1), Y = y0 + (c >> 1);      // padded coordinates; node = (X-1, Y-1, z-1)
+            v[c] = (X >= 1 && X <= P.nx && Y >= 1 && Y <= P.ny && z >= 1 && z <= P.nz)
+                       ? x[((size_t)(z - 1) * P.ny + (Y - 1)) * P.nx + (X - 1)] : 0.f;
+        }
+        quads[i] = make_float4(v[0], v[1], v[2], v[3]);
+    }
+}
+
+// x[n] = sum over the 4 parity arrays of the quad component that is node n (every node is in exactly
+// one quad of each array)
+__global__ void oat_unquad_kernel(const OatDev P, const float4 *__restrict__ quads, float *__restrict__ x)
+{
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int X = (int)(i % P.nx) + 1;
+        const long long r = i / P.nx;
+        const int Y = (int)(r % P.ny) + 1, Z = (int)(r / P.ny) + 1;
+        float sum = 0.f;
+#pragma unroll
+        for (int par = 0; par < 4; ++par) {
+            const int px = par & 1, py = par >> 1;
+            const int a = (X - px) >> 1, b = (Y - py) >> 1;
+            const int c = (X - px - 2 * a) + 2 * (Y - py - 2 * b);
+            const float4 q = quads[((size_t)(par * P.pz + Z) * P.qy + b) * P.qx + a];
+            sum += c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w;
+        }
+        x[i] = sum;
     }
 }
 
@@ -366,6 +466,18 @@ void oat_launch_pad(const OatDev &P, const float *x, float *xpad, cudaStream_t s
     oat_pad_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, xpad);
 }
 
+void oat_launch_pad_quads(const OatDev &P, const float *x, float4 *quads, cudaStream_t st)
+{
+    const long long n = 4LL * P.pz * P.qplane;
+    oat_pad_quads_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, quads);
+}
+
+void oat_launch_unquad(const OatDev &P, const float4 *quads, float *x, cudaStream_t st)
+{
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    oat_unquad_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, quads, x);
+}
+
 void oat_launch_pad_atlas(const OatDev &P, const float *x, cudaSurfaceObject_t surf, cudaStream_t st)
 {
     const long long n = (long long)P.pz * P.pxy;
@@ -399,10 +511,12 @@ cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *
                            double *g, unsigned long long *counter, cudaStream_t st)
 {
     if (P.n_items <= 0) return cudaSuccess;
-    if (mode == 0) return variant == 1 ? launch_ray_t<0, 1>(P, xpad, xacc, y, g, counter, st)
+    if (mode == 0) return variant == 2 ? launch_ray_t<0, 2>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 1 ? launch_ray_t<0, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_ray_t<0, 0>(P, xpad, xacc, y, g, counter, st);
-    if (mode == 1) return variant == 0 ? launch_ray_t<1, 0>(P, xpad, xacc, y, g, counter, st)
-                                       : launch_ray_t<1, 1>(P, xpad, xacc, y, g, counter, st);
+    if (mode == 1) return variant == 2 ? launch_ray_t<1, 2>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 1 ? launch_ray_t<1, 1>(P, xpad, xacc, y, g, counter, st)
+                                       : launch_ray_t<1, 0>(P, xpad, xacc, y, g, counter, st);
     return launch_ray_t<2, 0>(P, xpad, xacc, y, g, counter, st);
 }
 

@@ -249,7 +249,7 @@ def test_config4_cgls_first_iterations(env):
 
 
 # ------------------------------------------------------------------ kernel variants
-@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 1), ("backproject", 0), ("backproject", 1)])
+@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 1), ("project", 2), ("backproject", 0), ("backproject", 1), ("backproject", 2)])
 def test_every_kernel_variant_matches_the_oracle(env, key, variant):
     """each selectable kernel variant computes the same operator."""
     torch, orc, oat, wl = env
