@@ -168,6 +168,10 @@ def run_ours(args):
         from dataclasses import replace
         w = replace(w, trans_xyz=shard.weak_replica_transducers(w.trans_xyz, rank, world, 144))
     g = oat.oat_geometry_create(w, local)
+    if args.project_variant >= 0:
+        oat.oat_set_variant(g, "project", args.project_variant)
+    if args.backproject_variant >= 0:
+        oat.oat_set_variant(g, "backproject", args.backproject_variant)
     x = torch.from_numpy(w.phantom()).cuda()
     y = torch.empty((w.n_trans, w.nt), dtype=torch.float32, device="cuda")
     xb = torch.empty_like(x)
@@ -225,7 +229,7 @@ def run_ours(args):
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
     e2e = None
-    if rank == 0 or world > 1:
+    if args.e2e_steps > 0:
         hx = torch.from_numpy(w.phantom()).pin_memory()
         hy = torch.empty((w.n_trans, w.nt), dtype=torch.float32).pin_memory()
         hxb = torch.empty_like(hx).pin_memory()
@@ -301,6 +305,8 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=8, help="transducers in the oracle's timed sample")
     ap.add_argument("--ref-sample", type=int, default=8, help="transducers per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--project-variant", type=int, default=-1, help="kernel variant (DESIGN.md §5); -1 = library default")
+    ap.add_argument("--backproject-variant", type=int, default=-1)
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
