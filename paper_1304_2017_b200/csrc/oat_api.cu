@@ -47,6 +47,11 @@ struct oat_geometry {
     OatBand *d_band = nullptr;
     OatRing *d_ring = nullptr;
     int *d_qb_rings = nullptr;
+    int *d_rb_sectors = nullptr;
+    unsigned long long *d_patches = nullptr;  // schedule 1 work items (lazy)
+    unsigned long long patch_cap = 0;
+    int morton_shift = 4;                     // patches are sorted by the Morton code of (centre >> shift)
+    int schedule = 1;                         // 0 = ring-major chunks, 1 = Morton-sorted patches
     long long *d_item_prefix = nullptr;
     // scratch
     float *d_xpad = nullptr;                  // padded volume (gather source / scatter target)
@@ -77,7 +82,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
-    cudaFree(g->d_counter); cudaFree(g->d_quads);
+    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
     if (g->atlas) cudaFreeArray(g->atlas);
@@ -181,6 +186,28 @@ int build_geometry(oat_geometry *G)
         rings.push_back(sentinel);
     }
 
+    // ---- ring blocks of OAT_RI rings and their azimuth sector counts (schedule 1: patches)
+    std::vector<int> rb_sectors;
+    std::vector<std::vector<long long>> rb_prefix(NB);     // per band: sectors in ring blocks [0, rb)
+    for (int b = 0; b < NB; ++b) {
+        OatBand &bd = bands[b];
+        bd.rb_ofs = (int)rb_sectors.size();
+        bd.pad = 0;
+        const int n_rb = (bd.n_rings + OAT_RI - 1) / OAT_RI;
+        rb_prefix[b].assign(n_rb + 1, 0);
+        for (int rb = 0; rb < n_rb; ++rb) {
+            int nmax = 1;
+            for (int r = rb * OAT_RI; r < bd.n_rings && r < (rb + 1) * OAT_RI; ++r)
+                if (rings[bd.ring_ofs + r].N > nmax) nmax = rings[bd.ring_ofs + r].N;
+            const int S = (nmax + OAT_RJ - 1) / OAT_RJ;
+            if (S > 0xffff || n_rb > 0x3ff) return fail(OAT_ERR_INVALID, "too many patch sectors / ring blocks (surf_step too small)");
+            rb_sectors.push_back(S);
+            rb_prefix[b][rb + 1] = rb_prefix[b][rb] + S;
+        }
+        if (n_rb == 0) rb_sectors.push_back(1);
+    }
+    if (Q >= (1 << 26) || NB > 0xfff) return fail(OAT_ERR_INVALID, "too many transducers / bands");
+
     // ---- frames (S1) and the per-(q, band) ring bound (S9) + work-item prefix
     std::vector<double> frame((size_t)Q * 12);
     std::vector<int> qb_rings((size_t)Q * NB);
@@ -213,6 +240,7 @@ int build_geometry(oat_geometry *G)
                 }
             }
             qb_rings[(size_t)q * NB + b] = nr;
+            if (nr > 0) G->patch_cap += (unsigned long long)rb_prefix[b][(nr + OAT_RI - 1) / OAT_RI];
             prefix[(size_t)q * NB + b] = items;
             const long long cand = rings[bd.ring_ofs + nr].cum;
             items += (cand + OAT_CH - 1) / OAT_CH;
@@ -227,6 +255,7 @@ int build_geometry(oat_geometry *G)
     if ((rc = upload(&G->d_ring, rings))) return rc;
     if ((rc = upload(&G->d_qb_rings, qb_rings))) return rc;
     if ((rc = upload(&G->d_item_prefix, prefix))) return rc;
+    if ((rc = upload(&G->d_rb_sectors, rb_sectors))) return rc;
 
     OatDev &P = G->dev;
     P.nx = d.nx; P.ny = d.ny; P.nz = d.nz;
@@ -239,6 +268,7 @@ int build_geometry(oat_geometry *G)
     P.frame = G->d_frame; P.band = G->d_band; P.ring = G->d_ring;
     P.qb_rings = G->d_qb_rings; P.item_prefix = G->d_item_prefix;
     P.n_items = items;
+    P.rb_sectors = G->d_rb_sectors; P.patches = nullptr; P.n_patches = 0;
     P.tex = 0; P.atlas_shift = 0; P.atlas_mask = 0;
     P.qx = (d.nx + 2) / 2 + 1; P.qy = (d.ny + 2) / 2 + 1;
     P.qplane = (long long)P.qx * P.qy;
@@ -294,6 +324,31 @@ int ensure_atlas(oat_geometry *G)
     return OAT_OK;
 }
 
+int ensure_patches(oat_geometry *G)
+{
+    if (G->d_patches || G->patch_cap == 0) return OAT_OK;
+    long long n = 0;
+    cudaError_t e = oat_build_patches(G->dev, G->patch_cap, G->morton_shift, &G->d_patches, &n);
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? OAT_ERR_ALLOC : OAT_ERR_CUDA, "patch list generation failed: %s", cudaGetErrorString(e));
+    G->dev.patches = G->d_patches;
+    G->dev.n_patches = n;
+    return OAT_OK;
+}
+
+// one traversal of all samples: mode 0 gather, 1 scatter, 2 count; schedule picks the work decomposition
+int launch_traversal(oat_geometry *G, int mode, int variant, const float *src, float *acc, const float *y, double *g,
+                     unsigned long long *counter, cudaStream_t st, bool *launched)
+{
+    *launched = false;
+    if (G->schedule == 1) {
+        int rc = ensure_patches(G); if (rc) return rc;
+        if (G->dev.n_patches > 0) { CUDA_TRY(oat_launch_patch(mode, variant, G->dev, src, acc, y, g, counter, st)); *launched = true; }
+    } else if (G->dev.n_items > 0) {
+        CUDA_TRY(oat_launch_ray(mode, variant, G->dev, src, acc, y, g, counter, st)); *launched = true;
+    }
+    return OAT_OK;
+}
+
 int ensure_quads(oat_geometry *G)
 {
     if (G->d_quads) return OAT_OK;
@@ -318,7 +373,9 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     }
     CUDA_TRY(cudaMemsetAsync(G->d_g, 0, sizeof(double) * (G->n_dat ? G->n_dat : 1), st));
     CUDA_TRY(cudaEventRecord(G->ev0, st));
-    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(0, G->variant_project, P, src, nullptr, nullptr, G->d_g, nullptr, st)); ++G->last_launches; }
+    bool launched;
+    { int rc = launch_traversal(G, 0, G->variant_project, src, nullptr, nullptr, G->d_g, nullptr, st, &launched); if (rc) return rc; }
+    if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
     if (G->n_dat > 0) { oat_launch_diff(P, G->d_g, d_y, st); ++G->last_launches; }
@@ -330,7 +387,7 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    const bool quads = G->variant_backproject == 2;
+    const bool quads = G->variant_backproject >= 2;
     float *acc = G->d_xpad;
     if (quads) {
         int rc = ensure_quads(G); if (rc) return rc;
@@ -340,7 +397,9 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
         CUDA_TRY(cudaMemsetAsync(G->d_xpad, 0, sizeof(float) * G->n_pad, st));
     }
     CUDA_TRY(cudaEventRecord(G->ev0, st));
-    if (P.n_items > 0) { CUDA_TRY(oat_launch_ray(1, G->variant_backproject, P, nullptr, acc, d_y, nullptr, nullptr, st)); ++G->last_launches; }
+    bool launched;
+    { int rc = launch_traversal(G, 1, G->variant_backproject, nullptr, acc, d_y, nullptr, nullptr, st, &launched); if (rc) return rc; }
+    if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
     if (quads) oat_launch_unquad(P, G->d_quads, d_x, st);
@@ -430,7 +489,8 @@ int64_t oat_num_surface_samples(oat_geometry *g)
     if (check_handle(g)) return -1;
     if (g->n_surface_samples >= 0) return g->n_surface_samples;
     if (cudaMemset(g->d_counter, 0, sizeof(unsigned long long)) != cudaSuccess) return -1;
-    if (oat_launch_ray(2, 0, g->dev, nullptr, nullptr, nullptr, nullptr, g->d_counter, 0) != cudaSuccess) return -1;
+    bool launched;
+    if (launch_traversal(g, 2, 0, nullptr, nullptr, nullptr, nullptr, g->d_counter, 0, &launched)) return -1;
     unsigned long long v = 0;
     if (cudaMemcpy(&v, g->d_counter, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) {
         fail(OAT_ERR_CUDA, "sample count kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -547,7 +607,13 @@ int oat_set_variant(oat_geometry *g, const char *key, int variant)
 {
     if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");
     if (!strcmp(key, "project")) { if (variant < 0 || variant > 2) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
-    if (!strcmp(key, "backproject")) { if (variant < 0 || variant > 2) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
+    if (!strcmp(key, "backproject")) { if (variant < 0 || variant > 3) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
+    if (!strcmp(key, "morton_shift")) {
+        if (variant < 0 || variant > 10) return fail(OAT_ERR_INVALID, "morton_shift out of range");
+        if (g->morton_shift != variant) { cudaFree(g->d_patches); g->d_patches = nullptr; g->dev.patches = nullptr; g->dev.n_patches = 0; }
+        g->morton_shift = variant; return OAT_OK;
+    }
+    if (!strcmp(key, "schedule")) { if (variant < 0 || variant > 1) return fail(OAT_ERR_INVALID, "unknown schedule %d", variant); g->schedule = variant; return OAT_OK; }
     return fail(OAT_ERR_INVALID, "unknown variant key '%s'", key);
 }
 

@@ -19,6 +19,8 @@
 #define OAT_SB 1024        // candidates per shared-memory sub-batch
 #define OAT_NT 256         // threads per block of the ray kernels
 #define OAT_NW (OAT_NT / 32)
+#define OAT_RI 32          // rings per patch (schedule 1)
+#define OAT_RJ 32          // max azimuth samples per ring of a patch
 
 struct OatBand {
     double s_mid;      // radius of the band's anchor (k0 + (B-1)/2) in voxel units: rho/ds
@@ -27,6 +29,8 @@ struct OatBand {
     int ring_ofs;      // first ring of this band in the ring table
     int n_rings;       // rings with theta_i < pi
     int k0, nk;        // first sample and number of samples (ragged last band: nk < B)
+    int rb_ofs;        // first entry of this band in the ring-block sector table
+    int pad;
 };
 
 struct __align__(16) OatRing {
@@ -50,6 +54,9 @@ struct OatDev {
     const int *qb_rings;
     const long long *item_prefix;
     long long n_items;
+    const int *rb_sectors;               // per (band, ring block): number of azimuth sectors S
+    const unsigned long long *patches;   // schedule 1: Morton-sorted packed (q, band, ring block, sector)
+    long long n_patches;
     int qx, qy;                // quad layout (variant 2): quads per row / rows per plane
     long long qplane;          // qx*qy; one parity array holds pz*qplane float4 quads
     cudaTextureObject_t tex;   // slice atlas of the padded volume (project variant 1), 0 if unused
@@ -67,6 +74,9 @@ void oat_launch_unquad(const OatDev &P, const float4 *quads, float *x, cudaStrea
 void oat_launch_pad_atlas(const OatDev &P, const float *x, cudaSurfaceObject_t surf, cudaStream_t st);
 cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
                            double *g, unsigned long long *counter, cudaStream_t st);
+cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
+                             double *g, unsigned long long *counter, cudaStream_t st);
+cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, unsigned long long **patches_out, long long *n_patches);
 void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st);
 // vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)
 void oat_launch_dot(const float *a, const float *b, long long n, double *out, cudaStream_t st);

@@ -19,6 +19,8 @@
 
 #include <math.h>
 
+#include <cub/device/device_radix_sort.cuh>
+
 namespace {
 
 struct __align__(16) Entry {
@@ -106,6 +108,224 @@ __device__ __forceinline__ void fetch8(const OatDev &P, const float *__restrict_
 
 #define OAT_U 2    // list entries in flight per warp (independent dependency chains)
 
+// Per-lane constants of one (transducer q, band): lane = time sample k of the band.
+struct LaneCtx {
+    int k;
+    double rho;
+    bool active;
+    float delta;   // radial offset of sample k from the band anchor, in voxels
+    float coef;    // MODE 1: g'_k * rho_k^2  (S7, S8)
+};
+
+template <int MODE>
+__device__ __forceinline__ LaneCtx lane_setup(const OatDev &P, const OatBand &band, int q, int lane, const float *__restrict__ y)
+{
+    LaneCtx c;
+    c.k = band.k0 + lane;
+    const double tk = P.t0 + (double)c.k * P.dt;
+    c.rho = P.c * tk;
+    c.active = (lane < band.nk) && (c.rho > 0.0);
+    c.delta = (float)(((double)lane - 0.5 * (double)(P.B - 1)) * P.step);
+    c.coef = 0.f;
+    if (MODE == 1 && c.active) {
+        const float ym = (c.k - 1 >= 0) ? y[(size_t)q * P.K + c.k - 1] : 0.f;
+        const float yp = (c.k + 1 < P.K) ? y[(size_t)q * P.K + c.k + 1] : 0.f;
+        const double sp = P.kappa * ((double)ym - (double)yp) / (2.0 * P.dt);   // Eq. 22
+        c.coef = (float)(sp / tk * c.rho * c.rho);
+    }
+    return c;
+}
+
+// Direction (S3) of ring R, azimuth j in the frame of the transducer, and the ray's anchor point
+// base' + s_mid*u, all in fp64; returns false when the bounding box of the ray segment
+// [s_lo, s_hi] cannot meet the padded node box.
+__device__ __forceinline__ bool make_entry(const OatDev &P, const OatBand &band, const OatRing &R, int j,
+                                           const double *s_frame, Entry &e)
+{
+    double sd, cd;
+    sincospi(2.0 * (double)j / (double)R.N, &sd, &cd);
+    const double dlx = R.st * cd, dly = R.st * sd, dlz = R.ct;
+    float uu[3], af[3];
+    int ai[3];
+    bool hit = true;
+    const float lim[3] = {(float)P.nx + 1.01f, (float)P.ny + 1.01f, (float)P.nz + 1.01f};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double ua = dlx * s_frame[a] + dly * s_frame[3 + a] + dlz * s_frame[6 + a];
+        const double an = s_frame[9 + a] + band.s_mid * ua;
+        const double ar = rint(an);
+        uu[a] = (float)ua;
+        af[a] = (float)(an - ar);
+        ai[a] = (int)ar;
+        const float p0 = (float)(s_frame[9 + a] + (double)band.s_lo * ua);
+        const float p1 = (float)(s_frame[9 + a] + (double)band.s_hi * ua);
+        hit = hit && (fmaxf(p0, p1) >= -0.01f) && (fminf(p0, p1) <= lim[a]);
+    }
+    e.a = make_float4(af[0], af[1], af[2], R.omega);
+    e.u = make_float4(uu[0], uu[1], uu[2], 0.f);
+    e.i = make_int4(ai[0] - OAT_MAGIC_BITS, ai[1] - OAT_MAGIC_BITS, ai[2] - OAT_MAGIC_BITS, 0);
+    return hit;
+}
+
+// CONSUME: one warp per list entry (one ray), lane = time sample; OAT_U entries in flight.
+template <int MODE, int VAR>
+__device__ __forceinline__ void consume_list(const OatDev &P, const Entry *__restrict__ list, int n_list, int warp, int lane,
+                                             const LaneCtx &L, const float *__restrict__ xpad, float *__restrict__ xacc,
+                                             float &acc, unsigned &cnt)
+{
+    const float delta = L.delta, coef = L.coef;
+    const bool active = L.active;
+    for (int e0 = warp; e0 < n_list; e0 += OAT_NW * OAT_U) {
+        Sample s[OAT_U];
+        bool in[OAT_U];
+        float om[OAT_U];
+#pragma unroll
+        for (int u = 0; u < OAT_U; ++u) {
+            const int ei = e0 + u * OAT_NW;
+            const bool valid = ei < n_list;
+            const Entry e = list[valid ? ei : e0];
+            in[u] = lane_sample(P, e, delta, s[u]) && active && valid;
+            om[u] = e.a.w;
+        }
+        if (MODE == 2) {
+#pragma unroll
+            for (int u = 0; u < OAT_U; ++u) cnt += in[u] ? 1u : 0u;
+        } else if (MODE == 0) {
+            float v[OAT_U][8];
+#pragma unroll
+            for (int u = 0; u < OAT_U; ++u) fetch8<VAR>(P, xpad, s[u], in[u], v[u]);
+#pragma unroll
+            for (int u = 0; u < OAT_U; ++u) {
+                const float a00 = fmaf(s[u].fx, v[u][1] - v[u][0], v[u][0]);
+                const float a10 = fmaf(s[u].fx, v[u][3] - v[u][2], v[u][2]);
+                const float a01 = fmaf(s[u].fx, v[u][5] - v[u][4], v[u][4]);
+                const float a11 = fmaf(s[u].fx, v[u][7] - v[u][6], v[u][6]);
+                const float b0 = fmaf(s[u].fy, a10 - a00, a00);
+                const float b1 = fmaf(s[u].fy, a11 - a01, a01);
+                acc = fmaf(in[u] ? om[u] : 0.f, fmaf(s[u].fz, b1 - b0, b0), acc);
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < OAT_U; ++u) {
+                const unsigned idx = (VAR == 2) ? quad_index(P, s[u].ix, s[u].iy, s[u].iz)
+                                                : (unsigned)((s[u].iz * P.py + s[u].iy) * P.px + s[u].ix);
+                const float cw = in[u] ? coef * om[u] : 0.f;
+                const float wz1 = s[u].fz * cw, wz0 = cw - wz1;
+                const float gx = 1.f - s[u].fx, gy = 1.f - s[u].fy;
+                const float w00 = gx * gy, w10 = s[u].fx * gy, w01 = gx * s[u].fy, w11 = s[u].fx * s[u].fy;
+                float w[8] = {w00 * wz0, w10 * wz0, w01 * wz0, w11 * wz0, w00 * wz1, w10 * wz1, w01 * wz1, w11 * wz1};
+                bool writer = in[u];
+                if (VAR >= 1) {
+                    // Lanes step along one ray, so lanes that fall into the same cell are CONSECUTIVE:
+                    // sum each run into its first lane (segmented suffix sum by shuffles) and let only
+                    // run heads issue the atomics (~3x fewer L2 atomic operations).
+                    const unsigned cell = in[u] ? idx : (0xfffffff0u - (unsigned)lane);
+                    const unsigned prev = __shfl_up_sync(0xffffffffu, cell, 1);
+                    const bool head = (lane == 0) || (cell != prev);
+                    const unsigned heads = __ballot_sync(0xffffffffu, head);
+                    const unsigned above = (lane == 31) ? 0u : (heads & ~((2u << lane) - 1u));
+                    const int run_end = above ? (__ffs(above) - 2) : 31;
+                    const unsigned maxrun = __reduce_max_sync(0xffffffffu, (head && in[u]) ? (unsigned)(run_end - lane + 1) : 0u);
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) {
+                        if (maxrun > (unsigned)d) {                    // warp-uniform
+                            const float keep = (lane + d <= run_end) ? 1.f : 0.f;
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) w[c] = fmaf(keep, __shfl_down_sync(0xffffffffu, w[c], d), w[c]);
+                        }
+                    }
+                    writer = in[u] && head;
+                }
+                if (VAR == 2) {
+                    // one aligned 16-byte vector reduction per plane: 2 L2 sector operations per run
+                    if (writer) {
+                        float4 *qp = reinterpret_cast<float4 *>(xacc) + idx;
+                        red_add_v4(qp, w[0], w[1], w[2], w[3]);
+                        red_add_v4(qp + P.qplane, w[4], w[5], w[6], w[7]);
+                    }
+                } else if (writer) {
+                    float *p = xacc + idx;
+                    atomicAdd(p, w[0]);
+                    atomicAdd(p + 1, w[1]);
+                    atomicAdd(p + P.px, w[2]);
+                    atomicAdd(p + P.px + 1, w[3]);
+                    float *p1 = p + P.pxy;
+                    atomicAdd(p1, w[4]);
+                    atomicAdd(p1 + 1, w[5]);
+                    atomicAdd(p1 + P.px, w[6]);
+                    atomicAdd(p1 + P.px + 1, w[7]);
+                }
+            }
+        }
+    }
+}
+
+// CONSUME for H^T, "marching" form (backproject variant 3): one THREAD per ray, stepping through the
+// band's time samples in order.  Consecutive samples of a ray that fall in the same cell are summed in
+// registers and flushed with two 16-byte vector reductions when the ray leaves the cell -- the same
+// run-merging as variant 2 but without any shuffle.  Positions, cells and weights come from the same
+// lane_sample() as in H, with the same per-sample delta (table s_delta), so the sample set is identical.
+__device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid, int nk,
+                                              const float *__restrict__ s_delta, const float *__restrict__ s_coef,
+                                              float *__restrict__ xacc)
+{
+    float4 *__restrict__ quads = reinterpret_cast<float4 *>(xacc);
+    for (int ei = tid; ei < n_list; ei += OAT_NT) {
+        const Entry e = list[ei];
+        unsigned cur = 0xffffffffu;
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f, a5 = 0.f, a6 = 0.f, a7 = 0.f;
+        for (int k = 0; k < nk; ++k) {
+            const float cw0 = s_coef[k];
+            Sample s;
+            const bool in = lane_sample(P, e, s_delta[k], s) && (cw0 != 0.f);
+            const unsigned cell = in ? quad_index(P, s.ix, s.iy, s.iz) : 0xffffffffu;
+            if (cell != cur) {
+                if (cur != 0xffffffffu) {
+                    red_add_v4(quads + cur, a0, a1, a2, a3);
+                    red_add_v4(quads + cur + P.qplane, a4, a5, a6, a7);
+                }
+                a0 = a1 = a2 = a3 = a4 = a5 = a6 = a7 = 0.f;
+                cur = cell;
+            }
+            if (in) {
+                const float cw = cw0 * e.a.w;
+                const float wz1 = s.fz * cw, wz0 = cw - wz1;
+                const float gx = 1.f - s.fx, gy = 1.f - s.fy;
+                const float w00 = gx * gy, w10 = s.fx * gy, w01 = gx * s.fy, w11 = s.fx * s.fy;
+                a0 = fmaf(w00, wz0, a0); a1 = fmaf(w10, wz0, a1); a2 = fmaf(w01, wz0, a2); a3 = fmaf(w11, wz0, a3);
+                a4 = fmaf(w00, wz1, a4); a5 = fmaf(w10, wz1, a5); a6 = fmaf(w01, wz1, a6); a7 = fmaf(w11, wz1, a7);
+            }
+        }
+        if (cur != 0xffffffffu) {
+            red_add_v4(quads + cur, a0, a1, a2, a3);
+            red_add_v4(quads + cur + P.qplane, a4, a5, a6, a7);
+        }
+    }
+}
+
+// EPILOGUE of one work item: cross-warp combine in fp64 and one fp64 atomic per time sample (S5)
+template <int MODE>
+__device__ __forceinline__ void item_epilogue(const OatDev &P, int q, const LaneCtx &L, float acc, unsigned cnt, int warp, int lane,
+                                              float (*s_red)[32], double *__restrict__ g, unsigned long long *__restrict__ counter)
+{
+    if (MODE == 0) {
+        s_red[warp][lane] = acc;
+        __syncthreads();
+        if (warp == 0) {
+            double sum = 0.0;
+#pragma unroll
+            for (int w = 0; w < OAT_NW; ++w) sum += (double)s_red[w][lane];
+            if (L.active && sum != 0.0) atomicAdd(&g[(size_t)q * P.K + L.k], L.rho * L.rho * sum);
+        }
+    } else if (MODE == 2) {
+        const double tot = warp_sum((double)cnt);
+        if (lane == 0 && tot > 0) atomicAdd(counter, (unsigned long long)tot);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Schedule 0: work item = chunk of OAT_CH candidate directions (ring-major) of one (q, band)
+// ------------------------------------------------------------------------------------------------
 template <int MODE, int VAR>
 __global__ void __launch_bounds__(OAT_NT, 2)
 oat_ray_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict__ xacc,
@@ -146,25 +366,13 @@ oat_ray_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict
         const long long c_begin = (item - P.item_prefix[qb]) * (long long)OAT_CH;
         const int c_end = (int)min((long long)n_cand, c_begin + OAT_CH);
 
-        // lane = time sample of the band
-        const int k = band.k0 + lane;
-        const double tk = P.t0 + (double)k * P.dt;
-        const double rho = P.c * tk;
-        const bool active = (lane < band.nk) && (rho > 0.0);
-        const float delta = (float)(((double)lane - 0.5 * (double)(P.B - 1)) * P.step);
-        float coef = 0.f;                                 // MODE 1: g'_k * rho_k^2  (S7, S8)
-        if (MODE == 1 && active) {
-            const float ym = (k - 1 >= 0) ? y[(size_t)q * P.K + k - 1] : 0.f;
-            const float yp = (k + 1 < P.K) ? y[(size_t)q * P.K + k + 1] : 0.f;
-            const double sp = P.kappa * ((double)ym - (double)yp) / (2.0 * P.dt);   // Eq. 22
-            coef = (float)(sp / tk * rho * rho);
-        }
+        const LaneCtx L = lane_setup<MODE>(P, band, q, lane, y);
         float acc = 0.f;
         unsigned cnt = 0;
         __syncthreads();                                  // s_frame ready
         // every warp maps lane -> k the same way, so this vote is uniform over the block:
         // a band whose 32 data values give g' = 0 contributes exactly nothing to H^T y
-        const bool live = (MODE != 1) || __any_sync(0xffffffffu, coef != 0.f);
+        const bool live = (MODE != 1) || __any_sync(0xffffffffu, L.coef != 0.f);
 
         for (int sb = (int)c_begin; live && sb < c_end; sb += OAT_SB) {
             if (tid == 0) s_count = 0;
@@ -179,7 +387,7 @@ oat_ray_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict
                 }
                 const OatRing R = ring[lo];
                 const int j = c - R.cum;
-                // fp32 pre-test: bounding box of the ray segment against the padded box
+                // cheap fp32 pre-test (2.7x more candidates than hits in this schedule)
                 float sp, cp;
                 sincospif(2.0f * (float)j / (float)R.N, &sp, &cp);
                 const float stf = (float)R.st, ctf = (float)R.ct;
@@ -194,132 +402,151 @@ oat_ray_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict
                     hit = hit && (fmaxf(p0, p1) >= -0.01f) && (fminf(p0, p1) <= lim[a]);
                 }
                 if (!hit) continue;
-                // survivors: direction (S3) and anchor in fp64
-                double sd, cd;
-                sincospi(2.0 * (double)j / (double)R.N, &sd, &cd);
-                const double dlx = R.st * cd, dly = R.st * sd, dlz = R.ct;
                 Entry e;
-                float uu[3], af[3];
-                int ai[3];
-#pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    const double ua = dlx * s_frame[a] + dly * s_frame[3 + a] + dlz * s_frame[6 + a];
-                    const double an = s_frame[9 + a] + band.s_mid * ua;
-                    const double ar = rint(an);
-                    uu[a] = (float)ua;
-                    af[a] = (float)(an - ar);
-                    ai[a] = (int)ar;
-                }
-                e.a = make_float4(af[0], af[1], af[2], R.omega);
-                e.u = make_float4(uu[0], uu[1], uu[2], 0.f);
-                e.i = make_int4(ai[0] - OAT_MAGIC_BITS, ai[1] - OAT_MAGIC_BITS, ai[2] - OAT_MAGIC_BITS, 0);
-                const int slot = atomicAdd(&s_count, 1);
-                list[slot] = e;
+                if (!make_entry(P, band, R, j, s_frame, e)) continue;
+                list[atomicAdd(&s_count, 1)] = e;
             }
             __syncthreads();
             // ------------------------------------------------------------ consume
-            const int n_list = s_count;
-            for (int e0 = warp; e0 < n_list; e0 += OAT_NW * OAT_U) {
-                Sample s[OAT_U];
-                bool in[OAT_U];
-                float om[OAT_U];
-#pragma unroll
-                for (int u = 0; u < OAT_U; ++u) {
-                    const int ei = e0 + u * OAT_NW;
-                    const bool valid = ei < n_list;
-                    const Entry e = list[valid ? ei : e0];
-                    in[u] = lane_sample(P, e, delta, s[u]) && active && valid;
-                    om[u] = e.a.w;
-                }
-                if (MODE == 2) {
-#pragma unroll
-                    for (int u = 0; u < OAT_U; ++u) cnt += in[u] ? 1u : 0u;
-                } else if (MODE == 0) {
-                    float v[OAT_U][8];
-#pragma unroll
-                    for (int u = 0; u < OAT_U; ++u) fetch8<VAR>(P, xpad, s[u], in[u], v[u]);
-#pragma unroll
-                    for (int u = 0; u < OAT_U; ++u) {
-                        const float a00 = fmaf(s[u].fx, v[u][1] - v[u][0], v[u][0]);
-                        const float a10 = fmaf(s[u].fx, v[u][3] - v[u][2], v[u][2]);
-                        const float a01 = fmaf(s[u].fx, v[u][5] - v[u][4], v[u][4]);
-                        const float a11 = fmaf(s[u].fx, v[u][7] - v[u][6], v[u][6]);
-                        const float b0 = fmaf(s[u].fy, a10 - a00, a00);
-                        const float b1 = fmaf(s[u].fy, a11 - a01, a01);
-                        acc = fmaf(in[u] ? om[u] : 0.f, fmaf(s[u].fz, b1 - b0, b0), acc);
-                    }
-                } else {
-#pragma unroll
-                    for (int u = 0; u < OAT_U; ++u) {
-                        const unsigned idx = (VAR == 2) ? quad_index(P, s[u].ix, s[u].iy, s[u].iz)
-                                                        : (unsigned)((s[u].iz * P.py + s[u].iy) * P.px + s[u].ix);
-                        const float cw = in[u] ? coef * om[u] : 0.f;
-                        const float wz1 = s[u].fz * cw, wz0 = cw - wz1;
-                        const float gx = 1.f - s[u].fx, gy = 1.f - s[u].fy;
-                        const float w00 = gx * gy, w10 = s[u].fx * gy, w01 = gx * s[u].fy, w11 = s[u].fx * s[u].fy;
-                        float w[8] = {w00 * wz0, w10 * wz0, w01 * wz0, w11 * wz0, w00 * wz1, w10 * wz1, w01 * wz1, w11 * wz1};
-                        bool writer = in[u];
-                        if (VAR >= 1) {
-                            // Lanes step along one ray, so lanes that fall into the same cell are CONSECUTIVE:
-                            // sum each run into its first lane (segmented suffix sum by shuffles) and let only
-                            // run heads issue the atomics (~3x fewer L2 atomic operations).
-                            const unsigned cell = in[u] ? idx : (0xfffffff0u - (unsigned)lane);
-                            const unsigned prev = __shfl_up_sync(0xffffffffu, cell, 1);
-                            const bool head = (lane == 0) || (cell != prev);
-                            const unsigned heads = __ballot_sync(0xffffffffu, head);
-                            const unsigned above = (lane == 31) ? 0u : (heads & ~((2u << lane) - 1u));
-                            const int run_end = above ? (__ffs(above) - 2) : 31;
-                            const unsigned maxrun = __reduce_max_sync(0xffffffffu, (head && in[u]) ? (unsigned)(run_end - lane + 1) : 0u);
-#pragma unroll
-                            for (int d = 1; d < 32; d <<= 1) {
-                                if (maxrun > (unsigned)d) {                    // warp-uniform
-                                    const float keep = (lane + d <= run_end) ? 1.f : 0.f;
-#pragma unroll
-                                    for (int c = 0; c < 8; ++c) w[c] = fmaf(keep, __shfl_down_sync(0xffffffffu, w[c], d), w[c]);
-                                }
-                            }
-                            writer = in[u] && head;
-                        }
-                        if (VAR == 2) {
-                            // one aligned 16-byte vector reduction per plane: 2 L2 sector operations per run
-                            if (writer) {
-                                float4 *qp = reinterpret_cast<float4 *>(xacc) + idx;
-                                red_add_v4(qp, w[0], w[1], w[2], w[3]);
-                                red_add_v4(qp + P.qplane, w[4], w[5], w[6], w[7]);
-                            }
-                        } else if (writer) {
-                            float *p = xacc + idx;
-                            atomicAdd(p, w[0]);
-                            atomicAdd(p + 1, w[1]);
-                            atomicAdd(p + P.px, w[2]);
-                            atomicAdd(p + P.px + 1, w[3]);
-                            float *p1 = p + P.pxy;
-                            atomicAdd(p1, w[4]);
-                            atomicAdd(p1 + 1, w[5]);
-                            atomicAdd(p1 + P.px, w[6]);
-                            atomicAdd(p1 + P.px + 1, w[7]);
-                        }
-                    }
-                }
-            }
+            consume_list<MODE, VAR>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
             __syncthreads();                              // list is rebuilt next round
         }
-
-        // ---------------------------------------------------------------- epilogue
-        if (MODE == 0) {
-            s_red[warp][lane] = acc;
-            __syncthreads();
-            if (warp == 0) {
-                double sum = 0.0;
-#pragma unroll
-                for (int w = 0; w < OAT_NW; ++w) sum += (double)s_red[w][lane];
-                if (active && sum != 0.0) atomicAdd(&g[(size_t)q * P.K + k], rho * rho * sum);   // S5
-            }
-        } else if (MODE == 2) {
-            const double tot = warp_sum((double)cnt);
-            if (lane == 0 && tot > 0) atomicAdd(counter, (unsigned long long)tot);
-        }
+        item_epilogue<MODE>(P, q, L, acc, cnt, warp, lane, s_red, g, counter);
         __syncthreads();                                  // s_qb, s_frame, s_red reused by the next item
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Schedule 1: work item = PATCH = (q, band, block of OAT_RI rings, azimuth sector): a compact piece of
+// shell, ~32 x 32 x (B c dt / ds) voxels.  Items are generated and culled on the device at geometry
+// creation and sorted by the Morton code of their position, so the blocks in flight at any time all
+// work inside the same small sub-volume: the volume / the accumulators they touch stay in L1/L2.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void unpack_item(unsigned long long v, int &q, int &b, int &rb, int &s)
+{
+    s = (int)(v & 0xffffu);
+    rb = (int)((v >> 16) & 0x3ffu);
+    b = (int)((v >> 26) & 0xfffu);
+    q = (int)(v >> 38);
+}
+
+template <int MODE, int VAR>
+__global__ void __launch_bounds__(OAT_NT, 2)
+oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict__ xacc,
+                 const float *__restrict__ y, double *__restrict__ g, unsigned long long *__restrict__ counter)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Entry *list = reinterpret_cast<Entry *>(smem_raw);
+    __shared__ double s_frame[12];
+    __shared__ float s_red[OAT_NW][32];
+    __shared__ float s_delta[32], s_coef[32];
+    __shared__ int s_count;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (long long item = blockIdx.x; item < P.n_patches; item += gridDim.x) {
+        int q, b, rb, sec;
+        unpack_item(P.patches[item], q, b, rb, sec);
+        if (tid < 12) s_frame[tid] = P.frame[(size_t)q * 12 + tid];
+        if (tid == 0) s_count = 0;
+        const OatBand band = P.band[b];
+        const OatRing *__restrict__ ring = P.ring + band.ring_ofs;
+        const int r0 = rb * OAT_RI;
+        const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
+        const int S = P.rb_sectors[band.rb_ofs + rb];
+        const LaneCtx L = lane_setup<MODE>(P, band, q, lane, y);
+        if (MODE == 1 && VAR == 3 && warp == 0) { s_delta[lane] = L.delta; s_coef[lane] = L.active ? L.coef : 0.f; }
+        float acc = 0.f;
+        unsigned cnt = 0;
+        __syncthreads();
+        const bool live = (MODE != 1) || __any_sync(0xffffffffu, L.coef != 0.f);
+        if (live) {
+            // ---------------------------------------------------------------- build
+            for (int t = tid; t < OAT_RI * OAT_RJ; t += OAT_NT) {
+                const int r = r0 + t / OAT_RJ, jl = t % OAT_RJ;
+                if (r >= r1) break;
+                const OatRing R = ring[r];
+                const int j0 = (int)(((long long)R.N * sec + S - 1) / S);
+                const int j1 = (int)(((long long)R.N * (sec + 1) + S - 1) / S);
+                if (j0 + jl >= j1) continue;
+                Entry e;
+                if (!make_entry(P, band, R, j0 + jl, s_frame, e)) continue;
+                list[atomicAdd(&s_count, 1)] = e;
+            }
+            __syncthreads();
+            // ---------------------------------------------------------------- consume
+            if (MODE == 1 && VAR == 3) consume_march(P, list, s_count, tid, band.nk, s_delta, s_coef, xacc);
+            else consume_list<MODE, (VAR == 3 ? 2 : VAR)>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
+        }
+        item_epilogue<MODE>(P, q, L, acc, cnt, warp, lane, s_red, g, counter);
+        __syncthreads();
+    }
+}
+
+// Patch generation (once per geometry): one block per (q, band); threads stride over (ring block,
+// sector); a patch whose bounding sphere can meet the padded node box is appended as
+// (Morton key of its centre, packed descriptor).
+__device__ __forceinline__ unsigned part1by2(unsigned x)
+{
+    x &= 0x3ffu;
+    x = (x | (x << 16)) & 0x30000ffu;
+    x = (x | (x << 8)) & 0x300f00fu;
+    x = (x | (x << 4)) & 0x30c30c3u;
+    x = (x | (x << 2)) & 0x9249249u;
+    return x;
+}
+
+__global__ void oat_gen_patches_kernel(const OatDev P, unsigned *__restrict__ keys, unsigned long long *__restrict__ vals,
+                                       unsigned long long *__restrict__ n_out, unsigned long long cap, int shift)
+{
+    const int qb = blockIdx.x;
+    const int q = qb / P.NB, b = qb - q * P.NB;
+    const int nr = P.qb_rings[qb];
+    if (nr <= 0) return;
+    const OatBand band = P.band[b];
+    const OatRing *__restrict__ ring = P.ring + band.ring_ofs;
+    const double *f = P.frame + (size_t)q * 12;
+    const int n_rb = (nr + OAT_RI - 1) / OAT_RI;
+    // flatten (rb, sector) with a running offset per ring block
+    int total = 0;
+    for (int rb = 0; rb < n_rb; ++rb) total += P.rb_sectors[band.rb_ofs + rb];
+    for (int t = threadIdx.x; t < total; t += blockDim.x) {
+        int rb = 0, sec = t;
+        while (sec >= P.rb_sectors[band.rb_ofs + rb]) { sec -= P.rb_sectors[band.rb_ofs + rb]; ++rb; }
+        const int S = P.rb_sectors[band.rb_ofs + rb];
+        const int r0 = rb * OAT_RI, r1 = min(r0 + OAT_RI, nr);
+        // patch centre direction and angular radius
+        const double th0 = (double)(r0 + 1) * band.dtheta, th1 = (double)r1 * band.dtheta;   // ring index r <-> theta = (r+1) dtheta
+        const double thc = 0.5 * (th0 + th1);
+        const double phc = 2.0 * 3.14159265358979323846 * ((double)sec + 0.5) / (double)S;
+        const double smax = fmax(sin(th0), fmax(sin(th1), (th0 < 1.5707963267948966 && th1 > 1.5707963267948966) ? 1.0 : 0.0));
+        const double half_th = 0.5 * (th1 - th0) + band.dtheta;
+        const double half_ph = (3.14159265358979323846 / (double)S + 6.3 / (double)ring[r0].N) * smax;
+        const double gamma = sqrt(half_th * half_th + half_ph * half_ph);
+        double sc, cc; sincos(phc, &sc, &cc);
+        const double st = sin(thc), ct = cos(thc);
+        double cen[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const double ua = st * cc * f[a] + st * sc * f[3 + a] + ct * f[6 + a];
+            cen[a] = f[9 + a] + band.s_mid * ua;             // padded voxel coordinates
+        }
+        const double rad = (double)band.s_hi * fmin(gamma, 3.2) * 1.02 + 0.5 * ((double)band.s_hi - (double)band.s_lo) + 2.0;
+        const double hi[3] = {(double)P.nx + 1.0, (double)P.ny + 1.0, (double)P.nz + 1.0};
+        double d2 = 0.0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const double d = cen[a] < 0.0 ? -cen[a] : (cen[a] > hi[a] ? cen[a] - hi[a] : 0.0);
+            d2 += d * d;
+        }
+        if (d2 > rad * rad) continue;
+        unsigned cx = (unsigned)fmin(fmax(cen[0], 0.0), hi[0]) >> shift, cy = (unsigned)fmin(fmax(cen[1], 0.0), hi[1]) >> shift,
+                 cz = (unsigned)fmin(fmax(cen[2], 0.0), hi[2]) >> shift;
+        const unsigned key = part1by2(cx) | (part1by2(cy) << 1) | (part1by2(cz) << 2);
+        const unsigned long long slot = atomicAdd(n_out, 1ULL);
+        if (slot < cap) {
+            keys[slot] = key;
+            vals[slot] = ((unsigned long long)q << 38) | ((unsigned long long)b << 26) | ((unsigned long long)rb << 16) | (unsigned long long)sec;
+        }
     }
 }
 
@@ -507,6 +734,74 @@ static cudaError_t launch_ray_t(const OatDev &P, const float *xpad, float *xacc,
     return cudaGetLastError();
 }
 
+template <int MODE, int VAR>
+static cudaError_t launch_patch_t(const OatDev &P, const float *xpad, float *xacc, const float *y, double *g,
+                                  unsigned long long *counter, cudaStream_t st)
+{
+    const size_t smem = sizeof(Entry) * OAT_RI * OAT_RJ;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(oat_patch_kernel<MODE, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e) return e;
+        attr_set = true;
+    }
+    const long long cap = 0x7fffffffLL;
+    const unsigned grid = (unsigned)(P.n_patches < cap ? P.n_patches : cap);
+    oat_patch_kernel<MODE, VAR><<<grid, OAT_NT, smem, st>>>(P, xpad, xacc, y, g, counter);
+    return cudaGetLastError();
+}
+
+cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
+                             double *g, unsigned long long *counter, cudaStream_t st)
+{
+    if (P.n_patches <= 0) return cudaSuccess;
+    if (mode == 0) return variant == 2 ? launch_patch_t<0, 2>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 1 ? launch_patch_t<0, 1>(P, xpad, xacc, y, g, counter, st)
+                                       : launch_patch_t<0, 0>(P, xpad, xacc, y, g, counter, st);
+    if (mode == 1) return variant == 3 ? launch_patch_t<1, 3>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 2 ? launch_patch_t<1, 2>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 1 ? launch_patch_t<1, 1>(P, xpad, xacc, y, g, counter, st)
+                                       : launch_patch_t<1, 0>(P, xpad, xacc, y, g, counter, st);
+    return launch_patch_t<2, 0>(P, xpad, xacc, y, g, counter, st);
+}
+
+// Generates the patch list of a geometry on the device and sorts it by Morton key.  `cap` is the
+// host-computed upper bound on the number of patches.  On return *n_patches is the number generated;
+// *patches_out is a device buffer the caller owns.
+cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, unsigned long long **patches_out, long long *n_patches)
+{
+    *patches_out = nullptr; *n_patches = 0;
+    if (cap == 0 || P.Q == 0) return cudaSuccess;
+    unsigned *keys = nullptr, *keys2 = nullptr;
+    unsigned long long *vals = nullptr, *vals2 = nullptr, *cnt = nullptr;
+    void *tmp = nullptr;
+    cudaError_t e = cudaSuccess;
+    auto cleanup = [&]() { cudaFree(keys); cudaFree(keys2); cudaFree(vals); cudaFree(cnt); cudaFree(tmp); };
+#define OAT_TRY(x) do { e = (x); if (e != cudaSuccess) { cleanup(); cudaFree(vals2); return e; } } while (0)
+    OAT_TRY(cudaMalloc((void **)&keys, sizeof(unsigned) * cap));
+    OAT_TRY(cudaMalloc((void **)&vals, sizeof(unsigned long long) * cap));
+    OAT_TRY(cudaMalloc((void **)&cnt, sizeof(unsigned long long)));
+    OAT_TRY(cudaMemset(cnt, 0, sizeof(unsigned long long)));
+    oat_gen_patches_kernel<<<(unsigned)((long long)P.Q * P.NB), 128>>>(P, keys, vals, cnt, cap, shift);
+    OAT_TRY(cudaGetLastError());
+    unsigned long long n = 0;
+    OAT_TRY(cudaMemcpy(&n, cnt, sizeof(n), cudaMemcpyDeviceToHost));
+    if (n > cap) { cleanup(); return cudaErrorInvalidValue; }
+    if (n == 0) { cleanup(); return cudaSuccess; }
+    OAT_TRY(cudaMalloc((void **)&keys2, sizeof(unsigned) * n));
+    OAT_TRY(cudaMalloc((void **)&vals2, sizeof(unsigned long long) * n));
+    size_t tmp_bytes = 0;
+    OAT_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, (long long)n, 0, 30));
+    OAT_TRY(cudaMalloc(&tmp, tmp_bytes));
+    OAT_TRY(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, (long long)n, 0, 30));
+    OAT_TRY(cudaDeviceSynchronize());
+#undef OAT_TRY
+    cleanup();
+    *patches_out = vals2;
+    *n_patches = (long long)n;
+    return cudaSuccess;
+}
+
 cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
                            double *g, unsigned long long *counter, cudaStream_t st)
 {
@@ -514,7 +809,7 @@ cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *
     if (mode == 0) return variant == 2 ? launch_ray_t<0, 2>(P, xpad, xacc, y, g, counter, st)
                         : variant == 1 ? launch_ray_t<0, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_ray_t<0, 0>(P, xpad, xacc, y, g, counter, st);
-    if (mode == 1) return variant == 2 ? launch_ray_t<1, 2>(P, xpad, xacc, y, g, counter, st)
+    if (mode == 1) return variant >= 2 ? launch_ray_t<1, 2>(P, xpad, xacc, y, g, counter, st)
                         : variant == 1 ? launch_ray_t<1, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_ray_t<1, 0>(P, xpad, xacc, y, g, counter, st);
     return launch_ray_t<2, 0>(P, xpad, xacc, y, g, counter, st);

@@ -249,18 +249,37 @@ def test_config4_cgls_first_iterations(env):
 
 
 # ------------------------------------------------------------------ kernel variants
-@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 1), ("project", 2), ("backproject", 0), ("backproject", 1), ("backproject", 2)])
-def test_every_kernel_variant_matches_the_oracle(env, key, variant):
-    """each selectable kernel variant computes the same operator."""
+@pytest.mark.parametrize("schedule", [0, 1])
+@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 1), ("project", 2),
+                                         ("backproject", 0), ("backproject", 1), ("backproject", 2), ("backproject", 3)])
+def test_every_kernel_variant_matches_the_oracle(env, key, variant, schedule):
+    """each selectable kernel variant / work schedule computes the same operator."""
     torch, orc, oat, wl = env
-    w = wl.small(n=18, q=5, nt=75, kband=32)
+    w = wl.small(n=18, q=5, nt=75, kband=32, h=0.2)        # h < spacing: several patches per ring block
     x, y = w.phantom(), w.data_noise()
     g = oat.oat_geometry_create(w)
+    oat.oat_set_variant(g, "schedule", schedule)
     oat.oat_set_variant(g, key, variant)
     if key == "project":
         e = rel_l2(gpu_project(torch, oat, w, x, g), orc.project(w, x.astype(np.float64)))
     else:
         e = rel_l2(gpu_backproject(torch, oat, w, y, g), orc.backproject(w, y.astype(np.float64)))
     _, _, rel = oat.oat_adjoint_check(g, torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda())
+    cnt = oat.oat_num_surface_samples(g)
     g.close()
-    assert e <= TOL and rel <= TOL, (key, variant, e, rel)
+    assert e <= TOL and rel <= TOL, (key, variant, schedule, e, rel)
+    assert abs(cnt - orc.count_samples(w)) <= 2
+
+
+def test_both_schedules_on_config1(env):
+    torch, orc, oat, wl = env
+    w = wl.config(1)
+    x, y = w.phantom(), w.data_noise()
+    ref_hx, ref_hty, ref_cnt = orc.project(w, x.astype(np.float64)), orc.backproject(w, y.astype(np.float64)), orc.count_samples(w)
+    for schedule in (0, 1):
+        g = oat.oat_geometry_create(w)
+        oat.oat_set_variant(g, "schedule", schedule)
+        assert rel_l2(gpu_project(torch, oat, w, x, g), ref_hx) <= TOL
+        assert rel_l2(gpu_backproject(torch, oat, w, y, g), ref_hty) <= TOL
+        assert abs(oat.oat_num_surface_samples(g) - ref_cnt) <= max(2, 1e-6 * ref_cnt)
+        g.close()
