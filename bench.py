@@ -254,7 +254,7 @@ def run_ours(args):
         dom = "backproject" if k_t >= k_h else "project"
         k_ms = max(k_t, k_h)
         achieved = n_samples * FLOP_PER_SAMPLE / (k_ms * 1e-3) / 1e12 if k_ms > 0 else 0.0
-        roofline = {"bound": "alu", "kernel": f"oat_ray_kernel<{1 if dom == 'backproject' else 0}> ({dom})",
+        roofline = {"bound": "alu", "kernel": f"oat_patch_kernel<{1 if dom == 'backproject' else 0},*> ({dom})",
                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak else None,
                     "traffic": None, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_step if ms_step else None,
                     "peak_source": f"148 SM x 128 fp32 lanes x 2 flop x {peak_src}",

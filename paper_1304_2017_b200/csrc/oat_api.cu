@@ -57,6 +57,8 @@ struct oat_geometry {
     float *d_xpad = nullptr;                  // padded volume (gather source / scatter target)
     float4 *d_quads = nullptr;                // 4 parity-shifted quad arrays (variant 2, lazy)
     size_t n_quads = 0;
+    float4 *d_octs = nullptr;                 // 8 parity-shifted octet arrays (project variant 3, lazy)
+    size_t n_octs = 0;                        // in float4 units
     double *d_g = nullptr;                    // Q*K SRT accumulator
     float *d_y2 = nullptr, *d_x2 = nullptr;   // adjoint check / CGLS / host entry points (lazy)
     float *d_x3 = nullptr, *d_y3 = nullptr, *d_x4 = nullptr;   // CGLS vectors (lazy)
@@ -64,7 +66,7 @@ struct oat_geometry {
     unsigned long long *d_counter = nullptr;
     double *h_scal = nullptr;                 // pinned mirror of d_scal
     long long n_surface_samples = -1;
-    int variant_project = 1, variant_backproject = 2;   // measured best
+    int variant_project = 3, variant_backproject = 3;   // measured best
     cudaArray_t atlas = nullptr;              // slice atlas for the texture-gather projection (lazy)
     cudaTextureObject_t tex = 0;
     cudaSurfaceObject_t surf = 0;
@@ -82,7 +84,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
-    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches);
+    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
     if (g->atlas) cudaFreeArray(g->atlas);
@@ -272,11 +274,14 @@ int build_geometry(oat_geometry *G)
     P.tex = 0; P.atlas_shift = 0; P.atlas_mask = 0;
     P.qx = (d.nx + 2) / 2 + 1; P.qy = (d.ny + 2) / 2 + 1;
     P.qplane = (long long)P.qx * P.qy;
+    P.oz = (d.nz + 2) / 2 + 1;
 
     G->n_vox = (size_t)d.nx * d.ny * d.nz;
     G->n_dat = (size_t)Q * K;
     G->n_pad = (size_t)P.pz * P.pxy;
     G->n_quads = 4 * (size_t)P.pz * (size_t)P.qplane;
+    G->n_octs = 2 * 8 * (size_t)P.oz * (size_t)P.qplane;
+    if (G->n_octs / 2 >= (1ULL << 31)) return fail(OAT_ERR_INVALID, "grid too large for the octet layout");
     if (G->n_pad >= (1ULL << 31)) return fail(OAT_ERR_INVALID, "padded grid has more than 2^31 nodes");
     CUDA_TRY(cudaMalloc((void **)&G->d_xpad, sizeof(float) * G->n_pad));
     CUDA_TRY(cudaMalloc((void **)&G->d_g, sizeof(double) * (G->n_dat ? G->n_dat : 1)));
@@ -361,7 +366,11 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     const OatDev &P = G->dev;
     G->last_launches = 0;
     const float *src = G->d_xpad;
-    if (G->variant_project == 2) {
+    if (G->variant_project == 3) {
+        if (!G->d_octs) CUDA_TRY(cudaMalloc((void **)&G->d_octs, sizeof(float4) * G->n_octs));
+        oat_launch_pad_octs(P, d_x, G->d_octs, st); ++G->last_launches;
+        src = reinterpret_cast<const float *>(G->d_octs);
+    } else if (G->variant_project == 2) {
         int rc = ensure_quads(G); if (rc) return rc;
         oat_launch_pad_quads(P, d_x, G->d_quads, st); ++G->last_launches;
         src = reinterpret_cast<const float *>(G->d_quads);
@@ -606,7 +615,7 @@ int oat_cgls(oat_geometry *g, const float *d_y, float *d_x, int n_iter, double *
 int oat_set_variant(oat_geometry *g, const char *key, int variant)
 {
     if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");
-    if (!strcmp(key, "project")) { if (variant < 0 || variant > 2) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
+    if (!strcmp(key, "project")) { if (variant < 0 || variant > 3) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
     if (!strcmp(key, "backproject")) { if (variant < 0 || variant > 3) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
     if (!strcmp(key, "morton_shift")) {
         if (variant < 0 || variant > 10) return fail(OAT_ERR_INVALID, "morton_shift out of range");

@@ -59,6 +59,7 @@ struct OatDev {
     long long n_patches;
     int qx, qy;                // quad layout (variant 2): quads per row / rows per plane
     long long qplane;          // qx*qy; one parity array holds pz*qplane float4 quads
+    int oz;                    // octet layout (project variant 3): bricks along z; 8 arrays of oz*qplane records of 32 B
     cudaTextureObject_t tex;   // slice atlas of the padded volume (project variant 1), 0 if unused
     int atlas_shift, atlas_mask;   // slice z sits at column (z & mask), row (z >> shift) of the atlas
 };
@@ -70,6 +71,7 @@ void oat_launch_unpad(const OatDev &P, const float *xpad, float *x, cudaStream_t
 // quad layout: 4 parity-shifted arrays of xy-quads {(x0,y0),(x0+1,y0),(x0,y0+1),(x0+1,y0+1)} with
 // x0 = 2a + (p&1), y0 = 2b + (p>>1): the four in-plane corners of ANY cell are one aligned float4
 void oat_launch_pad_quads(const OatDev &P, const float *x, float4 *quads, cudaStream_t st);
+void oat_launch_pad_octs(const OatDev &P, const float *x, float4 *octs, cudaStream_t st);
 void oat_launch_unquad(const OatDev &P, const float4 *quads, float *x, cudaStream_t st);
 void oat_launch_pad_atlas(const OatDev &P, const float *x, cudaSurfaceObject_t surf, cudaStream_t st);
 cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,

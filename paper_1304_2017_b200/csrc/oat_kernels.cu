@@ -88,6 +88,13 @@ __device__ __forceinline__ void fetch8(const OatDev &P, const float *__restrict_
         const float *p1 = p + P.pxy;
         v[4] = __ldg(p1); v[5] = __ldg(p1 + 1);
         v[6] = __ldg(p1 + P.px); v[7] = __ldg(p1 + P.px + 1);
+    } else if (VAR == 3) {                                // ONE 256-bit load from the parity-shifted octet arrays
+        const int par = (ix & 1) | ((iy & 1) << 1) | ((iz & 1) << 2);
+        const unsigned oi = (unsigned)(((par * P.oz + (iz >> 1)) * P.qy + (iy >> 1)) * P.qx + (ix >> 1));
+        const float *op = xpad + (size_t)oi * 8;
+        asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+                     : "l"(op));
     } else if (VAR == 2) {                                // 2 x LDG.128 from the parity-shifted quad arrays
         const float4 *qp = reinterpret_cast<const float4 *>(xpad) + quad_index(P, ix, iy, iz);
         const float4 lo = __ldg(qp), hi = __ldg(qp + P.qplane);
@@ -106,7 +113,7 @@ __device__ __forceinline__ void fetch8(const OatDev &P, const float *__restrict_
     }
 }
 
-#define OAT_U 2    // list entries in flight per warp (independent dependency chains)
+#define OAT_U 4    // list entries in flight per warp (independent dependency chains)
 
 // Per-lane constants of one (transducer q, band): lane = time sample k of the band.
 struct LaneCtx {
@@ -274,6 +281,7 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
         const Entry e = list[ei];
         unsigned cur = 0xffffffffu;
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f, a5 = 0.f, a6 = 0.f, a7 = 0.f;
+#pragma unroll 2
         for (int k = 0; k < nk; ++k) {
             const float cw0 = s_coef[k];
             Sample s;
@@ -431,7 +439,7 @@ __device__ __forceinline__ void unpack_item(unsigned long long v, int &q, int &b
 }
 
 template <int MODE, int VAR>
-__global__ void __launch_bounds__(OAT_NT, 2)
+__global__ void __launch_bounds__(OAT_NT, 3)
 oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict__ xacc,
                  const float *__restrict__ y, double *__restrict__ g, unsigned long long *__restrict__ counter)
 {
@@ -475,7 +483,7 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
             __syncthreads();
             // ---------------------------------------------------------------- consume
             if (MODE == 1 && VAR == 3) consume_march(P, list, s_count, tid, band.nk, s_delta, s_coef, xacc);
-            else consume_list<MODE, (VAR == 3 ? 2 : VAR)>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
+            else consume_list<MODE, ((MODE == 1 && VAR == 3) ? 2 : VAR)>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
         }
         item_epilogue<MODE>(P, q, L, acc, cnt, warp, lane, s_red, g, counter);
         __syncthreads();
@@ -584,6 +592,30 @@ __global__ void oat_pad_quads_kernel(const OatDev P, const float *__restrict__ x
                        ? x[((size_t)(z - 1) * P.ny + (Y - 1)) * P.nx + (X - 1)] : 0.f;
         }
         quads[i] = make_float4(v[0], v[1], v[2], v[3]);
+    }
+}
+
+// octet arrays from x: array p = (px | py<<1 | pz<<2) holds 2x2x2 bricks with origin (2a+px, 2b+py, 2c+pz)
+// in padded coordinates, 8 floats = one aligned 32-byte record = all 8 corners of the cell at that origin
+__global__ void oat_pad_octs_kernel(const OatDev P, const float *__restrict__ x, float4 *__restrict__ octs)
+{
+    const long long n = 8LL * P.oz * P.qplane;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int a = (int)(i % P.qx);
+        long long r = i / P.qx;
+        const int b = (int)(r % P.qy); r /= P.qy;
+        const int c = (int)(r % P.oz);
+        const int par = (int)(r / P.oz);
+        const int x0 = 2 * a + (par & 1), y0 = 2 * b + ((par >> 1) & 1), z0 = 2 * c + (par >> 2);
+        float v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int X = x0 + (k & 1), Y = y0 + ((k >> 1) & 1), Z = z0 + (k >> 2);
+            v[k] = (X >= 1 && X <= P.nx && Y >= 1 && Y <= P.ny && Z >= 1 && Z <= P.nz)
+                       ? x[((size_t)(Z - 1) * P.ny + (Y - 1)) * P.nx + (X - 1)] : 0.f;
+        }
+        octs[2 * i] = make_float4(v[0], v[1], v[2], v[3]);
+        octs[2 * i + 1] = make_float4(v[4], v[5], v[6], v[7]);
     }
 }
 
@@ -699,6 +731,12 @@ void oat_launch_pad_quads(const OatDev &P, const float *x, float4 *quads, cudaSt
     oat_pad_quads_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, quads);
 }
 
+void oat_launch_pad_octs(const OatDev &P, const float *x, float4 *octs, cudaStream_t st)
+{
+    const long long n = 8LL * P.oz * P.qplane;
+    oat_pad_octs_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, octs);
+}
+
 void oat_launch_unquad(const OatDev &P, const float4 *quads, float *x, cudaStream_t st)
 {
     const long long n = (long long)P.nx * P.ny * P.nz;
@@ -755,7 +793,8 @@ cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float
                              double *g, unsigned long long *counter, cudaStream_t st)
 {
     if (P.n_patches <= 0) return cudaSuccess;
-    if (mode == 0) return variant == 2 ? launch_patch_t<0, 2>(P, xpad, xacc, y, g, counter, st)
+    if (mode == 0) return variant == 3 ? launch_patch_t<0, 3>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 2 ? launch_patch_t<0, 2>(P, xpad, xacc, y, g, counter, st)
                         : variant == 1 ? launch_patch_t<0, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_patch_t<0, 0>(P, xpad, xacc, y, g, counter, st);
     if (mode == 1) return variant == 3 ? launch_patch_t<1, 3>(P, xpad, xacc, y, g, counter, st)
@@ -806,7 +845,8 @@ cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *
                            double *g, unsigned long long *counter, cudaStream_t st)
 {
     if (P.n_items <= 0) return cudaSuccess;
-    if (mode == 0) return variant == 2 ? launch_ray_t<0, 2>(P, xpad, xacc, y, g, counter, st)
+    if (mode == 0) return variant == 3 ? launch_ray_t<0, 3>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 2 ? launch_ray_t<0, 2>(P, xpad, xacc, y, g, counter, st)
                         : variant == 1 ? launch_ray_t<0, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_ray_t<0, 0>(P, xpad, xacc, y, g, counter, st);
     if (mode == 1) return variant >= 2 ? launch_ray_t<1, 2>(P, xpad, xacc, y, g, counter, st)
