@@ -49,6 +49,7 @@ struct oat_geometry {
     int *d_qb_rings = nullptr;
     int *d_rb_sectors = nullptr;
     unsigned long long *d_patches = nullptr;  // schedule 1 work items (lazy)
+    int *d_q_count = nullptr, *d_q_done = nullptr;
     unsigned long long patch_cap = 0;
     int morton_shift = 4;                     // patches are sorted by the Morton code of (centre >> shift)
     int schedule = 1;                         // 0 = ring-major chunks, 1 = Morton-sorted patches
@@ -84,7 +85,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
-    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches);
+    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
     if (g->atlas) cudaFreeArray(g->atlas);
@@ -271,6 +272,7 @@ int build_geometry(oat_geometry *G)
     P.qb_rings = G->d_qb_rings; P.item_prefix = G->d_item_prefix;
     P.n_items = items;
     P.rb_sectors = G->d_rb_sectors; P.patches = nullptr; P.n_patches = 0;
+    P.q_count = nullptr; P.q_done = nullptr;
     P.tex = 0; P.atlas_shift = 0; P.atlas_mask = 0;
     P.qx = (d.nx + 2) / 2 + 1; P.qy = (d.ny + 2) / 2 + 1;
     P.qplane = (long long)P.qx * P.qy;
@@ -333,7 +335,14 @@ int ensure_patches(oat_geometry *G)
 {
     if (G->d_patches || G->patch_cap == 0) return OAT_OK;
     long long n = 0;
-    cudaError_t e = oat_build_patches(G->dev, G->patch_cap, G->morton_shift, &G->d_patches, &n);
+    const size_t nq = (size_t)(G->dev.Q > 0 ? G->dev.Q : 1);
+    if (!G->d_q_count) {
+        CUDA_TRY(cudaMalloc((void **)&G->d_q_count, sizeof(int) * nq));
+        CUDA_TRY(cudaMalloc((void **)&G->d_q_done, sizeof(int) * nq));
+    }
+    CUDA_TRY(cudaMemset(G->d_q_count, 0, sizeof(int) * nq));
+    G->dev.q_count = G->d_q_count; G->dev.q_done = G->d_q_done;
+    cudaError_t e = oat_build_patches(G->dev, G->patch_cap, G->morton_shift, G->d_q_count, &G->d_patches, &n);
     if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? OAT_ERR_ALLOC : OAT_ERR_CUDA, "patch list generation failed: %s", cudaGetErrorString(e));
     G->dev.patches = G->d_patches;
     G->dev.n_patches = n;
@@ -381,13 +390,19 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
         oat_launch_pad(P, d_x, G->d_xpad, st); ++G->last_launches;
     }
     CUDA_TRY(cudaMemsetAsync(G->d_g, 0, sizeof(double) * (G->n_dat ? G->n_dat : 1), st));
+    const bool fused = G->schedule == 1;                  // patch kernel applies 1/t and the time difference itself
+    if (fused) {
+        int rc = ensure_patches(G); if (rc) return rc;
+        if (G->n_dat > 0) CUDA_TRY(cudaMemsetAsync(d_y, 0, sizeof(float) * G->n_dat, st));   // rows without any sample
+        if (G->d_q_done) CUDA_TRY(cudaMemsetAsync(G->d_q_done, 0, sizeof(int) * (size_t)(P.Q > 0 ? P.Q : 1), st));
+    }
     CUDA_TRY(cudaEventRecord(G->ev0, st));
     bool launched;
-    { int rc = launch_traversal(G, 0, G->variant_project, src, nullptr, nullptr, G->d_g, nullptr, st, &launched); if (rc) return rc; }
+    { int rc = launch_traversal(G, 0, G->variant_project, src, fused ? d_y : nullptr, nullptr, G->d_g, nullptr, st, &launched); if (rc) return rc; }
     if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
-    if (G->n_dat > 0) { oat_launch_diff(P, G->d_g, d_y, st); ++G->last_launches; }
+    if (!fused && G->n_dat > 0) { oat_launch_diff(P, G->d_g, d_y, st); ++G->last_launches; }
     CUDA_TRY(cudaGetLastError());
     return OAT_OK;
 }

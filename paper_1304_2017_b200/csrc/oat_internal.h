@@ -57,6 +57,8 @@ struct OatDev {
     const int *rb_sectors;               // per (band, ring block): number of azimuth sectors S
     const unsigned long long *patches;   // schedule 1: Morton-sorted packed (q, band, ring block, sector)
     long long n_patches;
+    const int *q_count;                  // patches per transducer
+    int *q_done;                         // patches finished in the running projection (zeroed per call)
     int qx, qy;                // quad layout (variant 2): quads per row / rows per plane
     long long qplane;          // qx*qy; one parity array holds pz*qplane float4 quads
     int oz;                    // octet layout (project variant 3): bricks along z; 8 arrays of oz*qplane records of 32 B
@@ -78,7 +80,7 @@ cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *
                            double *g, unsigned long long *counter, cudaStream_t st);
 cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
                              double *g, unsigned long long *counter, cudaStream_t st);
-cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, unsigned long long **patches_out, long long *n_patches);
+cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, int *q_count, unsigned long long **patches_out, long long *n_patches);
 void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st);
 // vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)
 void oat_launch_dot(const float *a, const float *b, long long n, double *out, cudaStream_t st);

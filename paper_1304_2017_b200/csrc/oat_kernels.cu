@@ -449,6 +449,7 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
     __shared__ float s_red[OAT_NW][32];
     __shared__ float s_delta[32], s_coef[32];
     __shared__ int s_count;
+    __shared__ int s_last;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (long long item = blockIdx.x; item < P.n_patches; item += gridDim.x) {
@@ -486,8 +487,37 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
             else consume_list<MODE, ((MODE == 1 && VAR == 3) ? 2 : VAR)>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
         }
         item_epilogue<MODE>(P, q, L, acc, cnt, warp, lane, s_red, g, counter);
+        if (MODE == 0) {
+            // Fused step A4 (Eq. 3 L63 / Eq. 13): the block that completes the LAST patch of transducer q
+            // turns the finished fp64 row g[q,:] into pressure, y_k = kappa (g_{k+1}/t_{k+1} - g_{k-1}/t_{k-1})/(2 dt).
+            // Pattern: every lane fences its own atomics, then one lane counts the patch as done.
+            if (warp == 0) {
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) s_last = (atomicAdd(&P.q_done[q], 1) + 1 == P.q_count[q]) ? 1 : 0;
+            }
+            __syncthreads();
+            if (s_last) {
+                __threadfence();
+                const double *gq = g + (size_t)q * P.K;
+                float *yq = xacc + (size_t)q * P.K;          // MODE 0: xacc is the output data vector y
+                for (int k = tid; k < P.K; k += OAT_NT) {
+                    double sp = 0.0, sm = 0.0;
+                    if (k + 1 < P.K) { const double t = P.t0 + (double)(k + 1) * P.dt; if (t > 0.0) sp = __ldcg(gq + k + 1) / t; }
+                    if (k - 1 >= 0) { const double t = P.t0 + (double)(k - 1) * P.dt; if (t > 0.0) sm = __ldcg(gq + k - 1) / t; }
+                    yq[k] = (float)(P.kappa * (sp - sm) / (2.0 * P.dt));
+                }
+            }
+        }
         __syncthreads();
     }
+}
+
+// number of patches per transducer (for the fused time-difference epilogue)
+__global__ void oat_count_patches_kernel(const unsigned long long *__restrict__ patches, long long n, int *__restrict__ q_count)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        atomicAdd(&q_count[(int)(patches[i] >> 38)], 1);
 }
 
 // Patch generation (once per geometry): one block per (q, band); threads stride over (ring block,
@@ -807,7 +837,7 @@ cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float
 // Generates the patch list of a geometry on the device and sorts it by Morton key.  `cap` is the
 // host-computed upper bound on the number of patches.  On return *n_patches is the number generated;
 // *patches_out is a device buffer the caller owns.
-cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, unsigned long long **patches_out, long long *n_patches)
+cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, int *q_count, unsigned long long **patches_out, long long *n_patches)
 {
     *patches_out = nullptr; *n_patches = 0;
     if (cap == 0 || P.Q == 0) return cudaSuccess;
@@ -836,6 +866,10 @@ cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift
     OAT_TRY(cudaDeviceSynchronize());
 #undef OAT_TRY
     cleanup();
+    if (q_count) {
+        oat_count_patches_kernel<<<grid_for((long long)n, 256), 256>>>(vals2, (long long)n, q_count);
+        if ((e = cudaDeviceSynchronize()) != cudaSuccess) { cudaFree(vals2); return e; }
+    }
     *patches_out = vals2;
     *n_patches = (long long)n;
     return cudaSuccess;
