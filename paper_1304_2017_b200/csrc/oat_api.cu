@@ -60,6 +60,10 @@ struct oat_geometry {
     size_t n_quads = 0;
     float4 *d_octs = nullptr;                 // 8 parity-shifted octet arrays (project variant 3, lazy)
     size_t n_octs = 0;                        // in float4 units
+    float4 *d_faces = nullptr;                // face-quad accumulators of the 3 orientations (backproject variant 4, lazy)
+    size_t n_faces = 0;                       // float4 records, 0 = variant unavailable for this grid
+    float4 *d_cells = nullptr;                // per-cell polynomial records (project variant 4, lazy)
+    size_t n_cells = 0;                       // records incl. the trailing all-zero one (2 float4 each)
     double *d_g = nullptr;                    // Q*K SRT accumulator
     float *d_y2 = nullptr, *d_x2 = nullptr;   // adjoint check / CGLS / host entry points (lazy)
     float *d_x3 = nullptr, *d_y3 = nullptr, *d_x4 = nullptr;   // CGLS vectors (lazy)
@@ -67,7 +71,7 @@ struct oat_geometry {
     unsigned long long *d_counter = nullptr;
     double *h_scal = nullptr;                 // pinned mirror of d_scal
     long long n_surface_samples = -1;
-    int variant_project = 3, variant_backproject = 3;   // measured best
+    int variant_project = 4, variant_backproject = 4;   // measured best
     cudaArray_t atlas = nullptr;              // slice atlas for the texture-gather projection (lazy)
     cudaTextureObject_t tex = 0;
     cudaSurfaceObject_t surf = 0;
@@ -85,7 +89,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
-    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
+    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
     if (g->atlas) cudaFreeArray(g->atlas);
@@ -277,6 +281,23 @@ int build_geometry(oat_geometry *G)
     P.qx = (d.nx + 2) / 2 + 1; P.qy = (d.ny + 2) / 2 + 1;
     P.qplane = (long long)P.qx * P.qy;
     P.oz = (d.nz + 2) / 2 + 1;
+    P.cx = ((d.nx + 1 + 3) / 4) * 4; P.cy = d.ny + 1;      // 4 records = one 128-byte line
+    P.cxy = (long long)P.cx * P.cy;
+    if ((unsigned long long)(d.nz + 1) * (unsigned long long)P.cxy + 1 >= (1ULL << 31)) P.cx = 0;   // variant 4 unavailable
+    else P.zero_cell = (unsigned)((long long)(d.nz + 1) * P.cxy);
+    {   // face-quad accumulators: orientation a = x, y, z with in-plane axes (b, c) = (y,z), (z,x), (x,y)
+        const long long nn[3] = {d.nx, d.ny, d.nz};
+        long long tot = 0;
+        bool ok = true;
+        for (int o = 0; o < 3; ++o) {
+            const long long na = nn[o] + 2, nb = nn[(o + 1) % 3] + 1, nc = nn[(o + 2) % 3] + 1;
+            if (na * nb * nc >= (1LL << 31)) ok = false;
+            P.f_base[o] = tot; P.f_nb[o] = (int)nb; P.f_nc[o] = (int)nc;
+            tot += na * nb * nc;
+        }
+        G->n_faces = ok ? (size_t)tot : 0;
+    }
+    G->n_cells = P.cx ? (size_t)(d.nz + 1) * (size_t)P.cxy + 1 : 0;
 
     G->n_vox = (size_t)d.nx * d.ny * d.nz;
     G->n_dat = (size_t)Q * K;
@@ -375,15 +396,21 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     const OatDev &P = G->dev;
     G->last_launches = 0;
     const float *src = G->d_xpad;
-    if (G->variant_project == 3) {
+    int variant = G->variant_project;
+    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_cells)) variant = 3;   // marching form needs B = 32 patches
+    if (variant == 4) {
+        if (!G->d_cells) CUDA_TRY(cudaMalloc((void **)&G->d_cells, sizeof(float4) * 2 * G->n_cells));
+        oat_launch_pad_cells(P, d_x, G->d_cells, st); ++G->last_launches;
+        src = reinterpret_cast<const float *>(G->d_cells);
+    } else if (variant == 3) {
         if (!G->d_octs) CUDA_TRY(cudaMalloc((void **)&G->d_octs, sizeof(float4) * G->n_octs));
         oat_launch_pad_octs(P, d_x, G->d_octs, st); ++G->last_launches;
         src = reinterpret_cast<const float *>(G->d_octs);
-    } else if (G->variant_project == 2) {
+    } else if (variant == 2) {
         int rc = ensure_quads(G); if (rc) return rc;
         oat_launch_pad_quads(P, d_x, G->d_quads, st); ++G->last_launches;
         src = reinterpret_cast<const float *>(G->d_quads);
-    } else if (G->variant_project == 1) {
+    } else if (variant == 1) {
         int rc = ensure_atlas(G); if (rc) return rc;
         oat_launch_pad_atlas(P, d_x, G->surf, st); ++G->last_launches;
     } else {
@@ -398,7 +425,7 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     }
     CUDA_TRY(cudaEventRecord(G->ev0, st));
     bool launched;
-    { int rc = launch_traversal(G, 0, G->variant_project, src, fused ? d_y : nullptr, nullptr, G->d_g, nullptr, st, &launched); if (rc) return rc; }
+    { int rc = launch_traversal(G, 0, variant, src, fused ? d_y : nullptr, nullptr, G->d_g, nullptr, st, &launched); if (rc) return rc; }
     if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
@@ -411,9 +438,16 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    const bool quads = G->variant_backproject >= 2;
+    int variant = G->variant_backproject;
+    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_faces)) variant = 3;   // marching form needs B = 32 patches
+    const bool faces = variant == 4;
+    const bool quads = !faces && variant >= 2;
     float *acc = G->d_xpad;
-    if (quads) {
+    if (faces) {
+        if (!G->d_faces) CUDA_TRY(cudaMalloc((void **)&G->d_faces, sizeof(float4) * G->n_faces));
+        acc = reinterpret_cast<float *>(G->d_faces);
+        CUDA_TRY(cudaMemsetAsync(G->d_faces, 0, sizeof(float4) * G->n_faces, st));
+    } else if (quads) {
         int rc = ensure_quads(G); if (rc) return rc;
         acc = reinterpret_cast<float *>(G->d_quads);
         CUDA_TRY(cudaMemsetAsync(G->d_quads, 0, sizeof(float4) * G->n_quads, st));
@@ -422,11 +456,12 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
     }
     CUDA_TRY(cudaEventRecord(G->ev0, st));
     bool launched;
-    { int rc = launch_traversal(G, 1, G->variant_backproject, nullptr, acc, d_y, nullptr, nullptr, st, &launched); if (rc) return rc; }
+    { int rc = launch_traversal(G, 1, variant, nullptr, acc, d_y, nullptr, nullptr, st, &launched); if (rc) return rc; }
     if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
-    if (quads) oat_launch_unquad(P, G->d_quads, d_x, st);
+    if (faces) oat_launch_unface(P, G->d_faces, d_x, st);
+    else if (quads) oat_launch_unquad(P, G->d_quads, d_x, st);
     else oat_launch_unpad(P, G->d_xpad, d_x, st);
     ++G->last_launches;
     CUDA_TRY(cudaGetLastError());
@@ -630,8 +665,8 @@ int oat_cgls(oat_geometry *g, const float *d_y, float *d_x, int n_iter, double *
 int oat_set_variant(oat_geometry *g, const char *key, int variant)
 {
     if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");
-    if (!strcmp(key, "project")) { if (variant < 0 || variant > 3) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
-    if (!strcmp(key, "backproject")) { if (variant < 0 || variant > 3) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
+    if (!strcmp(key, "project")) { if (variant < 0 || variant > 4) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
+    if (!strcmp(key, "backproject")) { if (variant < 0 || variant > 4) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
     if (!strcmp(key, "morton_shift")) {
         if (variant < 0 || variant > 10) return fail(OAT_ERR_INVALID, "morton_shift out of range");
         if (g->morton_shift != variant) { cudaFree(g->d_patches); g->d_patches = nullptr; g->dev.patches = nullptr; g->dev.n_patches = 0; }

@@ -62,6 +62,14 @@ struct OatDev {
     int qx, qy;                // quad layout (variant 2): quads per row / rows per plane
     long long qplane;          // qx*qy; one parity array holds pz*qplane float4 quads
     int oz;                    // octet layout (project variant 3): bricks along z; 8 arrays of oz*qplane records of 32 B
+    int cx, cy;                // cell-record layout (variant 4): cells per row (pitch, multiple of 4) / rows per plane
+    long long cxy;             // cx*cy; record of padded cell (ix,iy,iz) = (iz*cy + iy)*cx + ix, 32 B each
+    unsigned zero_cell;        // index of an all-zero record (samples outside the padded box read / add into it)
+    // face-quad accumulators (backproject variant 4): orientation o = axis a normal to the quad, in-plane axes
+    // (b, c) = (y,z), (z,x), (x,y) for a = x, y, z; record (ia, ib, ic) = float4 of padded nodes
+    // {(ib,ic),(ib+1,ic),(ib,ic+1),(ib+1,ic+1)} on plane ia, at f_base[o] + (ia*f_nc[o] + ic)*f_nb[o] + ib
+    long long f_base[3];
+    int f_nb[3], f_nc[3];
     cudaTextureObject_t tex;   // slice atlas of the padded volume (project variant 1), 0 if unused
     int atlas_shift, atlas_mask;   // slice z sits at column (z & mask), row (z >> shift) of the atlas
 };
@@ -74,6 +82,11 @@ void oat_launch_unpad(const OatDev &P, const float *xpad, float *x, cudaStream_t
 // x0 = 2a + (p&1), y0 = 2b + (p>>1): the four in-plane corners of ANY cell are one aligned float4
 void oat_launch_pad_quads(const OatDev &P, const float *x, float4 *quads, cudaStream_t st);
 void oat_launch_pad_octs(const OatDev &P, const float *x, float4 *octs, cudaStream_t st);
+// cell records (variant 4): per padded cell the 8 coefficients of its trilinear polynomial
+// c0 + cx fx + cy fy + cxy fx fy + fz (cz + cxz fx + cyz fy + cxyz fx fy), fp64-computed, one 32-byte sector
+void oat_launch_pad_cells(const OatDev &P, const float *x, float4 *cells, cudaStream_t st);
+// x[n] = sum of the 12 face-quad components that are node n (backproject variant 4)
+void oat_launch_unface(const OatDev &P, const float4 *faces, float *x, cudaStream_t st);
 void oat_launch_unquad(const OatDev &P, const float4 *quads, float *x, cudaStream_t st);
 void oat_launch_pad_atlas(const OatDev &P, const float *x, cudaSurfaceObject_t surf, cudaStream_t st);
 cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,

@@ -289,8 +289,12 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
             const unsigned cell = in ? quad_index(P, s.ix, s.iy, s.iz) : 0xffffffffu;
             if (cell != cur) {
                 if (cur != 0xffffffffu) {
+#if OAT_HALF_RED
+                    red_add_v4(quads + cur, a0 + a4, a1 + a5, a2 + a6, a3 + a7);
+#else
                     red_add_v4(quads + cur, a0, a1, a2, a3);
                     red_add_v4(quads + cur + P.qplane, a4, a5, a6, a7);
+#endif
                 }
                 a0 = a1 = a2 = a3 = a4 = a5 = a6 = a7 = 0.f;
                 cur = cell;
@@ -309,6 +313,243 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
             red_add_v4(quads + cur + P.qplane, a4, a5, a6, a7);
         }
     }
+}
+
+// CONSUME for H, "marching" form (project variant 4, B = 32): one THREAD per ray, stepping through the
+// band's 32 time samples in order, OAT_MU rays interleaved per thread (independent load chains).
+//   position   t_k = fma(u*step, k - 15.5, anchor)   (same fp64 anchor as every other variant; the
+//              immediate-operand FMA keeps one rounding at |t| < ~6 voxels)
+//   cell       floor by the round-down magic add; the cell's 32-byte record (8 polynomial coefficients of
+//              the trilinear interpolant, see oat_pad_cells_kernel) is (re)loaded with a PREDICATED 256-bit
+//              load only when the ray has entered a new cell -- ~2-3 samples share one load, and the L1
+//              data stage sees ~0.4 sectors per sample instead of 8 scalar gathers
+//   value      7 FMAs (Horner in fx, fy, fz) instead of 7 lerps = 14 ops
+// acc[k] holds the thread's sum over its rays for sample k; the caller transposes/reduces over the warp.
+#ifndef OAT_MU
+#define OAT_MU 1
+#endif
+#ifndef OAT_ALWAYS_LOAD
+#define OAT_ALWAYS_LOAD 0
+#endif
+#ifndef OAT_HALF_RED
+#define OAT_HALF_RED 0   // experiment only: wrong results, half the reductions
+#endif
+#ifndef OAT_PREFETCH
+#define OAT_PREFETCH 0
+#endif
+#ifndef OAT_DBUF
+#define OAT_DBUF 0
+#endif
+#ifndef OAT_MB
+#define OAT_MB 4      // resident blocks per SM the marching variants are compiled for (measured best: 64 registers)
+#endif
+
+__device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
+        "@p ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]), "+f"(c[4]), "+f"(c[5]), "+f"(c[6]), "+f"(c[7])
+        : "l"(p), "r"((int)pred));
+}
+
+// predicated 256-bit load into fresh registers (contents undefined where pred is false)
+__device__ __forceinline__ void ldg256_to(float (&c)[8], const float4 *p, bool pred)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
+        "@p ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
+        : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3]), "=f"(c[4]), "=f"(c[5]), "=f"(c[6]), "=f"(c[7])
+        : "l"(p), "r"((int)pred));
+}
+
+__device__ __forceinline__ void prefetch_l1_if(const float4 *p, bool pred)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %1, 0;\n\t@p prefetch.global.L1 [%0];\n\t}" ::"l"(p), "r"((int)pred));
+}
+
+// one step of one ray: cell record index, "entered a new cell" flag and the in-cell fractions
+struct MarchStep {
+    unsigned idx;
+    bool ch;
+    float fx, fy, fz;
+};
+
+__device__ __forceinline__ void consume_march_fwd(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid,
+                                                  const float4 *__restrict__ cells, float (&acc)[32])
+{
+    const float stepf = (float)P.step;
+    for (int e0 = tid * OAT_MU; e0 < n_list; e0 += OAT_NT * OAT_MU) {   // thread t: rays t*MU .. t*MU+MU-1, so idle warps skip
+        float ax[OAT_MU], ay[OAT_MU], az[OAT_MU], om[OAT_MU], sx[OAT_MU], sy[OAT_MU], sz[OAT_MU];
+        int bx[OAT_MU], by[OAT_MU], bz[OAT_MU];
+        float prx[OAT_MU], pry[OAT_MU], prz[OAT_MU];      // previous step's rounded coordinates (cell identity)
+        float c[OAT_MU][8];
+        MarchStep nxt[OAT_MU];
+        auto step_of = [&](int u, int k) {
+            const float kk = (float)k - 15.5f;
+            const float tx = fmaf(sx[u], kk, ax[u]), ty = fmaf(sy[u], kk, ay[u]), tz = fmaf(sz[u], kk, az[u]);
+            const float rx = __fadd_rd(tx, OAT_MAGIC), ry = __fadd_rd(ty, OAT_MAGIC), rz = __fadd_rd(tz, OAT_MAGIC);
+            MarchStep m;
+            m.ch = (rx != prx[u]) | (ry != pry[u]) | (rz != prz[u]);
+            prx[u] = rx; pry[u] = ry; prz[u] = rz;
+            const int ix = __float_as_int(rx) + bx[u], iy = __float_as_int(ry) + by[u], iz = __float_as_int(rz) + bz[u];
+            const bool in = ((unsigned)ix <= (unsigned)P.nx) & ((unsigned)iy <= (unsigned)P.ny) & ((unsigned)iz <= (unsigned)P.nz);
+            m.idx = in ? (unsigned)((iz * P.cy + iy) * P.cx + ix) : P.zero_cell;
+            m.fx = tx - (rx - OAT_MAGIC); m.fy = ty - (ry - OAT_MAGIC); m.fz = tz - (rz - OAT_MAGIC);
+            return m;
+        };
+#pragma unroll
+        for (int u = 0; u < OAT_MU; ++u) {
+            const int ei = e0 + u;
+            const bool valid = ei < n_list;
+            const Entry e = list[valid ? ei : e0];
+            ax[u] = e.a.x; ay[u] = e.a.y; az[u] = e.a.z; om[u] = valid ? e.a.w : 0.f;
+            sx[u] = e.u.x * stepf; sy[u] = e.u.y * stepf; sz[u] = e.u.z * stepf;
+            bx[u] = e.i.x; by[u] = e.i.y; bz[u] = e.i.z;
+            prx[u] = pry[u] = prz[u] = 0.f;               // never equals a rounded coordinate (those are >= 2^22)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) c[u][i] = 0.f;
+            nxt[u] = step_of(u, 0);
+#if OAT_DBUF
+            ldg256_if(c[u], cells + 2 * (size_t)nxt[u].idx, true);
+#elif OAT_PREFETCH
+            prefetch_l1_if(cells + 2 * (size_t)nxt[u].idx, true);
+#endif
+        }
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+#pragma unroll
+            for (int u = 0; u < OAT_MU; ++u) {
+                const MarchStep cur = nxt[u];
+                if (k + 1 < 32) {                          // next step's cell: start its L2 -> L1 fetch now
+                    nxt[u] = step_of(u, k + 1);
+#if OAT_PREFETCH
+                    prefetch_l1_if(cells + 2 * (size_t)nxt[u].idx, nxt[u].ch);
+#endif
+                }
+#if OAT_DBUF
+                float Ln[8];                               // next step's record: in flight while this step is evaluated
+                if (k + 1 < 32) ldg256_to(Ln, cells + 2 * (size_t)nxt[u].idx, nxt[u].ch);
+#elif OAT_ALWAYS_LOAD
+                ldg256_if(c[u], cells + 2 * (size_t)cur.idx, true);
+#else
+                ldg256_if(c[u], cells + 2 * (size_t)cur.idx, cur.ch);
+#endif
+                const float lo = fmaf(cur.fy, fmaf(cur.fx, c[u][3], c[u][2]), fmaf(cur.fx, c[u][1], c[u][0]));
+                const float hi = fmaf(cur.fy, fmaf(cur.fx, c[u][7], c[u][6]), fmaf(cur.fx, c[u][5], c[u][4]));
+                acc[k] = fmaf(om[u], fmaf(cur.fz, hi, lo), acc[k]);
+#if OAT_DBUF
+                if (k + 1 < 32) {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) c[u][i] = nxt[u].ch ? Ln[i] : c[u][i];
+                }
+#endif
+            }
+        }
+    }
+}
+
+// CONSUME for H^T, face-carrying marching form (backproject variant 4, B = 32).  H^T is bound by the rate at
+// which an SM can retire vector reductions (~1.5 SM-cycles per RED.128 lane on scattered sectors, measured), so
+// the aim is FEWER reductions per sample, not fewer instructions:
+//   * one THREAD per ray, local axis 0 = the ray's dominant axis a (|u_a| largest), marched in the direction in
+//     which the ray ADVANCES along a (the 32 samples are walked backwards when u_a < 0; positions are identical
+//     because fma(-s, -kk, anchor) == fma(s, kk, anchor));
+//   * the 8 corner weights of the current cell are accumulated as two quads, L on plane i_a and H on plane
+//     i_a + 1, laid out as the face-quad records of orientation a (OatDev::f_base);
+//   * when the ray steps to the next cell along a only, the finished quad L is retired with ONE reduction and H
+//     is carried over as the new L; only a step across one of the two minor axes flushes both quads.
+// About 0.65 reductions per sample instead of 0.9 for the z-only quads of variant 3.  Same positions, cells and
+// weights as consume_march_fwd, so H and H^T visit identical samples (Eq. 12 vs Eq. 23).
+#ifndef OAT_MBT
+#define OAT_MBT 3     // resident blocks per SM for the marching H^T kernel
+#endif
+#ifndef OAT_HT_ORIENT
+#define OAT_HT_ORIENT 3      // 3: dominant-axis orientations; 1: always the z orientation (experiment)
+#endif
+
+__device__ __forceinline__ void red_add_v4_if(float4 *addr, float a, float b, float c, float d, bool pred)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t@p red.global.add.v4.f32 [%0], {%1,%2,%3,%4};\n\t}"
+                 ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d), "r"((int)pred) : "memory");
+}
+
+__device__ __forceinline__ void consume_march_bwd(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid,
+                                                  const float *__restrict__ s_coef, float4 *__restrict__ faces)
+{
+    const float stepf = (float)P.step;
+    for (int ei = tid; ei < n_list; ei += OAT_NT) {
+        const Entry e = list[ei];
+        const float mx = fabsf(e.u.x), my = fabsf(e.u.y), mz = fabsf(e.u.z);
+        int o = (mx >= my && mx >= mz) ? 0 : (my >= mz ? 1 : 2);
+        if (OAT_HT_ORIENT == 1) o = 2;
+        // local axes (0, 1, 2) = (a, b, c) = (x,y,z), (y,z,x), (z,x,y)
+        const float a0 = o == 0 ? e.a.x : o == 1 ? e.a.y : e.a.z, a1 = o == 0 ? e.a.y : o == 1 ? e.a.z : e.a.x,
+                    a2 = o == 0 ? e.a.z : o == 1 ? e.a.x : e.a.y;
+        const float u0 = o == 0 ? e.u.x : o == 1 ? e.u.y : e.u.z, u1 = o == 0 ? e.u.y : o == 1 ? e.u.z : e.u.x,
+                    u2 = o == 0 ? e.u.z : o == 1 ? e.u.x : e.u.y;
+        const int b0 = o == 0 ? e.i.x : o == 1 ? e.i.y : e.i.z, b1 = o == 0 ? e.i.y : o == 1 ? e.i.z : e.i.x,
+                  b2 = o == 0 ? e.i.z : o == 1 ? e.i.x : e.i.y;
+        const unsigned n0 = o == 0 ? P.nx : o == 1 ? P.ny : P.nz, n1 = o == 0 ? P.ny : o == 1 ? P.nz : P.nx,
+                       n2 = o == 0 ? P.nz : o == 1 ? P.nx : P.ny;
+        const int nb = o == 0 ? P.f_nb[0] : o == 1 ? P.f_nb[1] : P.f_nb[2];
+        const int nc = o == 0 ? P.f_nc[0] : o == 1 ? P.f_nc[1] : P.f_nc[2];
+        float4 *const qb = faces + (o == 0 ? P.f_base[0] : o == 1 ? P.f_base[1] : P.f_base[2]);
+        const int sa = nb * nc;                            // records per plane
+        const bool flip = u0 < 0.f;
+        const float sg = flip ? -stepf : stepf;
+        const float s0 = u0 * sg, s1 = u1 * sg, s2 = u2 * sg;   // s0 >= 0: the ray advances along local axis 0
+        const float *cp = s_coef + (flip ? 31 : 0);
+        const int cs = flip ? -1 : 1;
+        const float om = e.a.w;
+        float L0 = 0.f, L1 = 0.f, L2 = 0.f, L3 = 0.f, H0 = 0.f, H1 = 0.f, H2 = 0.f, H3 = 0.f;
+        float pr0 = 0.f, pr1 = 0.f, pr2 = 0.f;             // never equal to a rounded coordinate (those are >= 2^22)
+        float4 *cur = qb;
+        bool valid = false;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            const float kk = (float)k - 15.5f;
+            const float t0 = fmaf(s0, kk, a0), t1 = fmaf(s1, kk, a1), t2 = fmaf(s2, kk, a2);
+            const float r0 = __fadd_rd(t0, OAT_MAGIC), r1 = __fadd_rd(t1, OAT_MAGIC), r2 = __fadd_rd(t2, OAT_MAGIC);
+            const bool c12 = (r1 != pr1) | (r2 != pr2);
+            const bool c0 = r0 != pr0;
+            const bool carry = (!c12) & (r0 == pr0 + 1.0f);    // one cell forward along the dominant axis only
+            const bool full = c12 | (c0 & !carry);
+            red_add_v4_if(cur, L0, L1, L2, L3, valid & (c0 | c12));
+            red_add_v4_if(cur + sa, H0, H1, H2, H3, valid & full);
+            L0 = full ? 0.f : (carry ? H0 : L0); L1 = full ? 0.f : (carry ? H1 : L1);
+            L2 = full ? 0.f : (carry ? H2 : L2); L3 = full ? 0.f : (carry ? H3 : L3);
+            const bool zh = full | carry;
+            H0 = zh ? 0.f : H0; H1 = zh ? 0.f : H1; H2 = zh ? 0.f : H2; H3 = zh ? 0.f : H3;
+            pr0 = r0; pr1 = r1; pr2 = r2;
+            const int i0 = __float_as_int(r0) + b0, i1 = __float_as_int(r1) + b1, i2 = __float_as_int(r2) + b2;
+            valid = ((unsigned)i0 <= n0) & ((unsigned)i1 <= n1) & ((unsigned)i2 <= n2);
+            cur = qb + ((i0 * nc + i2) * nb + i1);
+            const float f0 = t0 - (r0 - OAT_MAGIC), f1 = t1 - (r1 - OAT_MAGIC), f2 = t2 - (r2 - OAT_MAGIC);
+            const float cw = valid ? cp[cs * k] * om : 0.f;
+            const float e1 = 1.f - f1, e2 = 1.f - f2;
+            const float q0 = e1 * e2, q1 = f1 * e2, q2 = e1 * f2, q3 = f1 * f2;
+            const float wh = cw * f0, wl = cw - wh;
+            L0 = fmaf(q0, wl, L0); L1 = fmaf(q1, wl, L1); L2 = fmaf(q2, wl, L2); L3 = fmaf(q3, wl, L3);
+            H0 = fmaf(q0, wh, H0); H1 = fmaf(q1, wh, H1); H2 = fmaf(q2, wh, H2); H3 = fmaf(q3, wh, H3);
+        }
+        red_add_v4_if(cur, L0, L1, L2, L3, valid);
+        red_add_v4_if(cur + sa, H0, H1, H2, H3, valid);
+    }
+}
+
+// sum acc[k] over the 32 lanes of the warp; lane l returns the total of sample k = l (31 shuffles)
+__device__ __forceinline__ float warp_transpose_sum(float (&acc)[32], int lane)
+{
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        const bool up = (lane & s) != 0;
+#pragma unroll
+        for (int i = 0; i < s; ++i) {
+            const float send = up ? acc[i] : acc[i + s];
+            const float keep = up ? acc[i + s] : acc[i];
+            acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, s);
+        }
+    }
+    return acc[0];
 }
 
 // EPILOGUE of one work item: cross-warp combine in fp64 and one fp64 atomic per time sample (S5)
@@ -439,7 +680,7 @@ __device__ __forceinline__ void unpack_item(unsigned long long v, int &q, int &b
 }
 
 template <int MODE, int VAR>
-__global__ void __launch_bounds__(OAT_NT, 3)
+__global__ void __launch_bounds__(OAT_NT, (VAR == 4 ? (MODE == 1 ? OAT_MBT : OAT_MB) : 3))
 oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict__ xacc,
                  const float *__restrict__ y, double *__restrict__ g, unsigned long long *__restrict__ counter)
 {
@@ -463,7 +704,7 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
         const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
         const int S = P.rb_sectors[band.rb_ofs + rb];
         const LaneCtx L = lane_setup<MODE>(P, band, q, lane, y);
-        if (MODE == 1 && VAR == 3 && warp == 0) { s_delta[lane] = L.delta; s_coef[lane] = L.active ? L.coef : 0.f; }
+        if (MODE == 1 && VAR >= 3 && warp == 0) { s_delta[lane] = L.delta; s_coef[lane] = L.active ? L.coef : 0.f; }
         float acc = 0.f;
         unsigned cnt = 0;
         __syncthreads();
@@ -483,8 +724,15 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
             }
             __syncthreads();
             // ---------------------------------------------------------------- consume
-            if (MODE == 1 && VAR == 3) consume_march(P, list, s_count, tid, band.nk, s_delta, s_coef, xacc);
-            else consume_list<MODE, ((MODE == 1 && VAR == 3) ? 2 : VAR)>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
+            if (MODE == 0 && VAR == 4) {
+                float a32[32];
+#pragma unroll
+                for (int i = 0; i < 32; ++i) a32[i] = 0.f;
+                consume_march_fwd(P, list, s_count, tid, reinterpret_cast<const float4 *>(xpad), a32);
+                acc = warp_transpose_sum(a32, lane);
+            } else if (MODE == 1 && VAR == 4) consume_march_bwd(P, list, s_count, tid, s_coef, reinterpret_cast<float4 *>(xacc));
+            else if (MODE == 1 && VAR == 3) consume_march(P, list, s_count, tid, band.nk, s_delta, s_coef, xacc);
+            else consume_list<MODE, ((MODE == 1 && VAR == 3) ? 2 : (VAR == 4 ? 3 : VAR))>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
         }
         item_epilogue<MODE>(P, q, L, acc, cnt, warp, lane, s_red, g, counter);
         if (MODE == 0) {
@@ -649,6 +897,34 @@ __global__ void oat_pad_octs_kernel(const OatDev P, const float *__restrict__ x,
     }
 }
 
+// cell records from x (variant 4): record of padded cell (X,Y,Z), X in [0,nx] etc. (corner nodes X-1..X in real
+// indices, zero outside the grid = reading G5), holds the coefficients of the cell's trilinear polynomial
+//   A(fx,fy,fz) = c0 + c1 fx + c2 fy + c3 fx fy + fz (c4 + c5 fx + c6 fy + c7 fx fy)        (Eq. 10 L110 expanded)
+// computed in fp64 from the 8 corner values and rounded once to fp32.
+__global__ void oat_pad_cells_kernel(const OatDev P, const float *__restrict__ x, float4 *__restrict__ cells)
+{
+    const long long n = (long long)(P.nz + 1) * P.cxy;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i <= n; i += (long long)gridDim.x * blockDim.x) {
+        double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        if (i < n) {
+            const int X = (int)(i % P.cx);
+            const long long r = i / P.cx;
+            const int Y = (int)(r % P.cy), Z = (int)(r / P.cy);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const int xx = X - 1 + (k & 1), yy = Y - 1 + ((k >> 1) & 1), zz = Z - 1 + (k >> 2);
+                if (xx >= 0 && xx < P.nx && yy >= 0 && yy < P.ny && zz >= 0 && zz < P.nz)
+                    v[k] = (double)x[((size_t)zz * P.ny + yy) * P.nx + xx];
+            }
+        }                                                  // i == n: the all-zero record (P.zero_cell)
+        const double c1 = v[1] - v[0], c2 = v[2] - v[0], c4 = v[4] - v[0];
+        const double c3 = v[3] - v[2] - c1, c5 = v[5] - v[4] - c1, c6 = v[6] - v[4] - c2;
+        const double c7 = v[7] - v[6] - (v[5] - v[4]) - c3;
+        cells[2 * i] = make_float4((float)v[0], (float)c1, (float)c2, (float)c3);
+        cells[2 * i + 1] = make_float4((float)c4, (float)c5, (float)c6, (float)c7);
+    }
+}
+
 // x[n] = sum over the 4 parity arrays of the quad component that is node n (every node is in exactly
 // one quad of each array)
 __global__ void oat_unquad_kernel(const OatDev P, const float4 *__restrict__ quads, float *__restrict__ x)
@@ -666,6 +942,29 @@ __global__ void oat_unquad_kernel(const OatDev P, const float4 *__restrict__ qua
             const int c = (X - px - 2 * a) + 2 * (Y - py - 2 * b);
             const float4 q = quads[((size_t)(par * P.pz + Z) * P.qy + b) * P.qx + a];
             sum += c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w;
+        }
+        x[i] = sum;
+    }
+}
+
+// x[n] = sum over the three orientations of the 4 face-quad components that are node n (backproject variant 4):
+// every node sits in the quads (ib, ic) in {pb-1, pb} x {pc-1, pc} of plane pa, as component (pb-ib) + 2 (pc-ic)
+__global__ void oat_unface_kernel(const OatDev P, const float4 *__restrict__ faces, float *__restrict__ x)
+{
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int p[3] = {(int)(i % P.nx) + 1, (int)((i / P.nx) % P.ny) + 1, (int)(i / ((long long)P.nx * P.ny)) + 1};
+        float sum = 0.f;
+#pragma unroll
+        for (int o = 0; o < 3; ++o) {
+            const int pa = p[o], pb = p[(o + 1) % 3], pc = p[(o + 2) % 3];
+            const float4 *q = faces + P.f_base[o];
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                const int ib = pb - (d & 1), ic = pc - (d >> 1);
+                const float4 v = q[((long long)pa * P.f_nc[o] + ic) * P.f_nb[o] + ib];
+                sum += d == 0 ? v.x : d == 1 ? v.y : d == 2 ? v.z : v.w;
+            }
         }
         x[i] = sum;
     }
@@ -767,6 +1066,18 @@ void oat_launch_pad_octs(const OatDev &P, const float *x, float4 *octs, cudaStre
     oat_pad_octs_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, octs);
 }
 
+void oat_launch_pad_cells(const OatDev &P, const float *x, float4 *cells, cudaStream_t st)
+{
+    const long long n = (long long)(P.nz + 1) * P.cxy + 1;
+    oat_pad_cells_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, cells);
+}
+
+void oat_launch_unface(const OatDev &P, const float4 *faces, float *x, cudaStream_t st)
+{
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    oat_unface_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, faces, x);
+}
+
 void oat_launch_unquad(const OatDev &P, const float4 *quads, float *x, cudaStream_t st)
 {
     const long long n = (long long)P.nx * P.ny * P.nz;
@@ -823,11 +1134,13 @@ cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float
                              double *g, unsigned long long *counter, cudaStream_t st)
 {
     if (P.n_patches <= 0) return cudaSuccess;
-    if (mode == 0) return variant == 3 ? launch_patch_t<0, 3>(P, xpad, xacc, y, g, counter, st)
+    if (mode == 0) return variant == 4 ? launch_patch_t<0, 4>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 3 ? launch_patch_t<0, 3>(P, xpad, xacc, y, g, counter, st)
                         : variant == 2 ? launch_patch_t<0, 2>(P, xpad, xacc, y, g, counter, st)
                         : variant == 1 ? launch_patch_t<0, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_patch_t<0, 0>(P, xpad, xacc, y, g, counter, st);
-    if (mode == 1) return variant == 3 ? launch_patch_t<1, 3>(P, xpad, xacc, y, g, counter, st)
+    if (mode == 1) return variant == 4 ? launch_patch_t<1, 4>(P, xpad, xacc, y, g, counter, st)
+                        : variant == 3 ? launch_patch_t<1, 3>(P, xpad, xacc, y, g, counter, st)
                         : variant == 2 ? launch_patch_t<1, 2>(P, xpad, xacc, y, g, counter, st)
                         : variant == 1 ? launch_patch_t<1, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_patch_t<1, 0>(P, xpad, xacc, y, g, counter, st);

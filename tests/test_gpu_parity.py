@@ -250,8 +250,8 @@ def test_config4_cgls_first_iterations(env):
 
 # ------------------------------------------------------------------ kernel variants
 @pytest.mark.parametrize("schedule", [0, 1])
-@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 1), ("project", 2), ("project", 3),
-                                         ("backproject", 0), ("backproject", 1), ("backproject", 2), ("backproject", 3)])
+@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 1), ("project", 2), ("project", 3), ("project", 4),
+                                         ("backproject", 0), ("backproject", 1), ("backproject", 2), ("backproject", 3), ("backproject", 4)])
 def test_every_kernel_variant_matches_the_oracle(env, key, variant, schedule):
     """each selectable kernel variant / work schedule computes the same operator."""
     torch, orc, oat, wl = env
