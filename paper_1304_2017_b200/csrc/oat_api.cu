@@ -60,6 +60,8 @@ struct oat_geometry {
     size_t n_quads = 0;
     float4 *d_octs = nullptr;                 // 8 parity-shifted octet arrays (project variant 3, lazy)
     size_t n_octs = 0;                        // in float4 units
+    double2 *d_dir = nullptr;                 // direction table of the marching kernels (variant 4)
+    float *d_coef = nullptr;                  // Q*K adjoint coefficients g'_k rho_k^2 (backproject variant 4, lazy)
     float4 *d_faces = nullptr;                // face-quad accumulators of the 3 orientations (backproject variant 4, lazy)
     size_t n_faces = 0;                       // float4 records, 0 = variant unavailable for this grid
     float4 *d_cells = nullptr;                // per-cell polynomial records (project variant 4, lazy)
@@ -89,7 +91,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
-    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
+    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
     if (g->atlas) cudaFreeArray(g->atlas);
@@ -199,7 +201,7 @@ int build_geometry(oat_geometry *G)
     for (int b = 0; b < NB; ++b) {
         OatBand &bd = bands[b];
         bd.rb_ofs = (int)rb_sectors.size();
-        bd.pad = 0;
+        bd.dir_rings = 0; bd.dir_ofs = 0;
         const int n_rb = (bd.n_rings + OAT_RI - 1) / OAT_RI;
         rb_prefix[b].assign(n_rb + 1, 0);
         for (int rb = 0; rb < n_rb; ++rb) {
@@ -254,6 +256,15 @@ int build_geometry(oat_geometry *G)
         }
     }
     prefix[(size_t)Q * NB] = items;
+    // direction table of the marching kernels: per band the leading rings any transducer can use
+    long long n_dir = 0;
+    for (int b = 0; b < NB; ++b) {
+        int mr = 0;
+        for (int q = 0; q < Q; ++q) if (qb_rings[(size_t)q * NB + b] > mr) mr = qb_rings[(size_t)q * NB + b];
+        bands[b].dir_rings = mr;
+        bands[b].dir_ofs = n_dir;
+        n_dir += rings[bands[b].ring_ofs + mr].cum;
+    }
 
     // ---- upload
     int rc;
@@ -277,6 +288,11 @@ int build_geometry(oat_geometry *G)
     P.n_items = items;
     P.rb_sectors = G->d_rb_sectors; P.patches = nullptr; P.n_patches = 0;
     P.q_count = nullptr; P.q_done = nullptr;
+    P.dir = nullptr;
+    if (B == 32 && n_dir > 0 && n_dir < (1LL << 31)) {     // 16 B per direction; otherwise variant 4 falls back to 3
+        CUDA_TRY(cudaMalloc((void **)&G->d_dir, sizeof(double2) * (size_t)n_dir));
+        P.dir = G->d_dir;
+    }
     P.tex = 0; P.atlas_shift = 0; P.atlas_mask = 0;
     P.qx = (d.nx + 2) / 2 + 1; P.qy = (d.ny + 2) / 2 + 1;
     P.qplane = (long long)P.qx * P.qy;
@@ -313,6 +329,11 @@ int build_geometry(oat_geometry *G)
     CUDA_TRY(cudaMallocHost((void **)&G->h_scal, sizeof(double) * 8));
     CUDA_TRY(cudaEventCreate(&G->ev0));
     CUDA_TRY(cudaEventCreate(&G->ev1));
+    if (P.dir) {
+        oat_launch_dir_table(P, NB, G->d_dir, 0);
+        CUDA_TRY(cudaGetLastError());
+        CUDA_TRY(cudaDeviceSynchronize());
+    }
     return OAT_OK;
 }
 
@@ -397,7 +418,7 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     G->last_launches = 0;
     const float *src = G->d_xpad;
     int variant = G->variant_project;
-    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_cells)) variant = 3;   // marching form needs B = 32 patches
+    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_cells || !P.dir)) variant = 3;   // marching form needs B = 32 patches
     if (variant == 4) {
         if (!G->d_cells) CUDA_TRY(cudaMalloc((void **)&G->d_cells, sizeof(float4) * 2 * G->n_cells));
         oat_launch_pad_cells(P, d_x, G->d_cells, st); ++G->last_launches;
@@ -425,7 +446,10 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     }
     CUDA_TRY(cudaEventRecord(G->ev0, st));
     bool launched;
-    { int rc = launch_traversal(G, 0, variant, src, fused ? d_y : nullptr, nullptr, G->d_g, nullptr, st, &launched); if (rc) return rc; }
+    if (variant == 4) {
+        launched = G->dev.n_patches > 0;
+        CUDA_TRY(oat_launch_march(0, G->dev, G->d_cells, nullptr, d_y, nullptr, G->d_g, st));
+    } else { int rc = launch_traversal(G, 0, variant, src, fused ? d_y : nullptr, nullptr, G->d_g, nullptr, st, &launched); if (rc) return rc; }
     if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
@@ -439,7 +463,7 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
     const OatDev &P = G->dev;
     G->last_launches = 0;
     int variant = G->variant_backproject;
-    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_faces)) variant = 3;   // marching form needs B = 32 patches
+    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_faces || !P.dir)) variant = 3;   // marching form needs B = 32 patches
     const bool faces = variant == 4;
     const bool quads = !faces && variant >= 2;
     float *acc = G->d_xpad;
@@ -447,6 +471,9 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
         if (!G->d_faces) CUDA_TRY(cudaMalloc((void **)&G->d_faces, sizeof(float4) * G->n_faces));
         acc = reinterpret_cast<float *>(G->d_faces);
         CUDA_TRY(cudaMemsetAsync(G->d_faces, 0, sizeof(float4) * G->n_faces, st));
+        int rc = ensure(&G->d_coef, G->n_dat); if (rc) return rc;
+        if ((rc = ensure_patches(G))) return rc;
+        oat_launch_coef(P, d_y, G->d_coef, st); ++G->last_launches;
     } else if (quads) {
         int rc = ensure_quads(G); if (rc) return rc;
         acc = reinterpret_cast<float *>(G->d_quads);
@@ -456,7 +483,10 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
     }
     CUDA_TRY(cudaEventRecord(G->ev0, st));
     bool launched;
-    { int rc = launch_traversal(G, 1, variant, nullptr, acc, d_y, nullptr, nullptr, st, &launched); if (rc) return rc; }
+    if (faces) {
+        launched = G->dev.n_patches > 0;
+        CUDA_TRY(oat_launch_march(1, G->dev, nullptr, G->d_faces, nullptr, G->d_coef, nullptr, st));
+    } else { int rc = launch_traversal(G, 1, variant, nullptr, acc, d_y, nullptr, nullptr, st, &launched); if (rc) return rc; }
     if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;

@@ -21,6 +21,10 @@
 #define OAT_NW (OAT_NT / 32)
 #define OAT_RI 32          // rings per patch (schedule 1)
 #define OAT_RJ 32          // max azimuth samples per ring of a patch
+#ifndef OAT_MT
+#define OAT_MT 128         // threads per block of the marching kernels
+#endif
+#define OAT_ML 512         // list entries per build/consume round of the marching kernels (16 rings x 32)
 
 struct OatBand {
     double s_mid;      // radius of the band's anchor (k0 + (B-1)/2) in voxel units: rho/ds
@@ -30,7 +34,8 @@ struct OatBand {
     int n_rings;       // rings with theta_i < pi
     int k0, nk;        // first sample and number of samples (ragged last band: nk < B)
     int rb_ofs;        // first entry of this band in the ring-block sector table
-    int pad;
+    int dir_rings;     // leading rings of this band covered by the direction table (max over q of qb_rings)
+    long long dir_ofs; // first direction of this band in the direction table
 };
 
 struct __align__(16) OatRing {
@@ -57,6 +62,8 @@ struct OatDev {
     const int *rb_sectors;               // per (band, ring block): number of azimuth sectors S
     const unsigned long long *patches;   // schedule 1: Morton-sorted packed (q, band, ring block, sector)
     long long n_patches;
+    const double2 *dir;                  // direction table (marching kernels): (sin th cos phi, sin th sin phi) of ring r,
+                                         // azimuth j of band b at band.dir_ofs + ring.cum + j, fp64 (S2, S3)
     const int *q_count;                  // patches per transducer
     int *q_done;                         // patches finished in the running projection (zeroed per call)
     int qx, qy;                // quad layout (variant 2): quads per row / rows per plane
@@ -93,6 +100,13 @@ cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *
                            double *g, unsigned long long *counter, cudaStream_t st);
 cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
                              double *g, unsigned long long *counter, cudaStream_t st);
+// marching kernels (variant 4, B = 32): mode 0 gathers from cell records into g (and writes y rows, step A4),
+// mode 1 scatters coef[q,k] = g'_k rho_k^2 into the face-quad accumulators
+cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, float4 *faces, float *y_out,
+                             const float *coef, double *g, cudaStream_t st);
+void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream_t st);
+// coef[q,k] = kappa (y[k-1] - y[k+1]) / (2 dt t_k) * rho_k^2   (Eq. 22 L172 with the rho^2 of S8; 0 where t_k <= 0)
+void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st);
 cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, int *q_count, unsigned long long **patches_out, long long *n_patches);
 void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st);
 // vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)

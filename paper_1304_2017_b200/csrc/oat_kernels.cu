@@ -373,11 +373,12 @@ struct MarchStep {
     float fx, fy, fz;
 };
 
+template <int NT>
 __device__ __forceinline__ void consume_march_fwd(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid,
                                                   const float4 *__restrict__ cells, float (&acc)[32])
 {
     const float stepf = (float)P.step;
-    for (int e0 = tid * OAT_MU; e0 < n_list; e0 += OAT_NT * OAT_MU) {   // thread t: rays t*MU .. t*MU+MU-1, so idle warps skip
+    for (int e0 = tid * OAT_MU; e0 < n_list; e0 += NT * OAT_MU) {   // thread t: rays t*MU .. t*MU+MU-1, so idle warps skip
         float ax[OAT_MU], ay[OAT_MU], az[OAT_MU], om[OAT_MU], sx[OAT_MU], sy[OAT_MU], sz[OAT_MU];
         int bx[OAT_MU], by[OAT_MU], bz[OAT_MU];
         float prx[OAT_MU], pry[OAT_MU], prz[OAT_MU];      // previous step's rounded coordinates (cell identity)
@@ -472,11 +473,12 @@ __device__ __forceinline__ void red_add_v4_if(float4 *addr, float a, float b, fl
                  ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d), "r"((int)pred) : "memory");
 }
 
+template <int NT>
 __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid,
                                                   const float *__restrict__ s_coef, float4 *__restrict__ faces)
 {
     const float stepf = (float)P.step;
-    for (int ei = tid; ei < n_list; ei += OAT_NT) {
+    for (int ei = tid; ei < n_list; ei += NT) {
         const Entry e = list[ei];
         const float mx = fabsf(e.u.x), my = fabsf(e.u.y), mz = fabsf(e.u.z);
         int o = (mx >= my && mx >= mz) ? 0 : (my >= mz ? 1 : 2);
@@ -497,8 +499,7 @@ __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const Entry *
         const bool flip = u0 < 0.f;
         const float sg = flip ? -stepf : stepf;
         const float s0 = u0 * sg, s1 = u1 * sg, s2 = u2 * sg;   // s0 >= 0: the ray advances along local axis 0
-        const float *cp = s_coef + (flip ? 31 : 0);
-        const int cs = flip ? -1 : 1;
+        const float *cp = s_coef + (flip ? 32 : 0);        // [0,32): coef_k, [32,64): coef_{31-k}
         const float om = e.a.w;
         float L0 = 0.f, L1 = 0.f, L2 = 0.f, L3 = 0.f, H0 = 0.f, H1 = 0.f, H2 = 0.f, H3 = 0.f;
         float pr0 = 0.f, pr1 = 0.f, pr2 = 0.f;             // never equal to a rounded coordinate (those are >= 2^22)
@@ -524,7 +525,8 @@ __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const Entry *
             valid = ((unsigned)i0 <= n0) & ((unsigned)i1 <= n1) & ((unsigned)i2 <= n2);
             cur = qb + ((i0 * nc + i2) * nb + i1);
             const float f0 = t0 - (r0 - OAT_MAGIC), f1 = t1 - (r1 - OAT_MAGIC), f2 = t2 - (r2 - OAT_MAGIC);
-            const float cw = valid ? cp[cs * k] * om : 0.f;
+            const float cwk = cp[k] * om;
+            const float cw = valid ? cwk : 0.f;
             const float e1 = 1.f - f1, e2 = 1.f - f2;
             const float q0 = e1 * e2, q1 = f1 * e2, q2 = e1 * f2, q3 = f1 * f2;
             const float wh = cw * f0, wl = cw - wh;
@@ -688,7 +690,7 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
     Entry *list = reinterpret_cast<Entry *>(smem_raw);
     __shared__ double s_frame[12];
     __shared__ float s_red[OAT_NW][32];
-    __shared__ float s_delta[32], s_coef[32];
+    __shared__ float s_delta[32], s_coef[64];
     __shared__ int s_count;
     __shared__ int s_last;
 
@@ -704,7 +706,7 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
         const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
         const int S = P.rb_sectors[band.rb_ofs + rb];
         const LaneCtx L = lane_setup<MODE>(P, band, q, lane, y);
-        if (MODE == 1 && VAR >= 3 && warp == 0) { s_delta[lane] = L.delta; s_coef[lane] = L.active ? L.coef : 0.f; }
+        if (MODE == 1 && VAR >= 3 && warp == 0) { s_delta[lane] = L.delta; s_coef[lane] = s_coef[63 - lane] = L.active ? L.coef : 0.f; }
         float acc = 0.f;
         unsigned cnt = 0;
         __syncthreads();
@@ -728,9 +730,9 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
                 float a32[32];
 #pragma unroll
                 for (int i = 0; i < 32; ++i) a32[i] = 0.f;
-                consume_march_fwd(P, list, s_count, tid, reinterpret_cast<const float4 *>(xpad), a32);
+                consume_march_fwd<OAT_NT>(P, list, s_count, tid, reinterpret_cast<const float4 *>(xpad), a32);
                 acc = warp_transpose_sum(a32, lane);
-            } else if (MODE == 1 && VAR == 4) consume_march_bwd(P, list, s_count, tid, s_coef, reinterpret_cast<float4 *>(xacc));
+            } else if (MODE == 1 && VAR == 4) consume_march_bwd<OAT_NT>(P, list, s_count, tid, s_coef, reinterpret_cast<float4 *>(xacc));
             else if (MODE == 1 && VAR == 3) consume_march(P, list, s_count, tid, band.nk, s_delta, s_coef, xacc);
             else consume_list<MODE, ((MODE == 1 && VAR == 3) ? 2 : (VAR == 4 ? 3 : VAR))>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
         }
@@ -758,6 +760,164 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
             }
         }
         __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Marching kernels (variant 4, B = 32): the patch schedule with everything that is not the per-sample
+// loop trimmed -- small blocks (OAT_MT threads, 8 resident per SM) so that the dependent loads at the top
+// of a patch overlap other blocks' marching; directions from the fp64 table instead of sincospi; the
+// adjoint time stencil precomputed per (q,k) by oat_coef_kernel; a patch's 32 rings built and consumed in
+// rounds of OAT_ML / 32 rings (24 KB of list per block).
+// ------------------------------------------------------------------------------------------------
+#ifndef OAT_MBLK
+#define OAT_MBLK 8
+#endif
+
+// same result as make_entry(), direction taken from the table: (dlx, dly) = sin(theta_i) (cos phi_j, sin phi_j)
+__device__ __forceinline__ bool make_entry_tab(const OatDev &P, const OatBand &band, double2 d, double ct, float omega,
+                                               const double *s_frame, Entry &e)
+{
+    float uu[3], af[3];
+    int ai[3];
+    bool hit = true;
+    const float lim[3] = {(float)P.nx + 1.01f, (float)P.ny + 1.01f, (float)P.nz + 1.01f};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double ua = d.x * s_frame[a] + d.y * s_frame[3 + a] + ct * s_frame[6 + a];
+        const double an = s_frame[9 + a] + band.s_mid * ua;
+        const double ar = rint(an);
+        uu[a] = (float)ua;
+        af[a] = (float)(an - ar);
+        ai[a] = (int)ar;
+        const float p0 = (float)(s_frame[9 + a] + (double)band.s_lo * ua);
+        const float p1 = (float)(s_frame[9 + a] + (double)band.s_hi * ua);
+        hit = hit && (fmaxf(p0, p1) >= -0.01f) && (fminf(p0, p1) <= lim[a]);
+    }
+    e.a = make_float4(af[0], af[1], af[2], omega);
+    e.u = make_float4(uu[0], uu[1], uu[2], 0.f);
+    e.i = make_int4(ai[0] - OAT_MAGIC_BITS, ai[1] - OAT_MAGIC_BITS, ai[2] - OAT_MAGIC_BITS, 0);
+    return hit;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(OAT_MT, OAT_MBLK)
+oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__restrict__ faces, float *__restrict__ y_out,
+                 const float *__restrict__ coef, double *__restrict__ g)
+{
+    __shared__ Entry list[OAT_ML];
+    __shared__ double s_frame[12];
+    __shared__ float s_red[OAT_MT / 32][32];
+    __shared__ float s_coef[64];
+    __shared__ int s_count[OAT_RI * OAT_RJ / OAT_ML];
+    __shared__ int s_flag;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (long long item = blockIdx.x; item < P.n_patches; item += gridDim.x) {
+        int q, b, rb, sec;
+        unpack_item(P.patches[item], q, b, rb, sec);
+        if (tid < 12) s_frame[tid] = P.frame[(size_t)q * 12 + tid];
+        if (tid < OAT_RI * OAT_RJ / OAT_ML) s_count[tid] = 0;
+        const OatBand band = P.band[b];
+        const OatRing *__restrict__ ring = P.ring + band.ring_ofs;
+        const double2 *__restrict__ dir = P.dir + band.dir_ofs;
+        const int r0 = rb * OAT_RI;
+        const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
+        const int S = P.rb_sectors[band.rb_ofs + rb];
+        if (MODE == 1 && warp == 0) {                      // B1: the band's 32 coefficients g'_k rho_k^2, forward and reversed
+            const float cf = lane < band.nk ? coef[(size_t)q * P.K + band.k0 + lane] : 0.f;
+            s_coef[lane] = cf;
+            s_coef[63 - lane] = cf;
+            const bool any = __any_sync(0xffffffffu, cf != 0.f);
+            if (lane == 0) s_flag = any ? 1 : 0;
+        }
+        float a32[32];
+        if (MODE == 0) {
+#pragma unroll
+            for (int i = 0; i < 32; ++i) a32[i] = 0.f;
+        }
+        __syncthreads();
+        // a band whose 32 data values give g' = 0 contributes exactly nothing to H^T y
+        const bool live = (MODE != 1) || (s_flag != 0);
+        for (int rc = r0, round = 0; live && rc < r1; rc += OAT_ML / OAT_RJ, ++round) {
+            // ---------------------------------------------------------------- build (A2: directions -> ray anchors)
+            const int re = min(rc + OAT_ML / OAT_RJ, r1);
+            for (int t = tid; t < OAT_ML; t += OAT_MT) {
+                const int r = rc + t / OAT_RJ, jl = t % OAT_RJ;
+                if (r >= re) break;
+                const OatRing R = ring[r];
+                const int j0 = (int)(((long long)R.N * sec + S - 1) / S);
+                const int j1 = (int)(((long long)R.N * (sec + 1) + S - 1) / S);
+                if (j0 + jl >= j1) continue;
+                Entry e;
+                if (!make_entry_tab(P, band, dir[R.cum + j0 + jl], R.ct, R.omega, s_frame, e)) continue;
+                list[atomicAdd(&s_count[round], 1)] = e;
+            }
+            __syncthreads();
+            // ---------------------------------------------------------------- consume (A3 / B2-B3)
+            if (MODE == 0) consume_march_fwd<OAT_MT>(P, list, s_count[round], tid, cells, a32);
+            else consume_march_bwd<OAT_MT>(P, list, s_count[round], tid, s_coef, faces);
+            __syncthreads();                               // the list is rebuilt by the next round / item
+        }
+        if (MODE == 0) {
+            // S5: warp sums -> fp64 cross-warp combine -> one fp64 atomic per time sample
+            s_red[warp][lane] = warp_transpose_sum(a32, lane);
+            __syncthreads();
+            if (warp == 0) {
+                double sum = 0.0;
+#pragma unroll
+                for (int w = 0; w < OAT_MT / 32; ++w) sum += (double)s_red[w][lane];
+                const int k = band.k0 + lane;
+                const double rho = P.c * (P.t0 + (double)k * P.dt);
+                if (lane < band.nk && rho > 0.0 && sum != 0.0) atomicAdd(&g[(size_t)q * P.K + k], rho * rho * sum);
+                // Fused step A4 (Eq. 3 L63 / Eq. 13): the block that completes the LAST patch of transducer q turns
+                // the finished fp64 row g[q,:] into pressure.  Every lane fences its own atomics, one lane counts.
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) s_flag = (atomicAdd(&P.q_done[q], 1) + 1 == P.q_count[q]) ? 1 : 0;
+            }
+            __syncthreads();
+            if (s_flag) {
+                __threadfence();
+                const double *gq = g + (size_t)q * P.K;
+                float *yq = y_out + (size_t)q * P.K;
+                for (int k = tid; k < P.K; k += OAT_MT) {
+                    double sp = 0.0, sm = 0.0;
+                    if (k + 1 < P.K) { const double t = P.t0 + (double)(k + 1) * P.dt; if (t > 0.0) sp = __ldcg(gq + k + 1) / t; }
+                    if (k - 1 >= 0) { const double t = P.t0 + (double)(k - 1) * P.dt; if (t > 0.0) sm = __ldcg(gq + k - 1) / t; }
+                    yq[k] = (float)(P.kappa * (sp - sm) / (2.0 * P.dt));
+                }
+            }
+        }
+        __syncthreads();                                   // s_flag, s_red, s_coef reused by the next item
+    }
+}
+
+// direction table (once per geometry): one block per (band, ring); see OatDev::dir
+__global__ void oat_dir_table_kernel(const OatDev P, double2 *__restrict__ dir)
+{
+    const OatBand band = P.band[blockIdx.y];
+    for (int r = blockIdx.x; r < band.dir_rings; r += gridDim.x) {
+        const OatRing R = P.ring[band.ring_ofs + r];
+        for (int j = threadIdx.x; j < R.N; j += blockDim.x) {
+            double sd, cd;
+            sincospi(2.0 * (double)j / (double)R.N, &sd, &cd);        // same expression as make_entry()
+            dir[band.dir_ofs + R.cum + j] = make_double2(R.st * cd, R.st * sd);
+        }
+    }
+}
+
+// S7 with the rho^2 of S8 folded in: coef[q,k] = kappa (y[k-1] - y[k+1]) / (2 dt) / t_k * rho_k^2, 0 where t_k <= 0
+__global__ void oat_coef_kernel(const OatDev P, const float *__restrict__ y, float *__restrict__ coef)
+{
+    const long long n = (long long)P.Q * P.K;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int k = (int)(i % P.K);
+        const double tk = P.t0 + (double)k * P.dt, rho = P.c * tk;
+        const float ym = (k - 1 >= 0) ? y[i - 1] : 0.f;
+        const float yp = (k + 1 < P.K) ? y[i + 1] : 0.f;
+        const double sp = P.kappa * ((double)ym - (double)yp) / (2.0 * P.dt);   // Eq. 22
+        coef[i] = rho > 0.0 ? (float)(sp / tk * rho * rho) : 0.f;
     }
 }
 
@@ -1128,6 +1288,28 @@ static cudaError_t launch_patch_t(const OatDev &P, const float *xpad, float *xac
     const unsigned grid = (unsigned)(P.n_patches < cap ? P.n_patches : cap);
     oat_patch_kernel<MODE, VAR><<<grid, OAT_NT, smem, st>>>(P, xpad, xacc, y, g, counter);
     return cudaGetLastError();
+}
+
+cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, float4 *faces, float *y_out,
+                             const float *coef, double *g, cudaStream_t st)
+{
+    if (P.n_patches <= 0) return cudaSuccess;
+    const long long cap = 0x7fffffffLL;
+    const unsigned grid = (unsigned)(P.n_patches < cap ? P.n_patches : cap);
+    if (mode == 0) oat_march_kernel<0><<<grid, OAT_MT, 0, st>>>(P, cells, faces, y_out, coef, g);
+    else oat_march_kernel<1><<<grid, OAT_MT, 0, st>>>(P, cells, faces, y_out, coef, g);
+    return cudaGetLastError();
+}
+
+void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream_t st)
+{
+    if (n_bands > 0) oat_dir_table_kernel<<<dim3(256, (unsigned)n_bands), 128, 0, st>>>(P, dir);
+}
+
+void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st)
+{
+    const long long n = (long long)P.Q * P.K;
+    if (n > 0) oat_coef_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, y, coef);
 }
 
 cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
