@@ -29,6 +29,9 @@ METRIC = "ms per H and per H^T at 240^3 voxels x 9216 transducers x 2048 t (valu
 # Algorithmic fp32 work per interpolation sample: position 3 FMA, 3 floor, 3 frac,
 # 7 lerps (sub + FMA) or 8 weight products + 8 accumulates, 1 quadrature FMA  ->  36 flop (FMA = 2).
 FLOP_PER_SAMPLE = 36.0
+# Vector reductions per interpolation sample of the face-carrying H^T: ncu counts 1.562e10
+# predicated-on RED.128 lanes for 2.478e10 in-box samples on the config-3 subset profiled in profiles/.
+RED_PER_SAMPLE = 0.63
 # B200 fp32 peak derived from unit counts and clocks (guide: 148 SMs x 128 fp32 lanes x 2 flop x max SM clock)
 N_SM, FP32_LANES = 148, 128
 
@@ -254,13 +257,25 @@ def run_ours(args):
         dom = "backproject" if k_t >= k_h else "project"
         k_ms = max(k_t, k_h)
         achieved = n_samples * FLOP_PER_SAMPLE / (k_ms * 1e-3) / 1e12 if k_ms > 0 else 0.0
-        roofline = {"bound": "alu", "kernel": f"oat_patch_kernel<{1 if dom == 'backproject' else 0},*> ({dom})",
+        roofline = {"bound": "alu", "kernel": f"oat_march_kernel<{1 if dom == 'backproject' else 0}> ({dom})",
                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak else None,
                     "traffic": None, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_step if ms_step else None,
                     "peak_source": f"148 SM x 128 fp32 lanes x 2 flop x {peak_src}",
                     "algorithmic": f"{FLOP_PER_SAMPLE:.0f} fp32 flop per interpolation sample x {n_samples:.4g} samples per launch",
                     "other_kernel": {"kernel_ms": min(k_t, k_h),
                                      "frac": (n_samples * FLOP_PER_SAMPLE / (min(k_t, k_h) * 1e-3) / 1e12 / peak) if min(k_t, k_h) > 0 else None}}
+        # What ncu and the micro-benchmarks name as the binding unit of each kernel: H^T retires
+        # vector reductions (RED.128) at the rate the L2 atomic path sustains; the peak is measured live.
+        try:
+            red_peak = oat.oat_measure_red_rate(local)
+            red_lanes = RED_PER_SAMPLE * n_samples
+            roofline["limiter"] = {"kernel": "oat_march_kernel<1> (backproject)", "unit": "L2 vector reductions (RED.128 lanes/s)",
+                                   "achieved": red_lanes / (k_t * 1e-3) if k_t > 0 else None, "peak": red_peak,
+                                   "frac": (red_lanes / (k_t * 1e-3) / red_peak) if (k_t > 0 and red_peak > 0) else None,
+                                   "algorithmic": f"{RED_PER_SAMPLE} reductions per sample (cell crossings of the marched rays, ncu inst count) x {n_samples:.4g} samples",
+                                   "peak_source": "oat_measure_red_rate(): scattered red.global.add.v4.f32 into an L2-resident 64 MB buffer, same run"}
+        except Exception as ex:
+            roofline["limiter"] = {"error": str(ex)}
         cpu = None
         if not args.no_cpu_baseline and world == 1:       # rank 0 at N=1 only
             try:

@@ -113,6 +113,12 @@ int oat_last_launch_count(const oat_geometry *geom);
  * oat_project / oat_backproject; synchronises that stream.  Negative if none was recorded. */
 float oat_last_kernel_ms(oat_geometry *geom);
 
+/* Measurement aid for the roofline of H^T: sustained rate, in lanes per second, at which
+ * `device` retires 16-byte vector reductions (red.global.add.v4.f32) that hit distinct 32-byte sectors of an
+ * L2-resident 64 MB buffer -- the unit that bounds the backprojection scatter (Alg. 6).  Allocates and
+ * frees its own scratch, synchronises the device.  Negative return on error. */
+int oat_measure_red_rate(int device, double *lanes_per_s);
+
 const char *oat_last_error(void);
 const char *oat_version(void);
 

@@ -19,7 +19,7 @@ EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
-    "oat_last_launch_count", "oat_last_kernel_ms", "oat_last_error", "oat_version",
+    "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_last_error", "oat_version",
 ]
 
 
@@ -79,6 +79,8 @@ def load():
     lib.oat_last_kernel_ms.restype = ctypes.c_float
     lib.oat_last_error.restype = ctypes.c_char_p
     lib.oat_version.restype = ctypes.c_char_p
+    lib.oat_measure_red_rate.argtypes = [ctypes.c_int, dp]
+    lib.oat_measure_red_rate.restype = ctypes.c_int
     _lib = lib
     return lib
 
@@ -252,3 +254,10 @@ def oat_last_launch_count(g) -> int:
 
 def oat_last_kernel_ms(g) -> float:
     return float(load().oat_last_kernel_ms(g.handle))
+
+
+def oat_measure_red_rate(device: int = 0) -> float:
+    """Sustained scattered RED.128 lanes per second on `device` (roofline unit of H^T)."""
+    v = ctypes.c_double(0.0)
+    _check(load().oat_measure_red_rate(int(device), ctypes.byref(v)))
+    return float(v.value)

@@ -107,6 +107,8 @@ cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, flo
 void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream_t st);
 // coef[q,k] = kappa (y[k-1] - y[k+1]) / (2 dt t_k) * rho_k^2   (Eq. 22 L172 with the rho^2 of S8; 0 where t_k <= 0)
 void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st);
+// micro-benchmark behind oat_measure_red_rate(): `iters` scattered RED.128 per thread into `buf` (n16 float4 records)
+void oat_launch_red_probe(float4 *buf, unsigned n16, int iters, int blocks, cudaStream_t st);
 cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, int *q_count, unsigned long long **patches_out, long long *n_patches);
 void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st);
 // vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)

@@ -921,6 +921,19 @@ __global__ void oat_coef_kernel(const OatDev P, const float *__restrict__ y, flo
     }
 }
 
+// probe for oat_measure_red_rate(): every lane adds a float4 into its own pseudo-random 32-byte sector
+__global__ void oat_red_probe_kernel(float4 *__restrict__ buf, unsigned n16, int iters)
+{
+    const unsigned lane = threadIdx.x & 31, gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    unsigned s = gw * 2654435761u + 12345u;
+    for (int i = 0; i < iters; ++i) {
+        s = s * 1664525u + 1013904223u;
+        const unsigned h = (s >> 4) + lane * 2654435761u;
+        const unsigned r = ((h ^ (h >> 13)) * 0x9E3779B1u) % (n16 / 2);
+        red_add_v4(buf + 2 * (size_t)r, 1.f, 1.f, 1.f, 1.f);
+    }
+}
+
 // number of patches per transducer (for the fused time-difference epilogue)
 __global__ void oat_count_patches_kernel(const unsigned long long *__restrict__ patches, long long n, int *__restrict__ q_count)
 {
@@ -1304,6 +1317,11 @@ cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, flo
 void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream_t st)
 {
     if (n_bands > 0) oat_dir_table_kernel<<<dim3(256, (unsigned)n_bands), 128, 0, st>>>(P, dir);
+}
+
+void oat_launch_red_probe(float4 *buf, unsigned n16, int iters, int blocks, cudaStream_t st)
+{
+    oat_red_probe_kernel<<<blocks, 256, 0, st>>>(buf, n16, iters);
 }
 
 void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st)
