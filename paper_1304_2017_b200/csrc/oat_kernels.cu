@@ -289,12 +289,8 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
             const unsigned cell = in ? quad_index(P, s.ix, s.iy, s.iz) : 0xffffffffu;
             if (cell != cur) {
                 if (cur != 0xffffffffu) {
-#if OAT_HALF_RED
-                    red_add_v4(quads + cur, a0 + a4, a1 + a5, a2 + a6, a3 + a7);
-#else
                     red_add_v4(quads + cur, a0, a1, a2, a3);
                     red_add_v4(quads + cur + P.qplane, a4, a5, a6, a7);
-#endif
                 }
                 a0 = a1 = a2 = a3 = a4 = a5 = a6 = a7 = 0.f;
                 cur = cell;
@@ -316,34 +312,19 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
 }
 
 // CONSUME for H, "marching" form (project variant 4, B = 32): one THREAD per ray, stepping through the
-// band's 32 time samples in order, OAT_MU rays interleaved per thread (independent load chains).
+// band's 32 time samples in order.
 //   position   t_k = fma(u*step, k - 15.5, anchor)   (same fp64 anchor as every other variant; the
 //              immediate-operand FMA keeps one rounding at |t| < ~6 voxels)
 //   cell       floor by the round-down magic add; the cell's 32-byte record (8 polynomial coefficients of
 //              the trilinear interpolant, see oat_pad_cells_kernel) is (re)loaded with a PREDICATED 256-bit
 //              load only when the ray has entered a new cell -- ~2-3 samples share one load, and the L1
-//              data stage sees ~0.4 sectors per sample instead of 8 scalar gathers
+//              data stage sees ~0.45 loads per sample instead of 8 scalar gathers
 //   value      7 FMAs (Horner in fx, fy, fz) instead of 7 lerps = 14 ops
 // acc[k] holds the thread's sum over its rays for sample k; the caller transposes/reduces over the warp.
-#ifndef OAT_MU
-#define OAT_MU 1
-#endif
-#ifndef OAT_ALWAYS_LOAD
-#define OAT_ALWAYS_LOAD 0
-#endif
-#ifndef OAT_HALF_RED
-#define OAT_HALF_RED 0   // experiment only: wrong results, half the reductions
-#endif
-#ifndef OAT_PREFETCH
-#define OAT_PREFETCH 0
-#endif
-#ifndef OAT_DBUF
-#define OAT_DBUF 0
-#endif
-#ifndef OAT_MB
-#define OAT_MB 4      // resident blocks per SM the marching variants are compiled for (measured best: 64 registers)
-#endif
-
+// Measured dead ends (B200, config-3 subset): two rays interleaved per thread, an L1 prefetch (CCTL.PF1) of the
+// next step's record, unconditional reloads, register double-buffering of the next record (ptxas hoists all 32
+// loads and spills) and cp.async staging through shared memory (LDGSTS of scattered 16-byte pieces is ~4x slower)
+// are all slower than this form at 8 resident 128-thread blocks per SM.
 __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
@@ -352,98 +333,35 @@ __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool p
         : "l"(p), "r"((int)pred));
 }
 
-// predicated 256-bit load into fresh registers (contents undefined where pred is false)
-__device__ __forceinline__ void ldg256_to(float (&c)[8], const float4 *p, bool pred)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
-        "@p ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
-        : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3]), "=f"(c[4]), "=f"(c[5]), "=f"(c[6]), "=f"(c[7])
-        : "l"(p), "r"((int)pred));
-}
-
-__device__ __forceinline__ void prefetch_l1_if(const float4 *p, bool pred)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %1, 0;\n\t@p prefetch.global.L1 [%0];\n\t}" ::"l"(p), "r"((int)pred));
-}
-
-// one step of one ray: cell record index, "entered a new cell" flag and the in-cell fractions
-struct MarchStep {
-    unsigned idx;
-    bool ch;
-    float fx, fy, fz;
-};
-
 template <int NT>
 __device__ __forceinline__ void consume_march_fwd(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid,
                                                   const float4 *__restrict__ cells, float (&acc)[32])
 {
     const float stepf = (float)P.step;
-    for (int e0 = tid * OAT_MU; e0 < n_list; e0 += NT * OAT_MU) {   // thread t: rays t*MU .. t*MU+MU-1, so idle warps skip
-        float ax[OAT_MU], ay[OAT_MU], az[OAT_MU], om[OAT_MU], sx[OAT_MU], sy[OAT_MU], sz[OAT_MU];
-        int bx[OAT_MU], by[OAT_MU], bz[OAT_MU];
-        float prx[OAT_MU], pry[OAT_MU], prz[OAT_MU];      // previous step's rounded coordinates (cell identity)
-        float c[OAT_MU][8];
-        MarchStep nxt[OAT_MU];
-        auto step_of = [&](int u, int k) {
-            const float kk = (float)k - 15.5f;
-            const float tx = fmaf(sx[u], kk, ax[u]), ty = fmaf(sy[u], kk, ay[u]), tz = fmaf(sz[u], kk, az[u]);
-            const float rx = __fadd_rd(tx, OAT_MAGIC), ry = __fadd_rd(ty, OAT_MAGIC), rz = __fadd_rd(tz, OAT_MAGIC);
-            MarchStep m;
-            m.ch = (rx != prx[u]) | (ry != pry[u]) | (rz != prz[u]);
-            prx[u] = rx; pry[u] = ry; prz[u] = rz;
-            const int ix = __float_as_int(rx) + bx[u], iy = __float_as_int(ry) + by[u], iz = __float_as_int(rz) + bz[u];
-            const bool in = ((unsigned)ix <= (unsigned)P.nx) & ((unsigned)iy <= (unsigned)P.ny) & ((unsigned)iz <= (unsigned)P.nz);
-            m.idx = in ? (unsigned)((iz * P.cy + iy) * P.cx + ix) : P.zero_cell;
-            m.fx = tx - (rx - OAT_MAGIC); m.fy = ty - (ry - OAT_MAGIC); m.fz = tz - (rz - OAT_MAGIC);
-            return m;
-        };
+    for (int ei = tid; ei < n_list; ei += NT) {
+        const Entry e = list[ei];
+        const float sx = e.u.x * stepf, sy = e.u.y * stepf, sz = e.u.z * stepf;
+        float prx = 0.f, pry = 0.f, prz = 0.f;            // previous step's rounded coordinates (cell identity);
+                                                          // 0 never equals a rounded coordinate (those are >= 2^22)
+        float c[8];
 #pragma unroll
-        for (int u = 0; u < OAT_MU; ++u) {
-            const int ei = e0 + u;
-            const bool valid = ei < n_list;
-            const Entry e = list[valid ? ei : e0];
-            ax[u] = e.a.x; ay[u] = e.a.y; az[u] = e.a.z; om[u] = valid ? e.a.w : 0.f;
-            sx[u] = e.u.x * stepf; sy[u] = e.u.y * stepf; sz[u] = e.u.z * stepf;
-            bx[u] = e.i.x; by[u] = e.i.y; bz[u] = e.i.z;
-            prx[u] = pry[u] = prz[u] = 0.f;               // never equals a rounded coordinate (those are >= 2^22)
-#pragma unroll
-            for (int i = 0; i < 8; ++i) c[u][i] = 0.f;
-            nxt[u] = step_of(u, 0);
-#if OAT_DBUF
-            ldg256_if(c[u], cells + 2 * (size_t)nxt[u].idx, true);
-#elif OAT_PREFETCH
-            prefetch_l1_if(cells + 2 * (size_t)nxt[u].idx, true);
-#endif
-        }
+        for (int i = 0; i < 8; ++i) c[i] = 0.f;
 #pragma unroll
         for (int k = 0; k < 32; ++k) {
-#pragma unroll
-            for (int u = 0; u < OAT_MU; ++u) {
-                const MarchStep cur = nxt[u];
-                if (k + 1 < 32) {                          // next step's cell: start its L2 -> L1 fetch now
-                    nxt[u] = step_of(u, k + 1);
-#if OAT_PREFETCH
-                    prefetch_l1_if(cells + 2 * (size_t)nxt[u].idx, nxt[u].ch);
-#endif
-                }
-#if OAT_DBUF
-                float Ln[8];                               // next step's record: in flight while this step is evaluated
-                if (k + 1 < 32) ldg256_to(Ln, cells + 2 * (size_t)nxt[u].idx, nxt[u].ch);
-#elif OAT_ALWAYS_LOAD
-                ldg256_if(c[u], cells + 2 * (size_t)cur.idx, true);
-#else
-                ldg256_if(c[u], cells + 2 * (size_t)cur.idx, cur.ch);
-#endif
-                const float lo = fmaf(cur.fy, fmaf(cur.fx, c[u][3], c[u][2]), fmaf(cur.fx, c[u][1], c[u][0]));
-                const float hi = fmaf(cur.fy, fmaf(cur.fx, c[u][7], c[u][6]), fmaf(cur.fx, c[u][5], c[u][4]));
-                acc[k] = fmaf(om[u], fmaf(cur.fz, hi, lo), acc[k]);
-#if OAT_DBUF
-                if (k + 1 < 32) {
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) c[u][i] = nxt[u].ch ? Ln[i] : c[u][i];
-                }
-#endif
-            }
+            const float kk = (float)k - 15.5f;
+            const float tx = fmaf(sx, kk, e.a.x), ty = fmaf(sy, kk, e.a.y), tz = fmaf(sz, kk, e.a.z);
+            const float rx = __fadd_rd(tx, OAT_MAGIC), ry = __fadd_rd(ty, OAT_MAGIC), rz = __fadd_rd(tz, OAT_MAGIC);
+            const bool ch = (rx != prx) | (ry != pry) | (rz != prz);
+            prx = rx; pry = ry; prz = rz;
+            const int ix = __float_as_int(rx) + e.i.x, iy = __float_as_int(ry) + e.i.y, iz = __float_as_int(rz) + e.i.z;
+            // padded cell n' in [0, N] <=> xi in [-1, N): the sample touches at least one existing node (S4)
+            const bool in = ((unsigned)ix <= (unsigned)P.nx) & ((unsigned)iy <= (unsigned)P.ny) & ((unsigned)iz <= (unsigned)P.nz);
+            const unsigned idx = in ? (unsigned)((iz * P.cy + iy) * P.cx + ix) : P.zero_cell;
+            ldg256_if(c, cells + 2 * (size_t)idx, ch);
+            const float fx = tx - (rx - OAT_MAGIC), fy = ty - (ry - OAT_MAGIC), fz = tz - (rz - OAT_MAGIC);
+            const float lo = fmaf(fy, fmaf(fx, c[3], c[2]), fmaf(fx, c[1], c[0]));
+            const float hi = fmaf(fy, fmaf(fx, c[7], c[6]), fmaf(fx, c[5], c[4]));
+            acc[k] = fmaf(e.a.w, fmaf(fz, hi, lo), acc[k]);
         }
     }
 }
@@ -460,12 +378,6 @@ __device__ __forceinline__ void consume_march_fwd(const OatDev &P, const Entry *
 //     is carried over as the new L; only a step across one of the two minor axes flushes both quads.
 // About 0.65 reductions per sample instead of 0.9 for the z-only quads of variant 3.  Same positions, cells and
 // weights as consume_march_fwd, so H and H^T visit identical samples (Eq. 12 vs Eq. 23).
-#ifndef OAT_MBT
-#define OAT_MBT 3     // resident blocks per SM for the marching H^T kernel
-#endif
-#ifndef OAT_HT_ORIENT
-#define OAT_HT_ORIENT 3      // 3: dominant-axis orientations; 1: always the z orientation (experiment)
-#endif
 
 __device__ __forceinline__ void red_add_v4_if(float4 *addr, float a, float b, float c, float d, bool pred)
 {
@@ -481,8 +393,7 @@ __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const Entry *
     for (int ei = tid; ei < n_list; ei += NT) {
         const Entry e = list[ei];
         const float mx = fabsf(e.u.x), my = fabsf(e.u.y), mz = fabsf(e.u.z);
-        int o = (mx >= my && mx >= mz) ? 0 : (my >= mz ? 1 : 2);
-        if (OAT_HT_ORIENT == 1) o = 2;
+        const int o = (mx >= my && mx >= mz) ? 0 : (my >= mz ? 1 : 2);
         // local axes (0, 1, 2) = (a, b, c) = (x,y,z), (y,z,x), (z,x,y)
         const float a0 = o == 0 ? e.a.x : o == 1 ? e.a.y : e.a.z, a1 = o == 0 ? e.a.y : o == 1 ? e.a.z : e.a.x,
                     a2 = o == 0 ? e.a.z : o == 1 ? e.a.x : e.a.y;
@@ -682,7 +593,7 @@ __device__ __forceinline__ void unpack_item(unsigned long long v, int &q, int &b
 }
 
 template <int MODE, int VAR>
-__global__ void __launch_bounds__(OAT_NT, (VAR == 4 ? (MODE == 1 ? OAT_MBT : OAT_MB) : 3))
+__global__ void __launch_bounds__(OAT_NT, 3)
 oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restrict__ xacc,
                  const float *__restrict__ y, double *__restrict__ g, unsigned long long *__restrict__ counter)
 {
@@ -690,7 +601,7 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
     Entry *list = reinterpret_cast<Entry *>(smem_raw);
     __shared__ double s_frame[12];
     __shared__ float s_red[OAT_NW][32];
-    __shared__ float s_delta[32], s_coef[64];
+    __shared__ float s_delta[32], s_coef[32];
     __shared__ int s_count;
     __shared__ int s_last;
 
@@ -706,7 +617,7 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
         const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
         const int S = P.rb_sectors[band.rb_ofs + rb];
         const LaneCtx L = lane_setup<MODE>(P, band, q, lane, y);
-        if (MODE == 1 && VAR >= 3 && warp == 0) { s_delta[lane] = L.delta; s_coef[lane] = s_coef[63 - lane] = L.active ? L.coef : 0.f; }
+        if (MODE == 1 && VAR == 3 && warp == 0) { s_delta[lane] = L.delta; s_coef[lane] = L.active ? L.coef : 0.f; }
         float acc = 0.f;
         unsigned cnt = 0;
         __syncthreads();
@@ -726,15 +637,8 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
             }
             __syncthreads();
             // ---------------------------------------------------------------- consume
-            if (MODE == 0 && VAR == 4) {
-                float a32[32];
-#pragma unroll
-                for (int i = 0; i < 32; ++i) a32[i] = 0.f;
-                consume_march_fwd<OAT_NT>(P, list, s_count, tid, reinterpret_cast<const float4 *>(xpad), a32);
-                acc = warp_transpose_sum(a32, lane);
-            } else if (MODE == 1 && VAR == 4) consume_march_bwd<OAT_NT>(P, list, s_count, tid, s_coef, reinterpret_cast<float4 *>(xacc));
-            else if (MODE == 1 && VAR == 3) consume_march(P, list, s_count, tid, band.nk, s_delta, s_coef, xacc);
-            else consume_list<MODE, ((MODE == 1 && VAR == 3) ? 2 : (VAR == 4 ? 3 : VAR))>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
+            if (MODE == 1 && VAR == 3) consume_march(P, list, s_count, tid, band.nk, s_delta, s_coef, xacc);
+            else consume_list<MODE, ((MODE == 1 && VAR == 3) ? 2 : VAR)>(P, list, s_count, warp, lane, L, xpad, xacc, acc, cnt);
         }
         item_epilogue<MODE>(P, q, L, acc, cnt, warp, lane, s_red, g, counter);
         if (MODE == 0) {
@@ -1334,13 +1238,11 @@ cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float
                              double *g, unsigned long long *counter, cudaStream_t st)
 {
     if (P.n_patches <= 0) return cudaSuccess;
-    if (mode == 0) return variant == 4 ? launch_patch_t<0, 4>(P, xpad, xacc, y, g, counter, st)
-                        : variant == 3 ? launch_patch_t<0, 3>(P, xpad, xacc, y, g, counter, st)
+    if (mode == 0) return variant == 3 ? launch_patch_t<0, 3>(P, xpad, xacc, y, g, counter, st)
                         : variant == 2 ? launch_patch_t<0, 2>(P, xpad, xacc, y, g, counter, st)
                         : variant == 1 ? launch_patch_t<0, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_patch_t<0, 0>(P, xpad, xacc, y, g, counter, st);
-    if (mode == 1) return variant == 4 ? launch_patch_t<1, 4>(P, xpad, xacc, y, g, counter, st)
-                        : variant == 3 ? launch_patch_t<1, 3>(P, xpad, xacc, y, g, counter, st)
+    if (mode == 1) return variant == 3 ? launch_patch_t<1, 3>(P, xpad, xacc, y, g, counter, st)
                         : variant == 2 ? launch_patch_t<1, 2>(P, xpad, xacc, y, g, counter, st)
                         : variant == 1 ? launch_patch_t<1, 1>(P, xpad, xacc, y, g, counter, st)
                                        : launch_patch_t<1, 0>(P, xpad, xacc, y, g, counter, st);
