@@ -32,6 +32,9 @@ FLOP_PER_SAMPLE = 36.0
 # Vector reductions per interpolation sample of the face-carrying H^T: ncu counts 1.562e10
 # predicated-on RED.128 lanes for 2.478e10 in-box samples on the config-3 subset profiled in profiles/.
 RED_PER_SAMPLE = 0.63
+# 32-byte cell records requested from L2 per interpolation sample of the marching H: ncu counts
+# 1.079e10 global-load sectors (L1 hit rate 5 %) for 2.478e10 in-box samples on the same subset.
+SECTORS_PER_SAMPLE = 0.435
 # B200 fp32 peak derived from unit counts and clocks (guide: 148 SMs x 128 fp32 lanes x 2 flop x max SM clock)
 N_SM, FP32_LANES = 148, 128
 
@@ -276,6 +279,17 @@ def run_ours(args):
                                    "peak_source": "oat_measure_red_rate(): scattered red.global.add.v4.f32 into an L2-resident 64 MB buffer, same run"}
         except Exception as ex:
             roofline["limiter"] = {"error": str(ex)}
+        # H requests one 32-byte cell record from L2 per cell run of a ray; the peak is the measured scattered-sector rate
+        try:
+            gat_peak = oat.oat_measure_gather_rate(local)
+            sec = SECTORS_PER_SAMPLE * n_samples
+            roofline["limiter_H"] = {"kernel": "oat_march_kernel<0> (project)", "unit": "L1-miss sector loads from L2 (32 B sectors/s)",
+                                     "achieved": sec / (k_h * 1e-3) if k_h > 0 else None, "peak": gat_peak,
+                                     "frac": (sec / (k_h * 1e-3) / gat_peak) if (k_h > 0 and gat_peak > 0) else None,
+                                     "algorithmic": f"{SECTORS_PER_SAMPLE} cell records per sample (one per cell run of a marched ray, ncu sector count) x {n_samples:.4g} samples",
+                                     "peak_source": "oat_measure_gather_rate(): scattered ld.global.nc.v8.f32, one sector per lane, L2-resident 64 MB buffer, same run"}
+        except Exception as ex:
+            roofline["limiter_H"] = {"error": str(ex)}
         cpu = None
         if not args.no_cpu_baseline and world == 1:       # rank 0 at N=1 only
             try:

@@ -119,6 +119,12 @@ float oat_last_kernel_ms(oat_geometry *geom);
  * frees its own scratch, synchronises the device.  Negative return on error. */
 int oat_measure_red_rate(int device, double *lanes_per_s);
 
+/* Measurement aid for the roofline of H: sustained rate, in 32-byte sectors per second, at
+ * which `device` serves scattered 256-bit loads (ld.global.nc.v8.f32, one distinct sector per lane) that miss L1
+ * and hit an L2-resident 64 MB buffer -- the access of the projection's marching loop (one cell record per cell
+ * run of a ray, Eq. 12 L121 / Alg. 4).  Allocates and frees its own scratch, synchronises the device. */
+int oat_measure_gather_rate(int device, double *sectors_per_s);
+
 const char *oat_last_error(void);
 const char *oat_version(void);
 

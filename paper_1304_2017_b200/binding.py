@@ -19,7 +19,7 @@ EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
-    "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_last_error", "oat_version",
+    "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_last_error", "oat_version",
 ]
 
 
@@ -81,6 +81,8 @@ def load():
     lib.oat_version.restype = ctypes.c_char_p
     lib.oat_measure_red_rate.argtypes = [ctypes.c_int, dp]
     lib.oat_measure_red_rate.restype = ctypes.c_int
+    lib.oat_measure_gather_rate.argtypes = [ctypes.c_int, dp]
+    lib.oat_measure_gather_rate.restype = ctypes.c_int
     _lib = lib
     return lib
 
@@ -260,4 +262,11 @@ def oat_measure_red_rate(device: int = 0) -> float:
     """Sustained scattered RED.128 lanes per second on `device` (roofline unit of H^T)."""
     v = ctypes.c_double(0.0)
     _check(load().oat_measure_red_rate(int(device), ctypes.byref(v)))
+    return float(v.value)
+
+
+def oat_measure_gather_rate(device: int = 0) -> float:
+    """Sustained scattered 32-byte sector loads per second that miss L1 and hit L2 (roofline unit of H)."""
+    v = ctypes.c_double(0.0)
+    _check(load().oat_measure_gather_rate(int(device), ctypes.byref(v)))
     return float(v.value)

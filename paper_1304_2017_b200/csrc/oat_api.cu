@@ -746,6 +746,38 @@ int oat_measure_red_rate(int device, double *lanes_per_s)
     return OAT_OK;
 }
 
+int oat_measure_gather_rate(int device, double *sectors_per_s)
+{
+    if (!sectors_per_s) return fail(OAT_ERR_INVALID, "NULL argument");
+    CUDA_TRY(cudaSetDevice(device));
+    const size_t bytes = 64u << 20;                       // L2-resident, far larger than L1
+    const int blocks = 148 * 8, iters = 500;
+    float4 *buf = nullptr;
+    float *sink = nullptr;
+    cudaEvent_t a = nullptr, b = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&buf, bytes));
+    cudaError_t e = cudaMemset(buf, 0, bytes);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&sink, sizeof(float));
+    if (e == cudaSuccess) e = cudaEventCreate(&a);
+    if (e == cudaSuccess) e = cudaEventCreate(&b);
+    float ms = 0.f;
+    if (e == cudaSuccess) {
+        oat_launch_gather_probe(buf, (unsigned)(bytes / 16), 50, blocks, sink, 0);      // warm-up (fills L2)
+        cudaEventRecord(a, 0);
+        oat_launch_gather_probe(buf, (unsigned)(bytes / 16), iters, blocks, sink, 0);
+        cudaEventRecord(b, 0);
+        e = cudaEventSynchronize(b);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    }
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
+    cudaFree(sink);
+    cudaFree(buf);
+    if (e != cudaSuccess || !(ms > 0.f)) return fail(OAT_ERR_CUDA, "gather-rate probe failed: %s", cudaGetErrorString(e));
+    *sectors_per_s = (double)blocks * 256.0 * 4.0 * iters / (ms * 1e-3);
+    return OAT_OK;
+}
+
 const char *oat_last_error(void) { return g_err; }
 const char *oat_version(void) { return "oat-b200 0.1 (OAT-DISC v1; sm_100a)"; }
 

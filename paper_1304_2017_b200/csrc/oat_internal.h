@@ -109,6 +109,8 @@ void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream
 void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st);
 // micro-benchmark behind oat_measure_red_rate(): `iters` scattered RED.128 per thread into `buf` (n16 float4 records)
 void oat_launch_red_probe(float4 *buf, unsigned n16, int iters, int blocks, cudaStream_t st);
+// micro-benchmark behind oat_measure_gather_rate(): 4 x `iters` scattered 256-bit loads per thread from `buf`
+void oat_launch_gather_probe(const float4 *buf, unsigned n16, int iters, int blocks, float *sink, cudaStream_t st);
 cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, int *q_count, unsigned long long **patches_out, long long *n_patches);
 void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st);
 // vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)

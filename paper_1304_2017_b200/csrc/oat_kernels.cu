@@ -324,7 +324,11 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
 // Measured dead ends (B200, config-3 subset): two rays interleaved per thread, an L1 prefetch (CCTL.PF1) of the
 // next step's record, unconditional reloads, register double-buffering of the next record (ptxas hoists all 32
 // loads and spills) and cp.async staging through shared memory (LDGSTS of scattered 16-byte pieces is ~4x slower)
-// are all slower than this form at 8 resident 128-thread blocks per SM.
+// are all slower than this form at 8 resident 128-thread blocks per SM.  So are a depth-1 software pipeline of the
+// record load (8 selects per step), two rays interleaved per thread on 16 accumulators, and 6 or 5 resident blocks
+// with more registers: the kernel time does not react to occupancy or to loads in flight because it sits at the
+// rate at which an SM's L1 can send sector misses to L2 (ncu: l1tex__m_l1tex2xbar_req_cycles_active 51 %, 0.46
+// sectors per SM-cycle, L1 hit rate 5 % by construction -- every record is used by exactly one ray).
 __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
@@ -333,9 +337,12 @@ __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool p
         : "l"(p), "r"((int)pred));
 }
 
-template <int NT>
+// The 32 samples are split into two halves of 16 (K0 = 0 or 16), marched by different warps: 16 accumulators
+// per thread fit the 64-register budget of 8 resident blocks per SM (32 spilled to local memory: ncu showed
+// 0.8 LDL + 0.8 STL per warp-step and 30 % of the L2 traffic), at the price of one extra record load per ray.
+template <int NT, int K0>
 __device__ __forceinline__ void consume_march_fwd(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid,
-                                                  const float4 *__restrict__ cells, float (&acc)[32])
+                                                  const float4 *__restrict__ cells, float (&acc)[16])
 {
     const float stepf = (float)P.step;
     for (int ei = tid; ei < n_list; ei += NT) {
@@ -347,8 +354,8 @@ __device__ __forceinline__ void consume_march_fwd(const OatDev &P, const Entry *
 #pragma unroll
         for (int i = 0; i < 8; ++i) c[i] = 0.f;
 #pragma unroll
-        for (int k = 0; k < 32; ++k) {
-            const float kk = (float)k - 15.5f;
+        for (int k = 0; k < 16; ++k) {
+            const float kk = (float)(K0 + k) - 15.5f;
             const float tx = fmaf(sx, kk, e.a.x), ty = fmaf(sy, kk, e.a.y), tz = fmaf(sz, kk, e.a.z);
             const float rx = __fadd_rd(tx, OAT_MAGIC), ry = __fadd_rd(ty, OAT_MAGIC), rz = __fadd_rd(tz, OAT_MAGIC);
             const bool ch = (rx != prx) | (ry != pry) | (rz != prz);
@@ -449,11 +456,11 @@ __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const Entry *
     }
 }
 
-// sum acc[k] over the 32 lanes of the warp; lane l returns the total of sample k = l (31 shuffles)
-__device__ __forceinline__ float warp_transpose_sum(float (&acc)[32], int lane)
+// sum acc[k] over the 32 lanes of the warp; lanes l and l + 16 return the total of sample k = l (16 shuffles)
+__device__ __forceinline__ float warp_transpose_sum(float (&acc)[16], int lane)
 {
 #pragma unroll
-    for (int s = 16; s >= 1; s >>= 1) {
+    for (int s = 8; s >= 1; s >>= 1) {
         const bool up = (lane & s) != 0;
 #pragma unroll
         for (int i = 0; i < s; ++i) {
@@ -462,7 +469,7 @@ __device__ __forceinline__ float warp_transpose_sum(float (&acc)[32], int lane)
             acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, s);
         }
     }
-    return acc[0];
+    return acc[0] + __shfl_xor_sync(0xffffffffu, acc[0], 16);
 }
 
 // EPILOGUE of one work item: cross-warp combine in fp64 and one fp64 atomic per time sample (S5)
@@ -711,7 +718,7 @@ oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__res
 {
     __shared__ Entry list[OAT_ML];
     __shared__ double s_frame[12];
-    __shared__ float s_red[OAT_MT / 32][32];
+    __shared__ float s_red[OAT_MT / 32][16];
     __shared__ float s_coef[64];
     __shared__ int s_count[OAT_RI * OAT_RJ / OAT_ML];
     __shared__ int s_flag;
@@ -735,10 +742,10 @@ oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__res
             const bool any = __any_sync(0xffffffffu, cf != 0.f);
             if (lane == 0) s_flag = any ? 1 : 0;
         }
-        float a32[32];
+        float a16[16];                                     // MODE 0: warps [0, NW/2) march samples 0..15, the rest 16..31
         if (MODE == 0) {
 #pragma unroll
-            for (int i = 0; i < 32; ++i) a32[i] = 0.f;
+            for (int i = 0; i < 16; ++i) a16[i] = 0.f;
         }
         __syncthreads();
         // a band whose 32 data values give g' = 0 contributes exactly nothing to H^T y
@@ -759,18 +766,21 @@ oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__res
             }
             __syncthreads();
             // ---------------------------------------------------------------- consume (A3 / B2-B3)
-            if (MODE == 0) consume_march_fwd<OAT_MT>(P, list, s_count[round], tid, cells, a32);
-            else consume_march_bwd<OAT_MT>(P, list, s_count[round], tid, s_coef, faces);
+            if (MODE == 0) {
+                if (tid < OAT_MT / 2) consume_march_fwd<OAT_MT / 2, 0>(P, list, s_count[round], tid, cells, a16);
+                else consume_march_fwd<OAT_MT / 2, 16>(P, list, s_count[round], tid - OAT_MT / 2, cells, a16);
+            } else consume_march_bwd<OAT_MT>(P, list, s_count[round], tid, s_coef, faces);
             __syncthreads();                               // the list is rebuilt by the next round / item
         }
         if (MODE == 0) {
             // S5: warp sums -> fp64 cross-warp combine -> one fp64 atomic per time sample
-            s_red[warp][lane] = warp_transpose_sum(a32, lane);
+            const float tot = warp_transpose_sum(a16, lane);
+            if (lane < 16) s_red[warp][lane] = tot;
             __syncthreads();
             if (warp == 0) {
-                double sum = 0.0;
+                double sum = 0.0;                          // lane = sample k of the band; its half's warps hold the partial sums
 #pragma unroll
-                for (int w = 0; w < OAT_MT / 32; ++w) sum += (double)s_red[w][lane];
+                for (int w = 0; w < OAT_MT / 64; ++w) sum += (double)s_red[(lane >> 4) * (OAT_MT / 64) + w][lane & 15];
                 const int k = band.k0 + lane;
                 const double rho = P.c * (P.t0 + (double)k * P.dt);
                 if (lane < band.nk && rho > 0.0 && sum != 0.0) atomicAdd(&g[(size_t)q * P.K + k], rho * rho * sum);
@@ -836,6 +846,30 @@ __global__ void oat_red_probe_kernel(float4 *__restrict__ buf, unsigned n16, int
         const unsigned r = ((h ^ (h >> 13)) * 0x9E3779B1u) % (n16 / 2);
         red_add_v4(buf + 2 * (size_t)r, 1.f, 1.f, 1.f, 1.f);
     }
+}
+
+// probe for oat_measure_gather_rate(): every lane loads its own pseudo-random 32-byte sector (one 256-bit load, the
+// access of consume_march_fwd), four independent loads in flight per thread; the sum keeps the loads alive
+__global__ void oat_gather_probe_kernel(const float4 *__restrict__ buf, unsigned n16, int iters, float *__restrict__ sink)
+{
+    const unsigned lane = threadIdx.x & 31, gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    unsigned s = gw * 2654435761u + 54321u;
+    float acc = 0.f;
+    for (int i = 0; i < iters; ++i) {
+        float v[4][8];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            s = s * 1664525u + 1013904223u;
+            const unsigned h = (s >> 4) + lane * 2654435761u;
+            const unsigned r = ((h ^ (h >> 13)) * 0x9E3779B1u) % (n16 / 2);
+            asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                         : "=f"(v[u][0]), "=f"(v[u][1]), "=f"(v[u][2]), "=f"(v[u][3]), "=f"(v[u][4]), "=f"(v[u][5]), "=f"(v[u][6]), "=f"(v[u][7])
+                         : "l"(buf + 2 * (size_t)r));
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) acc += v[u][0] + v[u][7];
+    }
+    if (acc == 12345.678f) sink[0] = acc;
 }
 
 // number of patches per transducer (for the fused time-difference epilogue)
@@ -1226,6 +1260,11 @@ void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream
 void oat_launch_red_probe(float4 *buf, unsigned n16, int iters, int blocks, cudaStream_t st)
 {
     oat_red_probe_kernel<<<blocks, 256, 0, st>>>(buf, n16, iters);
+}
+
+void oat_launch_gather_probe(const float4 *buf, unsigned n16, int iters, int blocks, float *sink, cudaStream_t st)
+{
+    oat_gather_probe_kernel<<<blocks, 256, 0, st>>>(buf, n16, iters, sink);
 }
 
 void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st)
