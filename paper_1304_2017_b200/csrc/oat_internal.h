@@ -24,6 +24,7 @@
 #ifndef OAT_MT
 #define OAT_MT 128         // threads per block of the marching kernels
 #endif
+#define OAT_BU 8           // steps per trip of the (rolled) backprojection marching loop
 #define OAT_ML 512         // list entries per build/consume round of the marching kernels (16 rings x 32)
 
 struct OatBand {
