@@ -296,6 +296,40 @@ def run_ours(args):
                                      "peak_source": "oat_measure_gather_rate(): scattered ld.global.nc.v8.f32, one sector per lane, L2-resident 64 MB buffer, same run"}
         except Exception as ex:
             roofline["limiter_H"] = {"error": str(ex)}
+        # ---- row NEXT-1 (EIR convolution, penalty stencil): the steps either side of the path, timed at this config's sizes
+        next1 = None
+        try:
+            hbm = None
+            try:
+                hbm = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs"))
+            except Exception:
+                pass
+            taps = 128
+            tt = np.arange(taps) * w.dt
+            oat.oat_eir_set(g, (w.dt * np.exp(-tt / (0.15 * taps * w.dt)) * np.sin(2 * np.pi * 2.5 * tt)).astype(np.float32))
+            u = torch.empty_like(y); lx = torch.empty_like(x)
+
+            def timed(fn, reps=5):
+                fn(); torch.cuda.synchronize()
+                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                for _ in range(reps):
+                    fn()
+                b.record(stream); torch.cuda.synchronize()
+                return a.elapsed_time(b) / reps
+            ms_e = timed(lambda: oat.oat_eir_apply(g, y, u))
+            ms_ea = timed(lambda: oat.oat_eir_apply(g, y, u, adjoint=True))
+            ms_p = timed(lambda: oat.oat_penalty_apply(g, xb, lx))
+            by, bx = 2.0 * y.numel() * 4, 2.0 * x.numel() * 4          # read + write once
+            next1 = {"eir_taps": taps, "ms_eir": ms_e, "ms_eir_adjoint": ms_ea, "ms_penalty": ms_p,
+                     "eir_GBps": by / (ms_e * 1e-3) / 1e9, "penalty_GBps": bx / (ms_p * 1e-3) / 1e9,
+                     "hbm_peak_GBps": hbm, "penalty_frac_of_hbm": (bx / (ms_p * 1e-3) / 1e9 / hbm) if hbm else None,
+                     "eir_frac_of_hbm": (by / (ms_e * 1e-3) / 1e9 / hbm) if hbm else None,
+                     "share_of_pls_iteration": (ms_e + ms_ea + ms_p) / (ms_step + ms_e + ms_ea + ms_p),
+                     "note": "outside the timed step; algorithmic bytes = read + write of the vector once; the EIR is a 128-tap FIR from shared memory (LDS-bound, not HBM-bound)"}
+            oat.oat_eir_set(g, np.zeros(0, dtype=np.float32))
+        except Exception as ex:
+            next1 = {"error": str(ex)}
         cpu = None
         if not args.no_cpu_baseline and world == 1:       # rank 0 at N=1 only
             try:
@@ -320,7 +354,7 @@ def run_ours(args):
                 "ms_H": ms_h, "ms_HT": ms_t,
                 "samples_per_operator": int(n_samples), "samples_per_s": 2.0 * float(tot_samples.item()) / (ms_step * 1e-3),
                 "samples_per_s_H": float(tot_samples.item()) / (ms_h * 1e-3), "samples_per_s_HT": float(tot_samples.item()) / (ms_t * 1e-3),
-                "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
+                "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "next1": next1, "cpu_baseline": cpu,
                 "paper_context": "PAPER.md Table I: PLS-Int 20-137 min/iteration on a Tesla C2050 for 1,440-11,520 transducers on 210x210x440 voxels (another workload and machine)"}
         print(json.dumps(line), flush=True)
     g.close()

@@ -102,6 +102,37 @@ int oat_backproject_host(oat_geometry *geom, const float *h_y, float *h_x);
 int oat_cgls(oat_geometry *geom, const float *d_y, float *d_x, int n_iter,
              double *h_res, double *h_grad, void *cuda_stream);
 
+/* ---- Row NEXT-1: the electrical impulse response H^e, the smoothness penalty R and the
+ * penalised least-squares CG loop "PLS-Int" of the paper (Eq. 29).
+ *
+ * oat_eir_set: h_he = HOST array of `len` taps [h^e]_m = dt h^e(m dt), m = 0..len-1 (Eq. 14), copied; taps
+ * outside that range are zero (reading G20).  len = 0 removes the EIR.  Synchronises the device.
+ * oat_eir_apply: adjoint = 0: Eq. (14), d_out[q,k] = sum_kappa h^e[k-1-kappa] d_in[q,kappa];
+ *                adjoint = 1: Eq. (21), d_out[q,k] = sum_kappa h^e[kappa-1-k] d_in[q,kappa].
+ * Both buffers Q*K fp32 on the device, distinct; d_out is OVERWRITTEN; asynchronous on the stream. */
+int oat_eir_set(oat_geometry *geom, const float *h_he, int32_t len);
+int oat_eir_apply(oat_geometry *geom, const float *d_in, float *d_out, int adjoint, void *cuda_stream);
+
+/* u = H^e D G x (Eq. 11) and x = G^T D^T H^e† u (L168); without an EIR set they equal oat_project /
+ * oat_backproject.  Same buffer rules. */
+int oat_project_eir(oat_geometry *geom, const float *d_x, float *d_u, void *cuda_stream);
+int oat_backproject_eir(oat_geometry *geom, const float *d_u, float *d_x, void *cuda_stream);
+
+/* Quadratic smoothness penalty, Eq. (34) L305 (reading G21: a voxel on the low face has no neighbour "before" it
+ * and that term is omitted).  oat_penalty_apply: d_lx = L x with R(x) = x^T L x (so grad R = 2 L x); volumes
+ * nz*ny*nx fp32 on the device, distinct, d_lx OVERWRITTEN, asynchronous.  oat_penalty_value: *value = R(x) with an
+ * fp64 reduction; synchronises the stream. */
+int oat_penalty_apply(oat_geometry *geom, const float *d_x, float *d_lx, void *cuda_stream);
+int oat_penalty_value(oat_geometry *geom, const float *d_x, double *value, void *cuda_stream);
+
+/* PLS-Int (Eq. 29; reading G22): n_iter steps of linear CG on (H^T H + mu L) x = H^T u from x = 0 with
+ * H = H^e D G (the EIR set by oat_eir_set, if any); one H and one H^T per iteration (L273); fp32 vectors, fp64 dot
+ * products.  d_u: Q*K (read), d_x: nz*ny*nx (OVERWRITTEN with the iterate after n_iter steps), mu >= 0.
+ * h_obj / h_grad: HOST arrays of n_iter+1 doubles (may be NULL) receiving ||u - H x_i||^2 + mu R(x_i) and
+ * ||H^T u - (H^T H + mu L) x_i|| for i = 0..n_iter.  Synchronises the stream every iteration. */
+int oat_pls_cg(oat_geometry *geom, const float *d_u, float *d_x, int n_iter, double mu,
+               double *h_obj, double *h_grad, void *cuda_stream);
+
 /* Kernel-variant selection for measurements ("chosen by ncu", north_star).  key = "project" or
  * "backproject"; the meaning of `variant` is listed in DESIGN.md §5.  Unknown => OAT_ERR_INVALID. */
 int oat_set_variant(oat_geometry *geom, const char *key, int variant);

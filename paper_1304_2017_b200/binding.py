@@ -19,6 +19,7 @@ EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
+    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg",
     "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_last_error", "oat_version",
 ]
 
@@ -83,6 +84,16 @@ def load():
     lib.oat_measure_red_rate.restype = ctypes.c_int
     lib.oat_measure_gather_rate.argtypes = [ctypes.c_int, dp]
     lib.oat_measure_gather_rate.restype = ctypes.c_int
+    lib.oat_eir_set.argtypes = [vp, fp, ctypes.c_int32]
+    lib.oat_eir_apply.argtypes = [vp, fp, fp, ctypes.c_int, vp]
+    lib.oat_project_eir.argtypes = [vp, fp, fp, vp]
+    lib.oat_backproject_eir.argtypes = [vp, fp, fp, vp]
+    lib.oat_penalty_apply.argtypes = [vp, fp, fp, vp]
+    lib.oat_penalty_value.argtypes = [vp, fp, dp, vp]
+    lib.oat_pls_cg.argtypes = [vp, fp, fp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
+    for n in ("oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply",
+              "oat_penalty_value", "oat_pls_cg"):
+        getattr(lib, n).restype = ctypes.c_int
     _lib = lib
     return lib
 
@@ -270,3 +281,62 @@ def oat_measure_gather_rate(device: int = 0) -> float:
     v = ctypes.c_double(0.0)
     _check(load().oat_measure_gather_rate(int(device), ctypes.byref(v)))
     return float(v.value)
+
+
+# ---------------------------------------------------------------- row NEXT-1: EIR, penalty, PLS-CG
+def oat_eir_set(g, he):
+    """Set (or, with an empty array, remove) the EIR taps [h^e]_m, m = 0..len-1 (Eq. 14)."""
+    he = np.ascontiguousarray(np.asarray(he, dtype=np.float32).ravel())
+    _check(load().oat_eir_set(g.handle, ctypes.c_void_p(he.ctypes.data if he.size else None), ctypes.c_int32(he.size)))
+
+
+def oat_eir_apply(g, p, out=None, adjoint=False, stream=None):
+    import torch
+    if out is None:
+        out = torch.empty((g.n_trans, g.nt), dtype=torch.float32, device=p.device)
+    _check(load().oat_eir_apply(g.handle, _dev_ptr(p, oat_num_samples(g), "in", g), _dev_ptr(out, oat_num_samples(g), "out", g),
+                                ctypes.c_int(1 if adjoint else 0), _stream(stream)))
+    return out
+
+
+def oat_project_eir(g, x, u=None, stream=None):
+    import torch
+    if u is None:
+        u = torch.empty((g.n_trans, g.nt), dtype=torch.float32, device=x.device)
+    _check(load().oat_project_eir(g.handle, _dev_ptr(x, oat_num_voxels(g), "x", g), _dev_ptr(u, oat_num_samples(g), "u", g), _stream(stream)))
+    return u
+
+
+def oat_backproject_eir(g, u, x=None, stream=None):
+    import torch
+    if x is None:
+        x = torch.empty(g.shape, dtype=torch.float32, device=u.device)
+    _check(load().oat_backproject_eir(g.handle, _dev_ptr(u, oat_num_samples(g), "u", g), _dev_ptr(x, oat_num_voxels(g), "x", g), _stream(stream)))
+    return x
+
+
+def oat_penalty_apply(g, x, lx=None, stream=None):
+    import torch
+    if lx is None:
+        lx = torch.empty(g.shape, dtype=torch.float32, device=x.device)
+    _check(load().oat_penalty_apply(g.handle, _dev_ptr(x, oat_num_voxels(g), "x", g), _dev_ptr(lx, oat_num_voxels(g), "lx", g), _stream(stream)))
+    return lx
+
+
+def oat_penalty_value(g, x, stream=None) -> float:
+    v = ctypes.c_double(0.0)
+    _check(load().oat_penalty_value(g.handle, _dev_ptr(x, oat_num_voxels(g), "x", g), ctypes.byref(v), _stream(stream)))
+    return float(v.value)
+
+
+def oat_pls_cg(g, u, n_iter, mu, x=None, stream=None):
+    """n_iter CG steps on (H^T H + mu L) x = H^T u from x = 0; returns (x, obj, grad), curves of length n_iter+1."""
+    import torch
+    if x is None:
+        x = torch.empty(g.shape, dtype=torch.float32, device=u.device)
+    obj = np.zeros(n_iter + 1, dtype=np.float64)
+    grad = np.zeros(n_iter + 1, dtype=np.float64)
+    dp = ctypes.POINTER(ctypes.c_double)
+    _check(load().oat_pls_cg(g.handle, _dev_ptr(u, oat_num_samples(g), "u", g), _dev_ptr(x, oat_num_voxels(g), "x", g),
+                             int(n_iter), ctypes.c_double(float(mu)), obj.ctypes.data_as(dp), grad.ctypes.data_as(dp), _stream(stream)))
+    return x, obj, grad

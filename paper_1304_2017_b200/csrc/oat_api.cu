@@ -69,6 +69,9 @@ struct oat_geometry {
     double *d_g = nullptr;                    // Q*K SRT accumulator
     float *d_y2 = nullptr, *d_x2 = nullptr;   // adjoint check / CGLS / host entry points (lazy)
     float *d_x3 = nullptr, *d_y3 = nullptr, *d_x4 = nullptr;   // CGLS vectors (lazy)
+    float *d_y4 = nullptr;                    // EIR scratch (row NEXT-1, lazy)
+    float *d_he = nullptr;                    // EIR taps [h^e]_m, m = 0..n_he-1 (Eq. 14), NULL = no EIR
+    int n_he = 0;
     double *d_scal = nullptr;                 // a few fp64 scalars (dots)
     unsigned long long *d_counter = nullptr;
     double *h_scal = nullptr;                 // pinned mirror of d_scal
@@ -91,6 +94,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
+    cudaFree(g->d_y4); cudaFree(g->d_he);
     cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
@@ -508,6 +512,24 @@ int dot_sync(oat_geometry *G, const float *a, const float *b, size_t n, double *
     return OAT_OK;
 }
 
+// H = H^e D G (Eq. 11) and H^T = G^T D^T H^e† (L168); without taps the EIR is left out
+int project_full(oat_geometry *G, const float *d_x, float *d_u, cudaStream_t st)
+{
+    if (!G->d_he) return project_impl(G, d_x, d_u, st);
+    int rc = ensure(&G->d_y4, G->n_dat); if (rc) return rc;
+    if ((rc = project_impl(G, d_x, G->d_y4, st))) return rc;
+    CUDA_TRY(oat_launch_eir(0, G->d_y4, d_u, G->d_he, G->n_he, G->dev.Q, G->dev.K, st));
+    return OAT_OK;
+}
+
+int backproject_full(oat_geometry *G, const float *d_u, float *d_x, cudaStream_t st)
+{
+    if (!G->d_he) return backproject_impl(G, d_u, d_x, st);
+    int rc = ensure(&G->d_y4, G->n_dat); if (rc) return rc;
+    CUDA_TRY(oat_launch_eir(1, d_u, G->d_y4, G->d_he, G->n_he, G->dev.Q, G->dev.K, st));
+    return backproject_impl(G, G->d_y4, d_x, st);
+}
+
 int check_handle(const oat_geometry *g)
 {
     if (!g) return fail(OAT_ERR_INVALID, "geometry handle is NULL");
@@ -688,6 +710,121 @@ int oat_cgls(oat_geometry *g, const float *d_y, float *d_x, int n_iter, double *
         }
         if (h_grad) h_grad[it + 1] = sqrt(gamma);
     }
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return OAT_OK;
+}
+
+int oat_eir_set(oat_geometry *g, const float *h_he, int32_t len)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (len < 0 || (len > 0 && !h_he)) return fail(OAT_ERR_INVALID, "bad EIR taps");
+    if (len > 16384) return fail(OAT_ERR_INVALID, "EIR longer than 16384 taps");
+    for (int i = 0; i < len; ++i) if (!isfinite(h_he[i])) return fail(OAT_ERR_INVALID, "EIR tap %d is not finite", i);
+    CUDA_TRY(cudaDeviceSynchronize());                    // the old taps may still be in use
+    cudaFree(g->d_he); g->d_he = nullptr; g->n_he = 0;
+    if (len == 0) return OAT_OK;
+    CUDA_TRY(cudaMalloc((void **)&g->d_he, sizeof(float) * (size_t)len));
+    CUDA_TRY(cudaMemcpy(g->d_he, h_he, sizeof(float) * (size_t)len, cudaMemcpyHostToDevice));
+    g->n_he = len;
+    return OAT_OK;
+}
+
+int oat_eir_apply(oat_geometry *g, const float *d_in, float *d_out, int adjoint, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if ((!d_in || !d_out) && g->n_dat) return fail(OAT_ERR_INVALID, "d_in / d_out must not be NULL");
+    if (d_in == d_out && g->n_dat) return fail(OAT_ERR_INVALID, "oat_eir_apply cannot run in place");
+    if (!g->d_he) return fail(OAT_ERR_INVALID, "no EIR set (oat_eir_set)");
+    CUDA_TRY(oat_launch_eir(adjoint ? 1 : 0, d_in, d_out, g->d_he, g->n_he, g->dev.Q, g->dev.K, (cudaStream_t)stream));
+    return OAT_OK;
+}
+
+int oat_penalty_apply(oat_geometry *g, const float *d_x, float *d_lx, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_x || !d_lx || d_x == d_lx) return fail(OAT_ERR_INVALID, "d_x / d_lx must be distinct non-NULL buffers");
+    oat_launch_penalty(g->dev, d_x, d_lx, 1.f, 0.f, (cudaStream_t)stream);
+    CUDA_TRY(cudaGetLastError());
+    return OAT_OK;
+}
+
+int oat_penalty_value(oat_geometry *g, const float *d_x, double *value, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_x || !value) return fail(OAT_ERR_INVALID, "NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = ensure(&g->d_x2, g->n_vox))) return rc;
+    oat_launch_penalty(g->dev, d_x, g->d_x2, 1.f, 0.f, st);
+    return dot_sync(g, d_x, g->d_x2, g->n_vox, value, st);   // R(x) = x^T L x
+}
+
+int oat_project_eir(oat_geometry *g, const float *d_x, float *d_u, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_x || (!d_u && g->n_dat)) return fail(OAT_ERR_INVALID, "d_x / d_u must not be NULL");
+    return project_full(g, d_x, d_u, (cudaStream_t)stream);
+}
+
+int oat_backproject_eir(oat_geometry *g, const float *d_u, float *d_x, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_x || (!d_u && g->n_dat)) return fail(OAT_ERR_INVALID, "d_x / d_u must not be NULL");
+    return backproject_full(g, d_u, d_x, (cudaStream_t)stream);
+}
+
+// Row NEXT-1 (reading G22): linear CG on (H^T H + mu L) x = H^T u from x = 0, H = H^e D G.
+int oat_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double mu, double *h_obj, double *h_grad, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_u || !d_x || n_iter < 0 || !(mu >= 0) || !isfinite(mu)) return fail(OAT_ERR_INVALID, "bad argument to oat_pls_cg");
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = ensure(&g->d_y2, g->n_dat))) return rc;     // d = u - H x
+    if ((rc = ensure(&g->d_y3, g->n_dat))) return rc;     // q = H p
+    if ((rc = ensure(&g->d_x2, g->n_vox))) return rc;     // w = (H^T H + mu L) p, later L x
+    if ((rc = ensure(&g->d_x3, g->n_vox))) return rc;     // r
+    if ((rc = ensure(&g->d_x4, g->n_vox))) return rc;     // p
+    float *d = g->d_y2, *q = g->d_y3, *w = g->d_x2, *r = g->d_x3, *p = g->d_x4;
+    CUDA_TRY(cudaMemsetAsync(d_x, 0, sizeof(float) * g->n_vox, st));
+    CUDA_TRY(cudaMemcpyAsync(d, d_u, sizeof(float) * g->n_dat, cudaMemcpyDeviceToDevice, st));
+    if ((rc = backproject_full(g, d_u, r, st))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(p, r, sizeof(float) * g->n_vox, cudaMemcpyDeviceToDevice, st));
+    double rr, dd;
+    if ((rc = dot_sync(g, r, r, g->n_vox, &rr, st))) return rc;
+    if ((rc = dot_sync(g, d, d, g->n_dat, &dd, st))) return rc;
+    if (h_obj) h_obj[0] = dd;
+    if (h_grad) h_grad[0] = sqrt(rr);
+    for (int it = 0; it < n_iter; ++it) {
+        double pw;
+        if ((rc = project_full(g, p, q, st))) return rc;
+        if ((rc = backproject_full(g, q, w, st))) return rc;
+        if (mu > 0) oat_launch_penalty(g->dev, p, w, (float)mu, 1.f, st);          // w += mu L p
+        if ((rc = dot_sync(g, p, w, g->n_vox, &pw, st))) return rc;
+        if (!(pw > 0) || rr == 0) {
+            if (h_obj) h_obj[it + 1] = h_obj[it];
+            if (h_grad) h_grad[it + 1] = h_grad[it];
+            continue;
+        }
+        const double alpha = rr / pw;
+        oat_launch_axpy((float)alpha, p, d_x, (long long)g->n_vox, st);
+        oat_launch_axpy((float)-alpha, q, d, (long long)g->n_dat, st);
+        oat_launch_axpy((float)-alpha, w, r, (long long)g->n_vox, st);
+        double rr_new;
+        if ((rc = dot_sync(g, r, r, g->n_vox, &rr_new, st))) return rc;
+        const double beta = rr_new / rr;
+        rr = rr_new;
+        oat_launch_xpay(r, (float)beta, p, (long long)g->n_vox, st);
+        if (h_obj) {
+            double pen = 0.0;
+            if ((rc = dot_sync(g, d, d, g->n_dat, &dd, st))) return rc;
+            if (mu > 0) {
+                oat_launch_penalty(g->dev, d_x, w, 1.f, 0.f, st);
+                if ((rc = dot_sync(g, d_x, w, g->n_vox, &pen, st))) return rc;
+            }
+            h_obj[it + 1] = dd + mu * pen;
+        }
+        if (h_grad) h_grad[it + 1] = sqrt(rr);
+    }
+    CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaStreamSynchronize(st));
     return OAT_OK;
 }

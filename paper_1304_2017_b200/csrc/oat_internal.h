@@ -118,3 +118,6 @@ void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st
 void oat_launch_dot(const float *a, const float *b, long long n, double *out, cudaStream_t st);
 void oat_launch_axpy(float alpha, const float *x, float *y, long long n, cudaStream_t st);   // y += alpha x
 void oat_launch_xpay(const float *x, float beta, float *y, long long n, cudaStream_t st);    // y = x + beta y
+// row NEXT-1: EIR convolution / correlation along time (Eq. 14 / Eq. 21) and the penalty stencil (Eq. 34)
+cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float *he, int L, int Q, int K, cudaStream_t st);
+void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha, float beta, cudaStream_t st);   // out = beta out + alpha L x

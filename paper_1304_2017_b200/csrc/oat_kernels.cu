@@ -1155,6 +1155,58 @@ __global__ void oat_xpay_kernel(const float *__restrict__ x, float beta, float *
         y[i] = fmaf(beta, y[i], x[i]);
 }
 
+// Row NEXT-1, EIR operator.  ADJ = 0: Eq. (14), out[q,k] = sum_m he[m] in[q, k-1-m]; ADJ = 1: Eq. (21),
+// out[q,k] = sum_m he[m] in[q, k+1+m]; he[m] given for m = 0..L-1, `in` zero outside [0, K) (reading G20).
+// One block = one transducer row x a tile of OAT_ET outputs; the taps and the input window of the tile sit in
+// shared memory; every output is one fixed-order fp32 FMA chain over the taps (deterministic).
+#define OAT_ET 256
+template <int ADJ>
+__global__ void __launch_bounds__(OAT_ET)
+oat_eir_kernel(const float *__restrict__ in, float *__restrict__ out, const float *__restrict__ he, int L, int K)
+{
+    extern __shared__ float sm[];
+    float *s_he = sm, *s_in = sm + L;                      // window: OAT_ET + L samples
+    const int q = blockIdx.y, k0 = blockIdx.x * OAT_ET, t = threadIdx.x;
+    const float *row = in + (size_t)q * K;
+    for (int m = t; m < L; m += OAT_ET) s_he[m] = he[m];
+    // ADJ = 0: window sample j <-> k0 - L + j  (inputs k-1-m, m < L, of outputs k0..k0+ET-1: k0-L .. k0+ET-2)
+    // ADJ = 1: window sample j <-> k0 + 1 + j  (inputs k+1+m: k0+1 .. k0+ET+L-1)
+    const int base = ADJ ? k0 + 1 : k0 - L;
+    for (int j = t; j < OAT_ET + L; j += OAT_ET) {
+        const int kk = base + j;
+        s_in[j] = (kk >= 0 && kk < K) ? row[kk] : 0.f;
+    }
+    __syncthreads();
+    const int k = k0 + t;
+    if (k >= K) return;
+    float acc = 0.f;
+    if (ADJ) { for (int m = 0; m < L; ++m) acc = fmaf(s_he[m], s_in[t + m], acc); }
+    else     { for (int m = 0; m < L; ++m) acc = fmaf(s_he[m], s_in[t + L - 1 - m], acc); }
+    out[(size_t)q * K + k] = acc;
+}
+
+// Row NEXT-1, smoothness penalty (Eq. 34, reading G21): out = beta out + alpha L x with R(x) = x^T L x,
+// (L x)_n = sum over the three axes of (x_n - x_before) + (x_n - x_after), each term only if that neighbour exists.
+__global__ void oat_penalty_kernel(const OatDev P, const float *__restrict__ x, float *__restrict__ out, float alpha, float beta)
+{
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    const long long sy = P.nx, sz = (long long)P.nx * P.ny;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int ix = (int)(i % P.nx);
+        const long long r = i / P.nx;
+        const int iy = (int)(r % P.ny), iz = (int)(r / P.ny);
+        const float c = x[i];
+        float s = 0.f;
+        if (ix > 0) s += c - x[i - 1];
+        if (ix + 1 < P.nx) s += c - x[i + 1];
+        if (iy > 0) s += c - x[i - sy];
+        if (iy + 1 < P.ny) s += c - x[i + sy];
+        if (iz > 0) s += c - x[i - sz];
+        if (iz + 1 < P.nz) s += c - x[i + sz];
+        out[i] = beta == 0.f ? alpha * s : fmaf(beta, out[i], alpha * s);
+    }
+}
+
 inline int grid_for(long long n, int block)
 {
     long long g = (n + block - 1) / block;
@@ -1354,6 +1406,26 @@ void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st
 {
     const long long n = (long long)P.Q * P.K;
     if (n > 0) oat_diff_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, g, y);
+}
+
+cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float *he, int L, int Q, int K, cudaStream_t st)
+{
+    if (Q <= 0 || K <= 0) return cudaSuccess;
+    const size_t smem = sizeof(float) * (size_t)(OAT_ET + 2 * L);
+    if (smem > 200 * 1024) return cudaErrorInvalidValue;
+    cudaError_t e = cudaFuncSetAttribute(oat_eir_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(oat_eir_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const dim3 grid((unsigned)((K + OAT_ET - 1) / OAT_ET), (unsigned)Q);
+    if (adjoint) oat_eir_kernel<1><<<grid, OAT_ET, smem, st>>>(in, out, he, L, K);
+    else oat_eir_kernel<0><<<grid, OAT_ET, smem, st>>>(in, out, he, L, K);
+    return cudaGetLastError();
+}
+
+void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha, float beta, cudaStream_t st)
+{
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    if (n > 0) oat_penalty_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, out, alpha, beta);
 }
 
 void oat_launch_dot(const float *a, const float *b, long long n, double *out, cudaStream_t st)
