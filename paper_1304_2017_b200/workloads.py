@@ -111,6 +111,29 @@ def arc_array(n_elem: int, n_views: int, radius: float,
     return np.ascontiguousarray(xyz.reshape(-1, 3))
 
 
+def patch_areas_equal(trans_xyz: np.ndarray, centre) -> np.ndarray:
+    """Patch area dS_q of an (almost) uniform sampling of a full sphere, e.g. the Fibonacci layout: 4 pi R_q^2 / Q."""
+    r = np.linalg.norm(np.asarray(trans_xyz, dtype=np.float64) - np.asarray(centre, dtype=np.float64), axis=1)
+    return 4.0 * math.pi * r * r / max(1, len(r))
+
+
+def patch_areas_arc(n_elem: int, n_views: int, radius: float, polar0_deg: float = 14.0, span_deg: float = 152.0) -> np.ndarray:
+    """Patch area of the ring/view layout of `arc_array` (L203, L211): (R^s)^2 dtheta dphi sin(theta_q), q = e * n_views + v."""
+    e = np.arange(n_elem, dtype=np.float64)
+    pol = np.deg2rad(polar0_deg + e * span_deg / max(1, n_elem - 1))
+    dth = np.deg2rad(span_deg / max(1, n_elem - 1))
+    dph = 2.0 * math.pi / n_views
+    return np.repeat(radius * radius * dth * dph * np.sin(pol), n_views)
+
+
+def fbp_weights(w: "Workload", areas: np.ndarray) -> np.ndarray:
+    """Input vector of row NEXT-2 (reading G23): w_q = -dS_q / (4 pi^2 kappa c^3 dt R_q), the constant of Eq. (27)
+    with kappa = beta / (4 pi C_p) and R_q the transducer's distance from the grid centre.  Handed to the oracle and
+    to the library alike (an INPUT of the operator, like the transducer positions)."""
+    r = np.linalg.norm(np.asarray(w.trans_xyz, dtype=np.float64) - w.centre, axis=1)
+    return -np.asarray(areas, dtype=np.float64) / (4.0 * math.pi ** 2 * w.gain * w.c ** 3 * w.dt * r)
+
+
 def default_t0(trans_xyz: np.ndarray, n: int, spacing: float, c: float, dt: float) -> float:
     """t0 = dt * max(1, floor((min_q |r_q - C| - R_pad)/(c dt)) - 1) with
     R_pad = sqrt(3) * ((N-1) spacing / 2 + spacing); grid centred at the origin."""
