@@ -330,6 +330,22 @@ def run_ours(args):
             oat.oat_eir_set(g, np.zeros(0, dtype=np.float32))
         except Exception as ex:
             next1 = {"error": str(ex)}
+        # ---- row NEXT-2 (FBP, Eq. 27): one image from the data of this config, voxel driven
+        next2 = None
+        try:
+            from paper_1304_2017_b200 import workloads as wl2
+            wb2, _ = workload(args)
+            areas = wl2.patch_areas_arc(64, 144, 65.0) if (args.config == 3 and not args.subset) else wl2.patch_areas_equal(wb2.trans_xyz, wb2.centre)
+            wq = torch.from_numpy(wl2.fbp_weights(wb2, areas).astype(np.float32)).cuda()
+            oat.oat_fbp(g, y, wq, xb); torch.cuda.synchronize()
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record(stream); oat.oat_fbp(g, y, wq, xb); b.record(stream); torch.cuda.synchronize()
+            ms_f = a.elapsed_time(b)
+            pairs = float(x.numel()) * w.n_trans
+            next2 = {"ms_fbp": ms_f, "voxel_transducer_pairs": pairs, "pairs_per_s": pairs / (ms_f * 1e-3),
+                     "note": "outside the timed step; fp64 distance + interval decision, fp32 brackets and sum (DESIGN.md section 5.6)"}
+        except Exception as ex:
+            next2 = {"error": str(ex)}
         cpu = None
         if not args.no_cpu_baseline and world == 1:       # rank 0 at N=1 only
             try:
@@ -354,7 +370,7 @@ def run_ours(args):
                 "ms_H": ms_h, "ms_HT": ms_t,
                 "samples_per_operator": int(n_samples), "samples_per_s": 2.0 * float(tot_samples.item()) / (ms_step * 1e-3),
                 "samples_per_s_H": float(tot_samples.item()) / (ms_h * 1e-3), "samples_per_s_HT": float(tot_samples.item()) / (ms_t * 1e-3),
-                "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "next1": next1, "cpu_baseline": cpu,
+                "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "next1": next1, "next2": next2, "cpu_baseline": cpu,
                 "paper_context": "PAPER.md Table I: PLS-Int 20-137 min/iteration on a Tesla C2050 for 1,440-11,520 transducers on 210x210x440 voxels (another workload and machine)"}
         print(json.dumps(line), flush=True)
     g.close()

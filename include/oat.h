@@ -133,6 +133,15 @@ int oat_penalty_value(oat_geometry *geom, const float *d_x, double *value, void 
 int oat_pls_cg(oat_geometry *geom, const float *d_u, float *d_x, int n_iter, double mu,
                double *h_obj, double *h_grad, void *cuda_stream);
 
+/* ---- Row NEXT-2: filtered backprojection, the discretised FBP formula Eq. (27) L221 (Eq. 4 L69 with Eq. 25-26),
+ * voxel driven (Alg. 2), with one weight per transducer (reading G23):
+ *   x[n] = sum_q w[q] { (1.5 - (k+tau)/(k~+tau)) p[q,k+1] + ((k+1+tau)/(k~+tau) - 1.5) p[q,k] },
+ *   k~ = (|r_q - r_n|/c - t0)/dt, k = floor(k~), tau = t0/dt; pairs with k < 0 or k+1 > K-1 contribute nothing.
+ * For the paper's ring/view geometry w[q] = -C_p R^s dtheta dphi sin(theta_q) / (pi beta c^3 dt).
+ * d_p: Q*K fp32 pressure data (read), d_w: Q fp32 weights (read), d_x: nz*ny*nx fp32 (OVERWRITTEN); device
+ * pointers owned by the caller; asynchronous on the stream. */
+int oat_fbp(oat_geometry *geom, const float *d_p, const float *d_w, float *d_x, void *cuda_stream);
+
 /* Kernel-variant selection for measurements ("chosen by ncu", north_star).  key = "project" or
  * "backproject"; the meaning of `variant` is listed in DESIGN.md §5.  Unknown => OAT_ERR_INVALID. */
 int oat_set_variant(oat_geometry *geom, const char *key, int variant);

@@ -62,3 +62,17 @@ def fbp(w, p, weights):
     """Eq. (27) on every node of the grid: returns (nz, ny, nx)."""
     pts = node_positions(w).reshape(-1, 3)
     return fbp_points(w, p, weights, pts).reshape(w.nz, w.ny, w.nx)
+
+
+def interval_margin(w, pts):
+    """min over transducers of |k~ - nearest integer| at each point (M,): where it is below the rounding noise of k~
+    (~1e-12) the choice of interval k = floor(k~) is a tie -- Eq. (27) is discontinuous across integer k~, both
+    neighbouring intervals are correct results -- and a parity test compares only the points where it is not."""
+    pts = np.asarray(pts, dtype=np.float64)
+    tr = np.asarray(w.trans_xyz, dtype=np.float64)
+    m = np.full(pts.shape[0], np.inf)
+    for q in range(tr.shape[0]):
+        kt = (np.sqrt(np.sum((pts - tr[q]) ** 2, axis=1)) / w.c - w.t0) / w.dt
+        inrec = (kt > -1.0) & (kt < w.nt)
+        m = np.minimum(m, np.where(inrec, np.abs(kt - np.rint(kt)), np.inf))
+    return m

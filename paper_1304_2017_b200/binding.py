@@ -19,7 +19,7 @@ EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
-    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg",
+    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp",
     "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_last_error", "oat_version",
 ]
 
@@ -91,6 +91,8 @@ def load():
     lib.oat_penalty_apply.argtypes = [vp, fp, fp, vp]
     lib.oat_penalty_value.argtypes = [vp, fp, dp, vp]
     lib.oat_pls_cg.argtypes = [vp, fp, fp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
+    lib.oat_fbp.argtypes = [vp, fp, fp, fp, vp]
+    lib.oat_fbp.restype = ctypes.c_int
     for n in ("oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply",
               "oat_penalty_value", "oat_pls_cg"):
         getattr(lib, n).restype = ctypes.c_int
@@ -340,3 +342,14 @@ def oat_pls_cg(g, u, n_iter, mu, x=None, stream=None):
     _check(load().oat_pls_cg(g.handle, _dev_ptr(u, oat_num_samples(g), "u", g), _dev_ptr(x, oat_num_voxels(g), "x", g),
                              int(n_iter), ctypes.c_double(float(mu)), obj.ctypes.data_as(dp), grad.ctypes.data_as(dp), _stream(stream)))
     return x, obj, grad
+
+
+# ---------------------------------------------------------------- row NEXT-2: filtered backprojection
+def oat_fbp(g, p, weights, x=None, stream=None):
+    """x = FBP(p) by Eq. (27) with one weight per transducer (device tensors; weights: Q float32)."""
+    import torch
+    if x is None:
+        x = torch.empty(g.shape, dtype=torch.float32, device=p.device)
+    _check(load().oat_fbp(g.handle, _dev_ptr(p, oat_num_samples(g), "p", g), _dev_ptr(weights, g.n_trans, "weights", g),
+                          _dev_ptr(x, oat_num_voxels(g), "x", g), _stream(stream)))
+    return x

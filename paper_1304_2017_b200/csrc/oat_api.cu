@@ -829,6 +829,16 @@ int oat_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double
     return OAT_OK;
 }
 
+int oat_fbp(oat_geometry *g, const float *d_p, const float *d_w, float *d_x, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_x || ((!d_p || !d_w) && g->n_dat)) return fail(OAT_ERR_INVALID, "d_p / d_w / d_x must not be NULL");
+    if (g->dev.K < 2) { CUDA_TRY(cudaMemsetAsync(d_x, 0, sizeof(float) * g->n_vox, (cudaStream_t)stream)); return OAT_OK; }
+    oat_launch_fbp(g->dev, d_p, d_w, d_x, (cudaStream_t)stream);
+    CUDA_TRY(cudaGetLastError());
+    return OAT_OK;
+}
+
 int oat_set_variant(oat_geometry *g, const char *key, int variant)
 {
     if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");

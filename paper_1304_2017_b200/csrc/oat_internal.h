@@ -121,3 +121,5 @@ void oat_launch_xpay(const float *x, float beta, float *y, long long n, cudaStre
 // row NEXT-1: EIR convolution / correlation along time (Eq. 14 / Eq. 21) and the penalty stencil (Eq. 34)
 cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float *he, int L, int Q, int K, cudaStream_t st);
 void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha, float beta, cudaStream_t st);   // out = beta out + alpha L x
+// row NEXT-2: filtered backprojection, Eq. (27), x[n] = sum_q wq[q] {...} (voxel driven)
+void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, cudaStream_t st);

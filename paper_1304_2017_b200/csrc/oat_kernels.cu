@@ -1207,6 +1207,57 @@ __global__ void oat_penalty_kernel(const OatDev P, const float *__restrict__ x, 
     }
 }
 
+// Row NEXT-2, filtered backprojection (Eq. 27 L221 with one weight per transducer, readings G23-G25): voxel driven,
+// one thread per node of an 8 x 8 x 4 tile, transducers staged through shared memory 256 at a time.  The sample index
+// k = floor(k~), k~ = |r_q - r_n| / (c dt) - t_min/dt, is an integer decision and is taken in fp64 like the oracle's
+// (the discretisation is discontinuous across integer k~: an fp32 distance, 1e-4 samples off at k~ ~ 2000, would move
+// ~1e-4 of all pairs into the neighbouring interval); the two brackets, the interpolation and the sum are fp32, with
+// an fp64 total over the chunks of 256 transducers.
+#define OAT_FQ 256
+__global__ void __launch_bounds__(256)
+oat_fbp_kernel(const OatDev P, const float *__restrict__ p, const float *__restrict__ wq, float *__restrict__ x)
+{
+    __shared__ double s_t[OAT_FQ][3];
+    __shared__ float s_w[OAT_FQ];
+    const int tid = threadIdx.x;
+    const int ix = blockIdx.x * 8 + (tid & 7), iy = blockIdx.y * 8 + ((tid >> 3) & 7), iz = blockIdx.z * 4 + (tid >> 6);
+    const bool inside = ix < P.nx && iy < P.ny && iz < P.nz;
+    const double vx = (double)ix, vy = (double)iy, vz = (double)iz;   // node coordinates; transducers in the same units
+    const double inv_step = 1.0 / P.step, tau = P.t0 / P.dt;
+    const float tauf = (float)tau;
+    double total = 0.0;
+    for (int q0 = 0; q0 < P.Q; q0 += OAT_FQ) {
+        const int nq = min(OAT_FQ, P.Q - q0);
+        __syncthreads();
+        if (tid < nq) {
+            const double *f = P.frame + (size_t)(q0 + tid) * 12;
+            s_t[tid][0] = f[9] - 1.0; s_t[tid][1] = f[10] - 1.0; s_t[tid][2] = f[11] - 1.0;   // frames hold padded coordinates
+            s_w[tid] = wq[q0 + tid];
+        }
+        __syncthreads();
+        if (!inside) continue;
+        float acc = 0.f;
+#pragma unroll 2
+        for (int j = 0; j < nq; ++j) {
+            const double dx = vx - s_t[j][0], dy = vy - s_t[j][1], dz = vz - s_t[j][2];
+            const double d = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
+            const double den = d * inv_step;               // k~ + tau = |r_q - r_n| / (c dt)
+            const double kt = den - tau;
+            const double kf = floor(kt);
+            const int k = (int)kf;
+            const bool ok = ((unsigned)k < (unsigned)(P.K - 1)) && den > 0.0;     // k >= 0, k+1 <= K-1 (reading G25)
+            const float ktau = (float)kf + tauf;           // k + tau
+            const float rden = __fdividef(1.f, (float)den);
+            const float a1 = fmaf(-ktau, rden, 1.5f), a0 = fmaf(ktau + 1.f, rden, -1.5f);
+            const float *row = p + (size_t)(q0 + j) * P.K;
+            const float p0 = ok ? __ldg(row + k) : 0.f, p1 = ok ? __ldg(row + k + 1) : 0.f;
+            acc = fmaf(s_w[j], fmaf(a1, p1, a0 * p0), acc);
+        }
+        total += (double)acc;
+    }
+    if (inside) x[((size_t)iz * P.ny + iy) * P.nx + ix] = (float)total;
+}
+
 inline int grid_for(long long n, int block)
 {
     long long g = (n + block - 1) / block;
@@ -1420,6 +1471,12 @@ cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float
     if (adjoint) oat_eir_kernel<1><<<grid, OAT_ET, smem, st>>>(in, out, he, L, K);
     else oat_eir_kernel<0><<<grid, OAT_ET, smem, st>>>(in, out, he, L, K);
     return cudaGetLastError();
+}
+
+void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, cudaStream_t st)
+{
+    const dim3 grid((unsigned)((P.nx + 7) / 8), (unsigned)((P.ny + 7) / 8), (unsigned)((P.nz + 3) / 4));
+    oat_fbp_kernel<<<grid, 256, 0, st>>>(P, p, wq, x);
 }
 
 void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha, float beta, cudaStream_t st)
