@@ -1,0 +1,77 @@
+"""Pins of the NEXT-3 oracle (oracle/oat_sph.py: spherical-voxel model H_sph, Eq. 17-19, and its adjoint, Eq. 24)
+against things other than itself: the time-domain N-wave of a uniform sphere (closed form from Eq. 2-3) recovered by
+an inverse Fourier sum, the small-f series of Eq. (19), and the adjoint identity.  CPU only."""
+import math
+
+import numpy as np
+
+from oracle import oat_sph as sph
+from paper_1304_2017_b200 import workloads as wl
+
+
+def problem(n=3, ds=0.5, q=3, rs=20.0, kappa=1.0):
+    tr = wl.fibonacci_sphere(max(q, 2), rs)[:q] + np.array([0.3, -0.2, 0.1])
+    o = -(n - 1) * ds / 2.0
+    return wl.Workload("sph-pin", n, n, n, ds, (o, o, o), tr, c=1.5, t0=0.0, dt=0.05, nt=8, surf_step=ds, kband=8, gain=kappa)
+
+
+def test_single_voxel_is_the_n_wave_of_a_uniform_sphere():
+    """One spherical voxel of radius ds/2 and unit amplitude: the inverse Fourier sum of Eq. (17) over a dense frequency
+    grid must give p(t) = kappa (-2 pi c^2 (ct - d)/d) for |ct - d| < ds/2 and 0 outside (Eq. 2-3 L59-63 for a ball; pin
+    P6 of the interpolation model).  Pins Eq. (19) -- sign, the factor 4 pi kappa = beta/C_p, cos/sin terms -- and the
+    Green's function exp(-j 2 pi f d/c)/(2 pi d) of Eq. (18)."""
+    w = problem(kappa=1.7)
+    x = np.zeros((w.nz, w.ny, w.nx)); x[1, 2, 0] = 1.0
+    node = np.asarray(w.origin) + w.spacing * np.array([0, 2, 1])
+    df, nf = 0.02, 10000                                  # 0 .. 200 MHz, period 50 us > d/c + a/c
+    f = sph.freqs(0.0, df, nf)
+    u = sph.project(w, x, 0.0, df, nf)
+    a = w.spacing / 2.0
+    taper = 0.5 * (1.0 + np.cos(np.pi * f / f[-1]))       # smooths p(t) over ~0.01 us; a linear ramp is unchanged by it
+    for q in range(w.n_trans):
+        d = np.linalg.norm(w.trans_xyz[q] - node)
+        s = np.array([-0.6, -0.3, 0.0, 0.25, 0.55]) * a    # ct - d, inside the N-wave
+        t = (d + s) / w.c
+        pt = 2.0 * df * np.real(np.exp(2j * np.pi * np.outer(t, f)) @ (u[q] * taper))   # real signal, P(0) = 0
+        exact = w.gain * (-2.0 * math.pi * w.c ** 2 * s / d)
+        assert np.allclose(pt, exact, rtol=2e-3, atol=2e-3 * abs(exact).max()), (q, pt, exact)
+        t_out = (d + np.array([-2.5, 1.8, 4.0]) * a) / w.c
+        p_out = 2.0 * df * np.real(np.exp(2j * np.pi * np.outer(t_out, f)) @ (u[q] * taper))
+        assert np.all(np.abs(p_out) < 5e-3 * abs(exact).max())
+
+
+def test_p0_small_frequency_series_and_dc():
+    """Eq. (19) near f = 0: bracket = (x cos x - sin x)/omega ~ -omega^2 T^3/3, T = ds/2c  =>  p~0 ~ +j (16 pi^3/3) kappa c^3 T^3 f."""
+    w = problem(kappa=0.8)
+    T = w.spacing / (2.0 * w.c)
+    f = np.array([0.0, 1e-3, 2e-3])
+    p0 = sph.p0_tilde(w, f)
+    assert p0[0] == 0.0
+    lead = 1j * (16.0 * math.pi ** 3 / 3.0) * w.gain * w.c ** 3 * T ** 3 * f[1:]
+    assert np.allclose(p0[1:], lead, rtol=1e-4)
+    assert np.all(np.abs(p0.real) < 1e-12 * np.abs(p0.imag).max())          # purely imaginary without an EIR
+    he = np.array([1.0, 2.0 - 1.0j, 0.5j])
+    assert np.allclose(sph.p0_tilde(w, f, he), p0 * he)
+
+
+def test_adjoint_identity_and_linearity():
+    w = problem(n=4, q=5)
+    rng = np.random.default_rng(0)
+    f0, df, nf = 0.3, 0.17, 23
+    x = rng.standard_normal((w.nz, w.ny, w.nx))
+    u = rng.standard_normal((w.n_trans, nf)) + 1j * rng.standard_normal((w.n_trans, nf))
+    he = rng.standard_normal(nf) + 1j * rng.standard_normal(nf)
+    hx = sph.project(w, x, f0, df, nf, he)
+    htu = sph.backproject(w, u, f0, df, nf, he)
+    lhs = np.real(np.vdot(u, hx))                          # Re <u, Hx> = Re sum conj(u) Hx
+    rhs = np.vdot(x, htu)
+    assert abs(lhs - rhs) <= 1e-12 * max(abs(lhs), abs(rhs))
+    x2 = rng.standard_normal(x.shape)
+    assert np.allclose(sph.project(w, 2 * x - 3 * x2, f0, df, nf, he), 2 * hx - 3 * sph.project(w, x2, f0, df, nf, he), rtol=1e-12, atol=1e-14)
+    # dense matrix column: one voxel, one transducer, written out from Eq. (17)-(18)
+    e = np.zeros_like(x); e[2, 1, 3] = 1.0
+    node = np.asarray(w.origin) + w.spacing * np.array([3, 1, 2])
+    d = np.linalg.norm(w.trans_xyz[4] - node)
+    fl = f0 + df * 7
+    col = sph.project(w, e, f0, df, nf, he)[4, 7]
+    assert np.allclose(col, sph.p0_tilde(w, np.array([fl]))[0] * he[7] * np.exp(-2j * np.pi * fl * d / w.c) / (2 * np.pi * d), rtol=1e-12)
