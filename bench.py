@@ -346,6 +346,28 @@ def run_ours(args):
                      "note": "outside the timed step; fp64 distance + interval decision, fp32 brackets and sum (DESIGN.md section 5.6)"}
         except Exception as ex:
             next2 = {"error": str(ex)}
+        # ---- row NEXT-3 (spherical-voxel model, frequency domain): this config's grid, 256 seeded transducers, 64 frequencies
+        next3 = None
+        try:
+            wb3, _ = workload(args)
+            _, ws3 = wb3.seeded_subset(256)
+            g3 = oat.oat_geometry_create(ws3, local)
+            nf3 = 64
+            oat.oat_sph_set(g3, nf3, 0.0, 0.078125)          # 0 .. 4.9 MHz
+            u3 = torch.empty((ws3.n_trans, nf3), dtype=torch.complex64, device="cuda")
+            oat.oat_sph_project(g3, x, u3); oat.oat_sph_backproject(g3, u3, xb); torch.cuda.synchronize()
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            ev[0].record(stream); oat.oat_sph_project(g3, x, u3); ev[1].record(stream); oat.oat_sph_backproject(g3, u3, xb); ev[2].record(stream)
+            torch.cuda.synchronize()
+            terms = float(x.numel()) * ws3.n_trans * nf3
+            nnz = float(torch.count_nonzero(x).item())
+            next3 = {"n_trans": ws3.n_trans, "n_freq": nf3, "ms_project": ev[0].elapsed_time(ev[1]), "ms_backproject": ev[1].elapsed_time(ev[2]),
+                     "voxel_transducer_frequency_terms": terms, "terms_per_s_backproject": terms / (ev[1].elapsed_time(ev[2]) * 1e-3),
+                     "nonzero_voxel_fraction": nnz / x.numel(),
+                     "note": "outside the timed step; the projection skips all-zero voxels (sparse vessel phantom), the backprojection visits every term"}
+            g3.close()
+        except Exception as ex:
+            next3 = {"error": str(ex)}
         cpu = None
         if not args.no_cpu_baseline and world == 1:       # rank 0 at N=1 only
             try:
@@ -370,7 +392,7 @@ def run_ours(args):
                 "ms_H": ms_h, "ms_HT": ms_t,
                 "samples_per_operator": int(n_samples), "samples_per_s": 2.0 * float(tot_samples.item()) / (ms_step * 1e-3),
                 "samples_per_s_H": float(tot_samples.item()) / (ms_h * 1e-3), "samples_per_s_HT": float(tot_samples.item()) / (ms_t * 1e-3),
-                "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "next1": next1, "next2": next2, "cpu_baseline": cpu,
+                "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "next1": next1, "next2": next2, "next3": next3, "cpu_baseline": cpu,
                 "paper_context": "PAPER.md Table I: PLS-Int 20-137 min/iteration on a Tesla C2050 for 1,440-11,520 transducers on 210x210x440 voxels (another workload and machine)"}
         print(json.dumps(line), flush=True)
     g.close()

@@ -142,6 +142,20 @@ int oat_pls_cg(oat_geometry *geom, const float *d_u, float *d_x, int n_iter, dou
  * pointers owned by the caller; asynchronous on the stream. */
 int oat_fbp(oat_geometry *geom, const float *d_p, const float *d_w, float *d_x, void *cuda_stream);
 
+/* ---- Row NEXT-3: the spherical-voxel imaging model in the temporal frequency domain and its adjoint (Eq. 17-20
+ * L137-161, Eq. 24; Algs. 7-12), for point-like transducers (Alg. 9 line 7; reading G28).
+ * oat_sph_set: frequencies f_l = f0 + l df (MHz), l = 0..nf-1 (reading G27); h_he = HOST array of 2*nf floats, the EIR
+ * spectrum h~e(f_l) as (re, im) pairs, or NULL for h~e = 1; p~0(f_l) of Eq. (19) is precomputed (p~0(0) = 0).  nf = 0
+ * removes the grid.  Synchronises the device.
+ * oat_sph_project:     u[q,l] = p~0(f_l) sum_n x_n exp(-j 2 pi f_l d_qn/c) / (2 pi d_qn)          (Eq. 17-18)
+ * oat_sph_backproject: x_n = Re sum_q sum_l u[q,l] conj(p~0(f_l)) exp(+j 2 pi f_l d_qn/c) / (2 pi d_qn)   (Eq. 24; real part:
+ *                      reading G29, so that Re<Hx,u> = <x,H†u>)
+ * d_x: nz*ny*nx fp32; d_u: Q*nf complex as interleaved (re, im) fp32 pairs, index q*nf + l; device pointers owned by the
+ * caller; the output is OVERWRITTEN; asynchronous on the stream. */
+int oat_sph_set(oat_geometry *geom, int32_t nf, double f0, double df, const float *h_he);
+int oat_sph_project(oat_geometry *geom, const float *d_x, float *d_u, void *cuda_stream);
+int oat_sph_backproject(oat_geometry *geom, const float *d_u, float *d_x, void *cuda_stream);
+
 /* Kernel-variant selection for measurements ("chosen by ncu", north_star).  key = "project" or
  * "backproject"; the meaning of `variant` is listed in DESIGN.md §5.  Unknown => OAT_ERR_INVALID. */
 int oat_set_variant(oat_geometry *geom, const char *key, int variant);

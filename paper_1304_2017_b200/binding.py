@@ -19,7 +19,7 @@ EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
-    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp",
+    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_sph_set", "oat_sph_project", "oat_sph_backproject",
     "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_last_error", "oat_version",
 ]
 
@@ -91,6 +91,11 @@ def load():
     lib.oat_penalty_apply.argtypes = [vp, fp, fp, vp]
     lib.oat_penalty_value.argtypes = [vp, fp, dp, vp]
     lib.oat_pls_cg.argtypes = [vp, fp, fp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
+    lib.oat_sph_set.argtypes = [vp, ctypes.c_int32, ctypes.c_double, ctypes.c_double, fp]
+    lib.oat_sph_project.argtypes = [vp, fp, fp, vp]
+    lib.oat_sph_backproject.argtypes = [vp, fp, fp, vp]
+    for n in ("oat_sph_set", "oat_sph_project", "oat_sph_backproject"):
+        getattr(lib, n).restype = ctypes.c_int
     lib.oat_fbp.argtypes = [vp, fp, fp, fp, vp]
     lib.oat_fbp.restype = ctypes.c_int
     for n in ("oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply",
@@ -352,4 +357,40 @@ def oat_fbp(g, p, weights, x=None, stream=None):
         x = torch.empty(g.shape, dtype=torch.float32, device=p.device)
     _check(load().oat_fbp(g.handle, _dev_ptr(p, oat_num_samples(g), "p", g), _dev_ptr(weights, g.n_trans, "weights", g),
                           _dev_ptr(x, oat_num_voxels(g), "x", g), _stream(stream)))
+    return x
+
+
+# ---------------------------------------------------------------- row NEXT-3: spherical-voxel model (frequency domain)
+def oat_sph_set(g, nf, f0, df, he=None):
+    """Frequency grid f_l = f0 + l df and (optionally) the complex EIR spectrum h~e(f_l); nf = 0 removes it."""
+    ptr = None
+    if he is not None:
+        he = np.asarray(he, dtype=np.complex64).ravel()
+        if he.size != nf:
+            raise OatError(OAT_ERR_INVALID, f"he must have {nf} complex samples")
+        buf = np.ascontiguousarray(he.view(np.float32))
+        ptr = ctypes.c_void_p(buf.ctypes.data)
+    _check(load().oat_sph_set(g.handle, ctypes.c_int32(int(nf)), ctypes.c_double(float(f0)), ctypes.c_double(float(df)), ptr))
+    g.sph_nf = int(nf)
+
+
+def oat_sph_project(g, x, u=None, stream=None):
+    """u = H_sph x: complex64 tensor (Q, nf)."""
+    import torch
+    nf = getattr(g, "sph_nf", 0)
+    if u is None:
+        u = torch.empty((g.n_trans, nf), dtype=torch.complex64, device=x.device)
+    ur = torch.view_as_real(u)
+    _check(load().oat_sph_project(g.handle, _dev_ptr(x, oat_num_voxels(g), "x", g), _dev_ptr(ur, 2 * g.n_trans * nf, "u", g), _stream(stream)))
+    return u
+
+
+def oat_sph_backproject(g, u, x=None, stream=None):
+    """x = Re H_sph† u for a complex64 tensor u (Q, nf)."""
+    import torch
+    nf = getattr(g, "sph_nf", 0)
+    if x is None:
+        x = torch.empty(g.shape, dtype=torch.float32, device=u.device)
+    ur = torch.view_as_real(u)
+    _check(load().oat_sph_backproject(g.handle, _dev_ptr(ur, 2 * g.n_trans * nf, "u", g), _dev_ptr(x, oat_num_voxels(g), "x", g), _stream(stream)))
     return x

@@ -72,6 +72,9 @@ struct oat_geometry {
     float *d_y4 = nullptr;                    // EIR scratch (row NEXT-1, lazy)
     float *d_he = nullptr;                    // EIR taps [h^e]_m, m = 0..n_he-1 (Eq. 14), NULL = no EIR
     int n_he = 0;
+    float2 *d_p0 = nullptr, *d_sv = nullptr;  // row NEXT-3: p~0(f_l) (Eq. 19) and the scratch v = u conj(p~0)
+    int sph_nf = 0;
+    double sph_f0 = 0, sph_df = 0;
     double *d_scal = nullptr;                 // a few fp64 scalars (dots)
     unsigned long long *d_counter = nullptr;
     double *h_scal = nullptr;                 // pinned mirror of d_scal
@@ -94,7 +97,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
-    cudaFree(g->d_y4); cudaFree(g->d_he);
+    cudaFree(g->d_y4); cudaFree(g->d_he); cudaFree(g->d_p0); cudaFree(g->d_sv);
     cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
@@ -826,6 +829,62 @@ int oat_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double
     }
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaStreamSynchronize(st));
+    return OAT_OK;
+}
+
+int oat_sph_set(oat_geometry *g, int32_t nf, double f0, double df, const float *h_he)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (nf < 0 || nf > (1 << 20) || !(f0 >= 0) || !(df >= 0) || !isfinite(f0) || !isfinite(df))
+        return fail(OAT_ERR_INVALID, "bad frequency grid (nf >= 0, f0 >= 0, df >= 0)");
+    CUDA_TRY(cudaDeviceSynchronize());
+    cudaFree(g->d_p0); cudaFree(g->d_sv); g->d_p0 = nullptr; g->d_sv = nullptr; g->sph_nf = 0;
+    if (nf == 0) return OAT_OK;
+    // Eq. (19) L153 in fp64 (reading G27): p~0(f) = -j (4 pi kappa c^3 / f) [ (ds/2c) cos(pi f ds/c) - sin(pi f ds/c)/(2 pi f) ] h~e(f), p~0(0) = 0
+    std::vector<float2> p0((size_t)nf);
+    const double ds = g->desc.spacing, c = g->desc.c;
+    for (int l = 0; l < nf; ++l) {
+        const double f = f0 + l * df;
+        double im = 0.0;
+        if (f != 0.0) {
+            const double a = kPi * f * ds / c;
+            im = -(4.0 * kPi * g->kappa * c * c * c / f) * ((ds / (2.0 * c)) * cos(a) - sin(a) / (2.0 * kPi * f));
+        }
+        double re = 0.0;
+        if (h_he) {                                        // (j im) (hr + j hi) = -im hi + j im hr
+            const double hr = h_he[2 * l], hi = h_he[2 * l + 1];
+            if (!isfinite(hr) || !isfinite(hi)) return fail(OAT_ERR_INVALID, "EIR spectrum sample %d is not finite", l);
+            re = -im * hi; im = im * hr;
+        }
+        p0[l] = make_float2((float)re, (float)im);
+    }
+    CUDA_TRY(cudaMalloc((void **)&g->d_p0, sizeof(float2) * (size_t)nf));
+    CUDA_TRY(cudaMemcpy(g->d_p0, p0.data(), sizeof(float2) * (size_t)nf, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMalloc((void **)&g->d_sv, sizeof(float2) * (size_t)nf * (size_t)(g->dev.Q > 0 ? g->dev.Q : 1)));
+    g->sph_nf = nf; g->sph_f0 = f0; g->sph_df = df;
+    return OAT_OK;
+}
+
+int oat_sph_project(oat_geometry *g, const float *d_x, float *d_u, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!g->sph_nf) return fail(OAT_ERR_INVALID, "no frequency grid set (oat_sph_set)");
+    if (!d_x || (!d_u && g->dev.Q)) return fail(OAT_ERR_INVALID, "d_x / d_u must not be NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (g->dev.Q > 0) CUDA_TRY(cudaMemsetAsync(d_u, 0, sizeof(float2) * (size_t)g->sph_nf * (size_t)g->dev.Q, st));
+    oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, d_x, g->d_p0, d_u, st);
+    CUDA_TRY(cudaGetLastError());
+    return OAT_OK;
+}
+
+int oat_sph_backproject(oat_geometry *g, const float *d_u, float *d_x, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!g->sph_nf) return fail(OAT_ERR_INVALID, "no frequency grid set (oat_sph_set)");
+    if (!d_x || (!d_u && g->dev.Q)) return fail(OAT_ERR_INVALID, "d_x / d_u must not be NULL");
+    oat_launch_sph_bwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, reinterpret_cast<const float2 *>(d_u),
+                       g->d_p0, g->d_sv, d_x, (cudaStream_t)stream);
+    CUDA_TRY(cudaGetLastError());
     return OAT_OK;
 }
 

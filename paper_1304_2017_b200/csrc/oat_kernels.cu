@@ -1258,6 +1258,135 @@ oat_fbp_kernel(const OatDev P, const float *__restrict__ p, const float *__restr
     if (inside) x[((size_t)iz * P.ny + iy) * P.nx + ix] = (float)total;
 }
 
+// Row NEXT-3, spherical-voxel model in the temporal frequency domain, point-like transducers (Eq. 17-19,
+// Eq. 24, Alg. 9; readings G27-G29).  u[q,l] = p0[l] sum_n x_n exp(-j 2 pi f_l d/c) / (2 pi d).
+// The phase 2 pi f d / c reaches ~10^3 cycles, so the distance and the phase reduction (frac of f d / c) are fp64; the
+// phasor of the first frequency of a group of OAT_SG and the phasor step exp(-j 2 pi df d/c) come from sincospif, the
+// other frequencies of the group by complex recurrence (OAT_SG - 1 fp32 rotations, error ~ OAT_SG eps).
+#define OAT_SG 16          // frequencies per thread (forward) / per re-seeded group (adjoint)
+#define OAT_SV 2048        // voxels per block chunk (forward)
+struct OatSph { int nf, n_lg; double f0, df, ds_over_c, ds; };   // ds_over_c: microseconds per node unit of distance
+
+__global__ void __launch_bounds__(128)
+oat_sph_fwd_kernel(const OatDev P, const OatSph S, const float *__restrict__ x, const float2 *__restrict__ p0, float *__restrict__ u)
+{
+    __shared__ float s_x[OAT_SV];
+    const long long n_vox = (long long)P.nx * P.ny * P.nz;
+    const long long v0 = (long long)blockIdx.y * OAT_SV;
+    const int nv = (int)min((long long)OAT_SV, n_vox - v0);
+    int any = 0;
+    for (int i = threadIdx.x; i < nv; i += blockDim.x) { const float v = x[v0 + i]; s_x[i] = v; any |= (v != 0.f); }
+    if (!__syncthreads_or(any)) return;                    // an all-zero chunk contributes nothing
+    const long long wi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (wi >= (long long)P.Q * S.n_lg) return;
+    const int q = (int)(wi / S.n_lg), lg = (int)(wi % S.n_lg);
+    const int l0 = lg * OAT_SG;
+    const double *f = P.frame + (size_t)q * 12;
+    const double tx = f[9] - 1.0, ty = f[10] - 1.0, tz = f[11] - 1.0;       // node coordinates (frames hold padded ones)
+    const double fa = S.f0 + (double)l0 * S.df;
+    float ar[OAT_SG], ai[OAT_SG];
+#pragma unroll
+    for (int j = 0; j < OAT_SG; ++j) ar[j] = ai[j] = 0.f;
+    int ix = (int)(v0 % P.nx), iy = (int)((v0 / P.nx) % P.ny), iz = (int)(v0 / ((long long)P.nx * P.ny));
+    for (int i = 0; i < nv; ++i) {
+        const float xv = s_x[i];                           // same address for the whole block: a broadcast
+        if (xv != 0.f) {                                   // block-uniform branch
+            const double dx = (double)ix - tx, dy = (double)iy - ty, dz = (double)iz - tz;
+            const double d = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
+            if (d > 0.0) {
+                const double td = d * S.ds_over_c;         // |r_q - r_n| / c
+                const double pa = fa * td, pd = S.df * td; // cycles
+                float sr, cr, sz, cz;
+                sincospif((float)(-2.0 * (pa - rint(pa))), &sr, &cr);
+                sincospif((float)(-2.0 * (pd - rint(pd))), &sz, &cz);
+                const float amp = xv / (float)(6.283185307179586 * d * S.ds);
+                float er = amp * cr, ei = amp * sr;
+#pragma unroll
+                for (int j = 0; j < OAT_SG; ++j) {
+                    ar[j] += er; ai[j] += ei;
+                    const float nr = fmaf(er, cz, -ei * sz);
+                    ei = fmaf(er, sz, ei * cz);
+                    er = nr;
+                }
+            }
+        }
+        if (++ix == P.nx) { ix = 0; if (++iy == P.ny) { iy = 0; ++iz; } }
+    }
+#pragma unroll
+    for (int j = 0; j < OAT_SG; ++j) {
+        const int l = l0 + j;
+        if (l < S.nf) {
+            const float2 c = p0[l];
+            float *o = u + 2 * ((size_t)q * S.nf + l);
+            atomicAdd(o, ar[j] * c.x - ai[j] * c.y);
+            atomicAdd(o + 1, ar[j] * c.y + ai[j] * c.x);
+        }
+    }
+}
+
+// v[q,l] = u[q,l] conj(p0[l])   (the data-side factor of Eq. 24)
+__global__ void oat_sph_prep_kernel(const OatSph S, int Q, const float2 *__restrict__ u, const float2 *__restrict__ p0, float2 *__restrict__ v)
+{
+    const long long n = (long long)Q * S.nf;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float2 a = u[i], c = p0[i % S.nf];
+        v[i] = make_float2(a.x * c.x + a.y * c.y, a.y * c.x - a.x * c.y);
+    }
+}
+
+// x[n] = Re sum_q sum_l v[q,l] exp(+j 2 pi f_l d/c) / (2 pi d)   (Eq. 24, reading G29); one thread per voxel, the rows
+// v[q,:] of OAT_SQ transducers staged in shared memory at a time (every thread reads the same element: broadcast)
+#define OAT_SQ 4
+#define OAT_SL 512         // frequencies per staged slab
+__global__ void __launch_bounds__(128)
+oat_sph_bwd_kernel(const OatDev P, const OatSph S, const float2 *__restrict__ v, float *__restrict__ x)
+{
+    __shared__ float2 s_v[OAT_SQ][OAT_SL];
+    __shared__ double s_t[OAT_SQ][3];
+    const long long n_vox = (long long)P.nx * P.ny * P.nz;
+    const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool inside = n < n_vox;
+    const int ix = (int)(n % P.nx), iy = (int)((n / P.nx) % P.ny), iz = (int)(n / ((long long)P.nx * P.ny));
+    double total = 0.0;
+    for (int q0 = 0; q0 < P.Q; q0 += OAT_SQ) {
+        const int nq = min(OAT_SQ, P.Q - q0);
+        for (int lb = 0; lb < S.nf; lb += OAT_SL) {
+            const int nl = min(OAT_SL, S.nf - lb);
+            __syncthreads();
+            for (int t = threadIdx.x; t < nq * nl; t += blockDim.x) s_v[t / nl][t % nl] = v[(size_t)(q0 + t / nl) * S.nf + lb + t % nl];
+            if (threadIdx.x < nq * 3) s_t[threadIdx.x / 3][threadIdx.x % 3] = P.frame[(size_t)(q0 + threadIdx.x / 3) * 12 + 9 + threadIdx.x % 3] - 1.0;
+            __syncthreads();
+            if (!inside) continue;
+            for (int j = 0; j < nq; ++j) {
+                const double dx = (double)ix - s_t[j][0], dy = (double)iy - s_t[j][1], dz = (double)iz - s_t[j][2];
+                const double d = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
+                if (!(d > 0.0)) continue;
+                const double td = d * S.ds_over_c, pd = S.df * td;
+                float sz, cz;
+                sincospif((float)(2.0 * (pd - rint(pd))), &sz, &cz);
+                const float amp = 1.f / (float)(6.283185307179586 * d * S.ds);
+                float acc = 0.f;
+                for (int g0 = 0; g0 < nl; g0 += OAT_SG) {
+                    const double pa = (S.f0 + (double)(lb + g0) * S.df) * td;
+                    float sr, cr;
+                    sincospif((float)(2.0 * (pa - rint(pa))), &sr, &cr);
+                    float er = amp * cr, ei = amp * sr;
+                    const int ng = min(OAT_SG, nl - g0);
+                    for (int k = 0; k < ng; ++k) {
+                        const float2 vv = s_v[j][g0 + k];
+                        acc = fmaf(vv.x, er, fmaf(-vv.y, ei, acc));        // Re(v e)
+                        const float nr = fmaf(er, cz, -ei * sz);
+                        ei = fmaf(er, sz, ei * cz);
+                        er = nr;
+                    }
+                }
+                total += (double)acc;
+            }
+        }
+    }
+    if (inside) x[n] = (float)total;
+}
+
 inline int grid_for(long long n, int block)
 {
     long long g = (n + block - 1) / block;
@@ -1477,6 +1606,23 @@ void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, 
 {
     const dim3 grid((unsigned)((P.nx + 7) / 8), (unsigned)((P.ny + 7) / 8), (unsigned)((P.nz + 3) / 4));
     oat_fbp_kernel<<<grid, 256, 0, st>>>(P, p, wq, x);
+}
+
+void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float *x, const float2 *p0, float *u, cudaStream_t st)
+{
+    OatSph S; S.nf = nf; S.n_lg = (nf + OAT_SG - 1) / OAT_SG; S.f0 = f0; S.df = df; S.ds = ds; S.ds_over_c = ds / c;
+    const long long n_vox = (long long)P.nx * P.ny * P.nz, work = (long long)P.Q * S.n_lg;
+    if (n_vox <= 0 || work <= 0) return;
+    const dim3 grid((unsigned)((work + 127) / 128), (unsigned)((n_vox + OAT_SV - 1) / OAT_SV));
+    oat_sph_fwd_kernel<<<grid, 128, 0, st>>>(P, S, x, p0, u);
+}
+
+void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st)
+{
+    OatSph S; S.nf = nf; S.n_lg = (nf + OAT_SG - 1) / OAT_SG; S.f0 = f0; S.df = df; S.ds = ds; S.ds_over_c = ds / c;
+    const long long n_vox = (long long)P.nx * P.ny * P.nz, n = (long long)P.Q * nf;
+    if (n > 0) oat_sph_prep_kernel<<<grid_for(n, 256), 256, 0, st>>>(S, P.Q, u, p0, v);
+    if (n_vox > 0) oat_sph_bwd_kernel<<<(unsigned)((n_vox + 127) / 128), 128, 0, st>>>(P, S, v, x);
 }
 
 void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha, float beta, cudaStream_t st)
