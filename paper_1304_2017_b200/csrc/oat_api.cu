@@ -3,9 +3,6 @@
 // management, and the operator entry points.  All hot work is in oat_kernels.cu.
 #include "../../include/oat.h"
 #include "oat_internal.h"
-#ifndef OAT_MARCH_TEX
-#define OAT_MARCH_TEX 0
-#endif
 
 #include <math.h>
 #include <stdarg.h>
@@ -432,9 +429,6 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     if (variant == 4) {
         if (!G->d_cells) CUDA_TRY(cudaMalloc((void **)&G->d_cells, sizeof(float4) * 2 * G->n_cells));
         oat_launch_pad_cells(P, d_x, G->d_cells, st); ++G->last_launches;
-#if OAT_MARCH_TEX
-        { int rc = ensure_atlas(G); if (rc) return rc; oat_launch_pad_atlas(P, d_x, G->surf, st); ++G->last_launches; }
-#endif
         src = reinterpret_cast<const float *>(G->d_cells);
     } else if (variant == 3) {
         if (!G->d_octs) CUDA_TRY(cudaMalloc((void **)&G->d_octs, sizeof(float4) * G->n_octs));

@@ -113,9 +113,6 @@ __device__ __forceinline__ void fetch8(const OatDev &P, const float *__restrict_
     }
 }
 
-#ifndef OAT_MARCH_TEX
-#define OAT_MARCH_TEX 0
-#endif
 #define OAT_U 4    // list entries in flight per warp (independent dependency chains)
 
 // Per-lane constants of one (transducer q, band): lane = time sample k of the band.
@@ -331,7 +328,9 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
 // record load (8 selects per step), two rays interleaved per thread on 16 accumulators, and 6 or 5 resident blocks
 // with more registers: the kernel time does not react to occupancy or to loads in flight because it sits at the
 // rate at which an SM's L1 can send sector misses to L2 (ncu: l1tex__m_l1tex2xbar_req_cycles_active 51 %, 0.46
-// sectors per SM-cycle, L1 hit rate 5 % by construction -- every record is used by exactly one ray).
+// sectors per SM-cycle, L1 hit rate 5 % by construction -- every record is used by exactly one ray).  Fetching the 8
+// corner values with two predicated texture gathers (tld4 from the slice atlas) instead of the record load: 122 ms
+// against 79.5 ms.
 __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
@@ -367,30 +366,11 @@ __device__ __forceinline__ void consume_march_fwd(const OatDev &P, const Entry *
             // padded cell n' in [0, N] <=> xi in [-1, N): the sample touches at least one existing node (S4)
             const bool in = ((unsigned)ix <= (unsigned)P.nx) & ((unsigned)iy <= (unsigned)P.ny) & ((unsigned)iz <= (unsigned)P.nz);
             const unsigned idx = in ? (unsigned)((iz * P.cy + iy) * P.cx + ix) : P.zero_cell;
-            const float fx = tx - (rx - OAT_MAGIC), fy = ty - (ry - OAT_MAGIC), fz = tz - (rz - OAT_MAGIC);
-#if OAT_MARCH_TEX
-            if (ch) {                                      // 2 texture gathers from the slice atlas: the 8 corner values
-                const int jx = in ? ix : 0, jy = in ? iy : 0, jz = in ? iz : 0;
-                const int z1 = jz + 1;
-                const float ux = (float)jx + 1.0f, uy = (float)jy + 1.0f;
-                const float ax0 = (float)((jz & P.atlas_mask) * P.px), ay0 = (float)((jz >> P.atlas_shift) * P.py);
-                const float ax1 = (float)((z1 & P.atlas_mask) * P.px), ay1 = (float)((z1 >> P.atlas_shift) * P.py);
-                const float4 glo = tex2Dgather<float4>(P.tex, ux + ax0, uy + ay0, 0);
-                const float4 ghi = tex2Dgather<float4>(P.tex, ux + ax1, uy + ay1, 0);
-                const float m = in ? 1.f : 0.f;
-                c[0] = glo.w * m; c[1] = glo.z * m; c[2] = glo.x * m; c[3] = glo.y * m;
-                c[4] = ghi.w * m; c[5] = ghi.z * m; c[6] = ghi.x * m; c[7] = ghi.y * m;
-            }
-            const float a00 = fmaf(fx, c[1] - c[0], c[0]), a10 = fmaf(fx, c[3] - c[2], c[2]);
-            const float a01 = fmaf(fx, c[5] - c[4], c[4]), a11 = fmaf(fx, c[7] - c[6], c[6]);
-            const float b0 = fmaf(fy, a10 - a00, a00), b1 = fmaf(fy, a11 - a01, a01);
-            acc[k] = fmaf(e.a.w, fmaf(fz, b1 - b0, b0), acc[k]);
-#else
             ldg256_if(c, cells + 2 * (size_t)idx, ch);
+            const float fx = tx - (rx - OAT_MAGIC), fy = ty - (ry - OAT_MAGIC), fz = tz - (rz - OAT_MAGIC);
             const float lo = fmaf(fy, fmaf(fx, c[3], c[2]), fmaf(fx, c[1], c[0]));
             const float hi = fmaf(fy, fmaf(fx, c[7], c[6]), fmaf(fx, c[5], c[4]));
             acc[k] = fmaf(e.a.w, fmaf(fz, hi, lo), acc[k]);
-#endif
         }
     }
 }
