@@ -80,6 +80,7 @@ struct oat_geometry {
     double *h_scal = nullptr;                 // pinned mirror of d_scal
     long long n_surface_samples = -1;
     int variant_project = 4, variant_backproject = 4;   // measured best
+    bool march_ok = false;                    // ray anchors fit the 10-bit packed offsets of the marching kernels' list
     cudaArray_t atlas = nullptr;              // slice atlas for the texture-gather projection (lazy)
     cudaTextureObject_t tex = 0;
     cudaSurfaceObject_t surf = 0;
@@ -321,6 +322,10 @@ int build_geometry(oat_geometry *G)
         G->n_faces = ok ? (size_t)tot : 0;
     }
     G->n_cells = P.cx ? (size_t)(d.nz + 1) * (size_t)P.cxy + 1 : 0;
+    {   // packed list entries: anchor node offsets in [-128, 895] (anchor = band midpoint, at most 16 samples outside the padded box)
+        const int nmax = d.nx > d.ny ? (d.nx > d.nz ? d.nx : d.nz) : (d.ny > d.nz ? d.ny : d.nz);
+        G->march_ok = (16.0 * P.step + 4.0 <= 128.0) && (nmax + 2 + 16.0 * P.step + 4.0 <= 895.0);
+    }
 
     G->n_vox = (size_t)d.nx * d.ny * d.nz;
     G->n_dat = (size_t)Q * K;
@@ -425,7 +430,7 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
     G->last_launches = 0;
     const float *src = G->d_xpad;
     int variant = G->variant_project;
-    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_cells || !P.dir)) variant = 3;   // marching form needs B = 32 patches
+    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_cells || !P.dir || !G->march_ok)) variant = 3;   // marching form needs B = 32 patches
     if (variant == 4) {
         if (!G->d_cells) CUDA_TRY(cudaMalloc((void **)&G->d_cells, sizeof(float4) * 2 * G->n_cells));
         oat_launch_pad_cells(P, d_x, G->d_cells, st); ++G->last_launches;
@@ -470,7 +475,7 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
     const OatDev &P = G->dev;
     G->last_launches = 0;
     int variant = G->variant_backproject;
-    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_faces || !P.dir)) variant = 3;   // marching form needs B = 32 patches
+    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_faces || !P.dir || !G->march_ok)) variant = 3;   // marching form needs B = 32 patches
     const bool faces = variant == 4;
     const bool quads = !faces && variant >= 2;
     float *acc = G->d_xpad;

@@ -25,7 +25,16 @@
 #define OAT_MT 128         // threads per block of the marching kernels
 #endif
 #define OAT_BU 8           // steps per trip of the (rolled) backprojection marching loop
-#define OAT_ML 512         // list entries per build/consume round of the marching kernels (16 rings x 32)
+// list entries (32 B each) per build/consume round of the marching kernels: 512 = 16 rings x 32 (16 KB per block).
+// Measured on the config-3 subset (H / H^T ms): 48-byte entries x 512: 79.5 / 91.5; 32-byte x 256: 75.8 / 95.9;
+// 32-byte x 512: 70.8 / 91.5; 32-byte x 1024 at 6 blocks: 78.9 / 91.4 -- less shared memory leaves more L1 for the
+// scattered record loads of H, fewer rounds mean fewer barriers.
+#ifndef OAT_MLH
+#define OAT_MLH 512
+#endif
+#ifndef OAT_MLT
+#define OAT_MLT 512
+#endif
 
 struct OatBand {
     double s_mid;      // radius of the band's anchor (k0 + (B-1)/2) in voxel units: rho/ds

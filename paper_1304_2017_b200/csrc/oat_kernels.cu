@@ -23,11 +23,43 @@
 
 namespace {
 
+#define OAT_MAGIC_BITS_C 0x4B400000   // bit pattern of 1.5 * 2^23 (OAT_MAGIC below)
 struct __align__(16) Entry {
     float4 a;   // anchor fraction (x,y,z) in [-0.5,0.5], omega
     float4 u;   // direction (x,y,z) in voxel axes, unused
     int4 i;     // anchor integer node offset in the padded volume (x,y,z), unused
 };
+
+// 32-byte list entry of the marching kernels: the three integer anchor offsets (each in [-OAT_PB, 1023 - OAT_PB]:
+// checked at variant selection) packed into the bit pattern of u.w.  A third less shared memory per block than
+// Entry: what is not carved out for shared memory is L1, and the rate at which L1 serves the scattered record loads
+// of H falls with its size (micro-benchmark in profiles/r1h_*).
+#define OAT_PB 128
+struct __align__(16) PEntry {
+    float4 a;   // anchor fraction (x,y,z), omega
+    float4 u;   // direction (x,y,z), packed anchor node offsets
+};
+
+__device__ __forceinline__ PEntry pack_entry(const Entry &e)
+{
+    PEntry p;
+    p.a = e.a;
+    const unsigned pk = (unsigned)(e.i.x + OAT_MAGIC_BITS_C + OAT_PB) | ((unsigned)(e.i.y + OAT_MAGIC_BITS_C + OAT_PB) << 10) |
+                        ((unsigned)(e.i.z + OAT_MAGIC_BITS_C + OAT_PB) << 20);
+    p.u = make_float4(e.u.x, e.u.y, e.u.z, __uint_as_float(pk));
+    return p;
+}
+
+__device__ __forceinline__ Entry unpack_entry(const PEntry &p)
+{
+    Entry e;
+    e.a = p.a;
+    e.u = make_float4(p.u.x, p.u.y, p.u.z, 0.f);
+    const unsigned pk = __float_as_uint(p.u.w);
+    e.i = make_int4((int)(pk & 1023u) - (OAT_MAGIC_BITS_C + OAT_PB), (int)((pk >> 10) & 1023u) - (OAT_MAGIC_BITS_C + OAT_PB),
+                    (int)((pk >> 20) & 1023u) - (OAT_MAGIC_BITS_C + OAT_PB), 0);
+    return e;
+}
 
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -343,12 +375,12 @@ __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool p
 // per thread fit the 64-register budget of 8 resident blocks per SM (32 spilled to local memory: ncu showed
 // 0.8 LDL + 0.8 STL per warp-step and 30 % of the L2 traffic), at the price of one extra record load per ray.
 template <int NT, int K0>
-__device__ __forceinline__ void consume_march_fwd(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid,
+__device__ __forceinline__ void consume_march_fwd(const OatDev &P, const PEntry *__restrict__ list, int n_list, int tid,
                                                   const float4 *__restrict__ cells, float (&acc)[16])
 {
     const float stepf = (float)P.step;
     for (int ei = tid; ei < n_list; ei += NT) {
-        const Entry e = list[ei];
+        const Entry e = unpack_entry(list[ei]);
         const float sx = e.u.x * stepf, sy = e.u.y * stepf, sz = e.u.z * stepf;
         float prx = 0.f, pry = 0.f, prz = 0.f;            // previous step's rounded coordinates (cell identity);
                                                           // 0 never equals a rounded coordinate (those are >= 2^22)
@@ -395,12 +427,12 @@ __device__ __forceinline__ void red_add_v4_if(float4 *addr, float a, float b, fl
 }
 
 template <int NT>
-__device__ __forceinline__ void consume_march_bwd(const OatDev &P, const Entry *__restrict__ list, int n_list, int tid,
+__device__ __forceinline__ void consume_march_bwd(const OatDev &P, const PEntry *__restrict__ list, int n_list, int tid,
                                                   const float *__restrict__ s_coef, float4 *__restrict__ faces)
 {
     const float stepf = (float)P.step;
     for (int ei = tid; ei < n_list; ei += NT) {
-        const Entry e = list[ei];
+        const Entry e = unpack_entry(list[ei]);
         const float mx = fabsf(e.u.x), my = fabsf(e.u.y), mz = fabsf(e.u.z);
         const int o = (mx >= my && mx >= mz) ? 0 : (my >= mz ? 1 : 2);
         // local axes (0, 1, 2) = (a, b, c) = (x,y,z), (y,z,x), (z,x,y)
@@ -688,7 +720,7 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
 // loop trimmed -- small blocks (OAT_MT threads, 8 resident per SM) so that the dependent loads at the top
 // of a patch overlap other blocks' marching; directions from the fp64 table instead of sincospi; the
 // adjoint time stencil precomputed per (q,k) by oat_coef_kernel; a patch's 32 rings built and consumed in
-// rounds of OAT_ML / 32 rings (24 KB of list per block).
+// rounds of ML / 32 rings (16 KB of packed list entries per block).
 // ------------------------------------------------------------------------------------------------
 #ifndef OAT_MBLK
 #define OAT_MBLK 8
@@ -720,16 +752,16 @@ __device__ __forceinline__ bool make_entry_tab(const OatDev &P, const OatBand &b
     return hit;
 }
 
-template <int MODE>
+template <int MODE, int ML>
 __global__ void __launch_bounds__(OAT_MT, OAT_MBLK)
 oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__restrict__ faces, float *__restrict__ y_out,
                  const float *__restrict__ coef, double *__restrict__ g)
 {
-    __shared__ Entry list[OAT_ML];
+    __shared__ PEntry list[ML];
     __shared__ double s_frame[12];
     __shared__ float s_red[OAT_MT / 32][16];
     __shared__ float s_coef[64];
-    __shared__ int s_count[OAT_RI * OAT_RJ / OAT_ML];
+    __shared__ int s_count[OAT_RI * OAT_RJ / ML];
     __shared__ int s_flag;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -737,7 +769,7 @@ oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__res
         int q, b, rb, sec;
         unpack_item(P.patches[item], q, b, rb, sec);
         if (tid < 12) s_frame[tid] = P.frame[(size_t)q * 12 + tid];
-        if (tid < OAT_RI * OAT_RJ / OAT_ML) s_count[tid] = 0;
+        if (tid < OAT_RI * OAT_RJ / ML) s_count[tid] = 0;
         const OatBand band = P.band[b];
         const OatRing *__restrict__ ring = P.ring + band.ring_ofs;
         const double2 *__restrict__ dir = P.dir + band.dir_ofs;
@@ -759,10 +791,10 @@ oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__res
         __syncthreads();
         // a band whose 32 data values give g' = 0 contributes exactly nothing to H^T y
         const bool live = (MODE != 1) || (s_flag != 0);
-        for (int rc = r0, round = 0; live && rc < r1; rc += OAT_ML / OAT_RJ, ++round) {
+        for (int rc = r0, round = 0; live && rc < r1; rc += ML / OAT_RJ, ++round) {
             // ---------------------------------------------------------------- build (A2: directions -> ray anchors)
-            const int re = min(rc + OAT_ML / OAT_RJ, r1);
-            for (int t = tid; t < OAT_ML; t += OAT_MT) {
+            const int re = min(rc + ML / OAT_RJ, r1);
+            for (int t = tid; t < ML; t += OAT_MT) {
                 const int r = rc + t / OAT_RJ, jl = t % OAT_RJ;
                 if (r >= re) break;
                 const OatRing R = ring[r];
@@ -771,7 +803,7 @@ oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__res
                 if (j0 + jl >= j1) continue;
                 Entry e;
                 if (!make_entry_tab(P, band, dir[R.cum + j0 + jl], R.ct, R.omega, s_frame, e)) continue;
-                list[atomicAdd(&s_count[round], 1)] = e;
+                list[atomicAdd(&s_count[round], 1)] = pack_entry(e);
             }
             __syncthreads();
             // ---------------------------------------------------------------- consume (A3 / B2-B3)
@@ -1488,8 +1520,8 @@ cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, flo
     if (P.n_patches <= 0) return cudaSuccess;
     const long long cap = 0x7fffffffLL;
     const unsigned grid = (unsigned)(P.n_patches < cap ? P.n_patches : cap);
-    if (mode == 0) oat_march_kernel<0><<<grid, OAT_MT, 0, st>>>(P, cells, faces, y_out, coef, g);
-    else oat_march_kernel<1><<<grid, OAT_MT, 0, st>>>(P, cells, faces, y_out, coef, g);
+    if (mode == 0) oat_march_kernel<0, OAT_MLH><<<grid, OAT_MT, 0, st>>>(P, cells, faces, y_out, coef, g);
+    else oat_march_kernel<1, OAT_MLT><<<grid, OAT_MT, 0, st>>>(P, cells, faces, y_out, coef, g);
     return cudaGetLastError();
 }
 
