@@ -362,7 +362,8 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
 // rate at which an SM's L1 can send sector misses to L2 (ncu: l1tex__m_l1tex2xbar_req_cycles_active 51 %, 0.46
 // sectors per SM-cycle, L1 hit rate 5 % by construction -- every record is used by exactly one ray).  Fetching the 8
 // corner values with two predicated texture gathers (tld4 from the slice atlas) instead of the record load: 122 ms
-// against 79.5 ms.
+// against 79.5 ms.  Splitting the block into independent warp pairs with their own lists and 64-thread named
+// barriers (so that one pair's build overlaps the other's marching): 74.1 ms against 70.8 ms.
 __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
@@ -761,7 +762,8 @@ oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__res
     __shared__ double s_frame[12];
     __shared__ float s_red[OAT_MT / 32][16];
     __shared__ float s_coef[64];
-    __shared__ int s_count[OAT_RI * OAT_RJ / ML];
+    constexpr int NR = (OAT_RI + ML / OAT_RJ - 1) / (ML / OAT_RJ);   // build/consume rounds per patch
+    __shared__ int s_count[NR];
     __shared__ int s_flag;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -769,7 +771,7 @@ oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__res
         int q, b, rb, sec;
         unpack_item(P.patches[item], q, b, rb, sec);
         if (tid < 12) s_frame[tid] = P.frame[(size_t)q * 12 + tid];
-        if (tid < OAT_RI * OAT_RJ / ML) s_count[tid] = 0;
+        if (tid < NR) s_count[tid] = 0;
         const OatBand band = P.band[b];
         const OatRing *__restrict__ ring = P.ring + band.ring_ofs;
         const double2 *__restrict__ dir = P.dir + band.dir_ofs;
