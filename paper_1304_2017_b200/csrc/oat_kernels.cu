@@ -363,7 +363,8 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
 // sectors per SM-cycle, L1 hit rate 5 % by construction -- every record is used by exactly one ray).  Fetching the 8
 // corner values with two predicated texture gathers (tld4 from the slice atlas) instead of the record load: 122 ms
 // against 79.5 ms.  Splitting the block into independent warp pairs with their own lists and 64-thread named
-// barriers (so that one pair's build overlaps the other's marching): 74.1 ms against 70.8 ms.
+// barriers (so that one pair's build overlaps the other's marching): 74.1 ms against 70.8 ms; two rays per thread
+// again, now with the larger L1: 85.6 ms (6 blocks, no spills).
 __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
