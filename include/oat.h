@@ -179,6 +179,15 @@ int oat_measure_red_rate(int device, double *lanes_per_s);
  * run of a ray, Eq. 12 L121 / Alg. 4).  Allocates and frees its own scratch, synchronises the device. */
 int oat_measure_gather_rate(int device, double *sectors_per_s);
 
+/* Parametrised forms of the two probes, behind the tables of DESIGN.md section 5.3 (`python -m paper_1304_2017_b200.probe`).
+ * oat_measure_gather_rate_ex: `lanes_active` of 32 lanes load one scattered sector each, ONE load in flight per warp (the
+ * request shape of H's marching loop), 8 blocks of 128 threads per SM each holding `smem_kb_per_block` KB of (unused)
+ * shared memory -- what is carved out for shared memory is taken from L1.
+ * oat_measure_red_rate_ex: RED.128 with an address pattern within the warp: 0 every lane its own record, 1 32 consecutive
+ * records (16 sectors), 2 one record per 128-byte line, 3 lane pairs sharing a sector, 4 four scattered lines of 8 records. */
+int oat_measure_gather_rate_ex(int device, int lanes_active, int smem_kb_per_block, double *sectors_per_s);
+int oat_measure_red_rate_ex(int device, int pattern, double *lanes_per_s);
+
 const char *oat_last_error(void);
 const char *oat_version(void);
 

@@ -20,7 +20,7 @@ EXPORTS = [
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
     "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_sph_set", "oat_sph_project", "oat_sph_backproject",
-    "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_last_error", "oat_version",
+    "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_measure_gather_rate_ex", "oat_measure_red_rate_ex", "oat_last_error", "oat_version",
 ]
 
 
@@ -84,6 +84,10 @@ def load():
     lib.oat_measure_red_rate.restype = ctypes.c_int
     lib.oat_measure_gather_rate.argtypes = [ctypes.c_int, dp]
     lib.oat_measure_gather_rate.restype = ctypes.c_int
+    lib.oat_measure_gather_rate_ex.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp]
+    lib.oat_measure_gather_rate_ex.restype = ctypes.c_int
+    lib.oat_measure_red_rate_ex.argtypes = [ctypes.c_int, ctypes.c_int, dp]
+    lib.oat_measure_red_rate_ex.restype = ctypes.c_int
     lib.oat_eir_set.argtypes = [vp, fp, ctypes.c_int32]
     lib.oat_eir_apply.argtypes = [vp, fp, fp, ctypes.c_int, vp]
     lib.oat_project_eir.argtypes = [vp, fp, fp, vp]
@@ -394,3 +398,15 @@ def oat_sph_backproject(g, u, x=None, stream=None):
     ur = torch.view_as_real(u)
     _check(load().oat_sph_backproject(g.handle, _dev_ptr(ur, 2 * g.n_trans * nf, "u", g), _dev_ptr(x, oat_num_voxels(g), "x", g), _stream(stream)))
     return x
+
+
+def oat_measure_gather_rate_ex(device: int, lanes_active: int, smem_kb_per_block: int) -> float:
+    v = ctypes.c_double(0.0)
+    _check(load().oat_measure_gather_rate_ex(int(device), int(lanes_active), int(smem_kb_per_block), ctypes.byref(v)))
+    return float(v.value)
+
+
+def oat_measure_red_rate_ex(device: int, pattern: int) -> float:
+    v = ctypes.c_double(0.0)
+    _check(load().oat_measure_red_rate_ex(int(device), int(pattern), ctypes.byref(v)))
+    return float(v.value)

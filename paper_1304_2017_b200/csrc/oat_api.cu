@@ -989,6 +989,66 @@ int oat_measure_gather_rate(int device, double *sectors_per_s)
     return OAT_OK;
 }
 
+int oat_measure_gather_rate_ex(int device, int lanes_active, int smem_kb_per_block, double *sectors_per_s)
+{
+    if (!sectors_per_s || lanes_active < 1 || lanes_active > 32 || smem_kb_per_block < 0 || smem_kb_per_block > 27)
+        return fail(OAT_ERR_INVALID, "bad argument (lanes_active 1..32, smem_kb_per_block 0..27)");
+    CUDA_TRY(cudaSetDevice(device));
+    const size_t bytes = 64u << 20;
+    const int blocks = 148 * 8, iters = 2000;
+    float4 *buf = nullptr; float *sink = nullptr;
+    cudaEvent_t a = nullptr, b = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&buf, bytes));
+    cudaError_t e = cudaMemset(buf, 0, bytes);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&sink, sizeof(float));
+    if (e == cudaSuccess) e = cudaEventCreate(&a);
+    if (e == cudaSuccess) e = cudaEventCreate(&b);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = oat_launch_gather_probe_ex(buf, (unsigned)(bytes / 32), 100, lanes_active, smem_kb_per_block * 1024, blocks, sink, 0);
+    if (e == cudaSuccess) {
+        cudaEventRecord(a, 0);
+        e = oat_launch_gather_probe_ex(buf, (unsigned)(bytes / 32), iters, lanes_active, smem_kb_per_block * 1024, blocks, sink, 0);
+        cudaEventRecord(b, 0);
+        if (e == cudaSuccess) e = cudaEventSynchronize(b);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    }
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
+    cudaFree(sink); cudaFree(buf);
+    if (e != cudaSuccess || !(ms > 0.f)) return fail(OAT_ERR_CUDA, "gather-rate probe failed: %s", cudaGetErrorString(e));
+    *sectors_per_s = (double)blocks * 4.0 * iters * lanes_active / (ms * 1e-3);
+    return OAT_OK;
+}
+
+int oat_measure_red_rate_ex(int device, int pattern, double *lanes_per_s)
+{
+    if (!lanes_per_s || pattern < 0 || pattern > 4) return fail(OAT_ERR_INVALID, "bad argument (pattern 0..4)");
+    CUDA_TRY(cudaSetDevice(device));
+    const size_t bytes = 64u << 20;
+    const int blocks = 148 * 8, iters = 2000;
+    float4 *buf = nullptr;
+    cudaEvent_t a = nullptr, b = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&buf, bytes));
+    cudaError_t e = cudaMemset(buf, 0, bytes);
+    if (e == cudaSuccess) e = cudaEventCreate(&a);
+    if (e == cudaSuccess) e = cudaEventCreate(&b);
+    float ms = 0.f;
+    if (e == cudaSuccess) {
+        oat_launch_red_probe_ex(buf, (unsigned)(bytes / 16), 200, pattern, blocks, 0);
+        cudaEventRecord(a, 0);
+        oat_launch_red_probe_ex(buf, (unsigned)(bytes / 16), iters, pattern, blocks, 0);
+        cudaEventRecord(b, 0);
+        e = cudaEventSynchronize(b);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    }
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
+    cudaFree(buf);
+    if (e != cudaSuccess || !(ms > 0.f)) return fail(OAT_ERR_CUDA, "reduction-rate probe failed: %s", cudaGetErrorString(e));
+    *lanes_per_s = (double)blocks * 256.0 * iters / (ms * 1e-3);
+    return OAT_OK;
+}
+
 const char *oat_last_error(void) { return g_err; }
 const char *oat_version(void) { return "oat-b200 0.1 (OAT-DISC v1; sm_100a)"; }
 

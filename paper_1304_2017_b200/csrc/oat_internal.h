@@ -135,3 +135,6 @@ void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, 
 // row NEXT-3: spherical-voxel model (Eq. 17-19, 24), point-like transducers; u, v: Q x nf complex (float2), p0: nf complex
 void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float *x, const float2 *p0, float *u, cudaStream_t st);
 void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st);
+// parametrised roofline probes (oat_measure_gather_rate_ex / oat_measure_red_rate_ex)
+cudaError_t oat_launch_gather_probe_ex(const float4 *buf, unsigned nsec, int iters, int active, int smem_bytes, int blocks, float *sink, cudaStream_t st);
+void oat_launch_red_probe_ex(float4 *buf, unsigned n16, int iters, int pattern, int blocks, cudaStream_t st);

@@ -916,6 +916,48 @@ __global__ void oat_gather_probe_kernel(const float4 *__restrict__ buf, unsigned
     if (acc == 12345.678f) sink[0] = acc;
 }
 
+// probe for oat_measure_gather_rate_ex(): `active` of the 32 lanes load one pseudo-random sector each, ONE load in flight
+// per thread (its result is consumed before the next is issued) -- the request shape of the marching loop of H;
+// dynamic shared memory (unused) sets the shared-memory carve-out and with it the size of L1
+__global__ void __launch_bounds__(128, 8) oat_gather_probe_ex_kernel(const float4 *__restrict__ buf, unsigned nsec, int iters, int active, float *__restrict__ sink)
+{
+    const unsigned lane = threadIdx.x & 31, gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    unsigned s = gw * 2654435761u + 54321u;
+    float acc = 0.f;
+    const bool act = (int)((lane * 7) & 31) < active;
+    for (int i = 0; i < iters; ++i) {
+        float v[8];
+        s = s * 1664525u + 1013904223u;
+        const unsigned h = (s >> 4) + lane * 2654435761u;
+        const unsigned r = ((h ^ (h >> 13)) * 0x9E3779B1u) & (nsec - 1);      // nsec is a power of two
+        if (act) {
+            asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                         : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+                         : "l"(buf + 2 * (size_t)r));
+            acc += v[0] + v[7];
+        }
+    }
+    if (acc == 12345.678f) sink[0] = acc;
+}
+
+// probe for oat_measure_red_rate_ex(): RED.128 with a chosen address pattern within the warp
+__global__ void oat_red_probe_ex_kernel(float4 *__restrict__ buf, unsigned n16, int iters, int pattern)
+{
+    const unsigned lane = threadIdx.x & 31, gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    unsigned s = gw * 2654435761u + 12345u;
+    for (int i = 0; i < iters; ++i) {
+        s = s * 1664525u + 1013904223u;
+        const unsigned wbase = ((s >> 4) ^ (s >> 17)) * 0x9E3779B1u;       // the same for all lanes of the warp
+        unsigned r;
+        if (pattern == 0) { const unsigned h = (s >> 4) + lane * 2654435761u; r = (h ^ (h >> 13)) * 0x9E3779B1u; }   // every lane its own record
+        else if (pattern == 1) r = wbase + lane;                           // 32 consecutive records = 16 sectors in 4 lines
+        else if (pattern == 2) r = wbase + lane * 8;                       // one record per 128-byte line, 32 lines
+        else if (pattern == 3) r = wbase + (lane >> 1) * 64 + (lane & 1);  // lane pairs share a sector, pairs 1 KB apart
+        else r = wbase + (lane >> 3) * 1024 + (lane & 7);                  // 4 scattered lines of 8 records
+        red_add_v4(buf + (r % n16), 1.f, 1.f, 1.f, 1.f);
+    }
+}
+
 // number of patches per transducer (for the fused time-difference epilogue)
 __global__ void oat_count_patches_kernel(const unsigned long long *__restrict__ patches, long long n, int *__restrict__ q_count)
 {
@@ -1541,6 +1583,19 @@ void oat_launch_red_probe(float4 *buf, unsigned n16, int iters, int blocks, cuda
 void oat_launch_gather_probe(const float4 *buf, unsigned n16, int iters, int blocks, float *sink, cudaStream_t st)
 {
     oat_gather_probe_kernel<<<blocks, 256, 0, st>>>(buf, n16, iters, sink);
+}
+
+cudaError_t oat_launch_gather_probe_ex(const float4 *buf, unsigned nsec, int iters, int active, int smem_bytes, int blocks, float *sink, cudaStream_t st)
+{
+    cudaError_t e = cudaFuncSetAttribute(oat_gather_probe_ex_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+    if (e != cudaSuccess) return e;
+    oat_gather_probe_ex_kernel<<<blocks, 128, smem_bytes, st>>>(buf, nsec, iters, active, sink);
+    return cudaGetLastError();
+}
+
+void oat_launch_red_probe_ex(float4 *buf, unsigned n16, int iters, int pattern, int blocks, cudaStream_t st)
+{
+    oat_red_probe_ex_kernel<<<blocks, 256, 0, st>>>(buf, n16, iters, pattern);
 }
 
 void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st)
