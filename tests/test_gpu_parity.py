@@ -241,6 +241,7 @@ def test_config4_cgls_first_iterations(env):
     g = oat.oat_geometry_create(ws)
     x, res, grad = oat.oat_cgls(g, torch.from_numpy(y).cuda(), 3)
     xo, reso, grado = orc.cgls(ws, y.astype(np.float64), 3)
+    print(f"config4[6]: CGLS x3 |x - x_oracle|/|x_oracle| {rel_l2(x.cpu().numpy(), xo):.2e}, residual curve max rel. diff {np.max(np.abs(res - reso) / reso):.2e}")
     assert np.allclose(res, reso, rtol=2e-4, atol=1e-7)
     assert np.allclose(grad, grado, rtol=2e-3)
     assert rel_l2(x.cpu().numpy(), xo) <= 5e-4
