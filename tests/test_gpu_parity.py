@@ -95,6 +95,16 @@ def test_non_cubic_grid_and_offset_origin(env):
     check_pair(env, w, x=x)
 
 
+def test_coarse_time_sampling_falls_back_from_the_marching_kernels(env):
+    """c dt = 9 voxels per sample: the ray anchors of a 32-sample band lie up to 144 voxels outside the box and do not
+    fit the packed list entries of the marching kernels, so the library must fall back to the
+    lane-per-sample kernels -- same operator, same tolerance."""
+    torch, orc, oat, wl = env
+    w = wl.small(n=14, q=4, nt=40, spacing=0.05, radius=6.0, kband=32, dt=0.3)
+    assert w.c * w.dt / w.spacing > 7.8
+    check_pair(env, w)
+
+
 def test_config1_tiny_full(env):
     """BASELINE.json config 1: one H, one H^T, adjoint test with seeded N(0,1) y."""
     torch, orc, oat, wl = env
