@@ -21,6 +21,7 @@ from __future__ import annotations
 import numpy as np
 
 from .oat_fbp import node_positions
+from . import oat_pls as _pls
 
 
 def freqs(f0, df, nf):
@@ -72,3 +73,34 @@ def backproject(w, u, f0, df, nf, he=None):
         s = (v @ np.exp(2j * np.pi * np.outer(f, d) / w.c)).real
         x += np.where(ok, s / (2.0 * np.pi * np.where(ok, d, 1.0)), 0.0)
     return x.reshape(w.nz, w.ny, w.nx)
+
+
+def pls_cg(w, u, n_iter, mu, f0, df, nf, he=None):
+    """PLS-Sph, Eq. (30) L271 with "linear CG" (L265): CG on (H† H + mu L) x = H† u from x0 = 0 with H = H_sph, H† its
+    real-part adjoint (reading G29) and L the penalty matrix of Eq. (34) (oat_pls.penalty_apply); the data space is
+    C^{QL} with the real inner product Re<.,.>.  Same loop and curves as oat_pls.pls_cg (reading G22):
+    obj_i = ||u - H x_i||^2 + mu R(x_i), grad_i = ||H† u - (H† H + mu L) x_i||."""
+    u = np.asarray(u, dtype=np.complex128)
+    x = np.zeros((w.nz, w.ny, w.nx), dtype=np.float64)
+    d = u.copy()
+    r = backproject(w, u, f0, df, nf, he)
+    p = r.copy()
+    rr = float(np.vdot(r, r))
+    obj = [float(np.real(np.vdot(d, d)))]
+    grad = [rr ** 0.5]
+    for _ in range(n_iter):
+        q = project(w, p, f0, df, nf, he)
+        wv = backproject(w, q, f0, df, nf, he) + mu * _pls.penalty_apply(p)
+        pw = float(np.vdot(p, wv))
+        if pw <= 0.0 or rr == 0.0:
+            obj.append(obj[-1]); grad.append(grad[-1]); continue
+        alpha = rr / pw
+        x += alpha * p
+        d -= alpha * q
+        r -= alpha * wv
+        rr_new = float(np.vdot(r, r))
+        p = r + (rr_new / rr) * p
+        rr = rr_new
+        obj.append(float(np.real(np.vdot(d, d))) + mu * _pls.penalty_value(x))
+        grad.append(rr ** 0.5)
+    return x, np.array(obj), np.array(grad)

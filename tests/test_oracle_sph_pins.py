@@ -75,3 +75,51 @@ def test_adjoint_identity_and_linearity():
     fl = f0 + df * 7
     col = sph.project(w, e, f0, df, nf, he)[4, 7]
     assert np.allclose(col, sph.p0_tilde(w, np.array([fl]))[0] * he[7] * np.exp(-2j * np.pi * fl * d / w.c) / (2 * np.pi * d), rtol=1e-12)
+
+
+def laplacian_edge_by_edge(nz, ny, nx):
+    """Graph Laplacian of the 6-neighbour grid, one pass over the edges (n, n-before) of Eq. (34) (reading G21)."""
+    N = nz * ny * nx
+    Lm = np.zeros((N, N))
+    idx = lambda z, y, x: (z * ny + y) * nx + x
+    for z in range(nz):
+        for y in range(ny):
+            for x in range(nx):
+                n = idx(z, y, x)
+                for (dz, dy, dx) in ((0, 0, 1), (0, 1, 0), (1, 0, 0)):
+                    zz, yy, xx = z - dz, y - dy, x - dx
+                    if zz < 0 or yy < 0 or xx < 0:
+                        continue
+                    m = idx(zz, yy, xx)
+                    Lm[n, n] += 1; Lm[m, m] += 1; Lm[n, m] -= 1; Lm[m, n] -= 1
+    return Lm
+
+
+def test_pls_sph_cg_matches_the_dense_real_system():
+    """Eq. (30): stack real and imaginary parts of the dense H_sph (built column by column) into a real matrix M; the CG
+    iterates must equal textbook CG on (M^T M + mu L) x = M^T u_stacked and converge to numpy.linalg.solve."""
+    w = problem(n=3, q=4)
+    f0, df, nf = 0.2, 0.35, 9
+    N = w.n_voxels
+    Hc = np.stack([sph.project(w, np.eye(N)[n].reshape(w.nz, w.ny, w.nx), f0, df, nf).ravel() for n in range(N)], axis=1)
+    M = np.vstack([Hc.real, Hc.imag])
+    rng = np.random.default_rng(4)
+    xt = rng.random(N)
+    uc = (Hc @ xt).reshape(w.n_trans, nf) * (1.0 + 0.01 * rng.standard_normal((w.n_trans, nf)))
+    us = np.concatenate([uc.ravel().real, uc.ravel().imag])
+    Lm = laplacian_edge_by_edge(w.nz, w.ny, w.nx)
+    mu = 0.02 * np.linalg.norm(M, 2) ** 2
+    A = M.T @ M + mu * Lm; b = M.T @ us
+    assert np.allclose(sph.backproject(w, uc, f0, df, nf).ravel(), b, rtol=1e-11, atol=1e-14 * np.abs(b).max())
+    xc = np.zeros(N); r = b.copy(); p = r.copy(); xs = []
+    for _ in range(6):
+        Ap = A @ p; al = (r @ r) / (p @ Ap); xc = xc + al * p
+        rn = r - al * Ap; p = rn + ((rn @ rn) / (r @ r)) * p; r = rn
+        xs.append(xc.copy())
+    x3, obj, grad = sph.pls_cg(w, uc, 3, mu, f0, df, nf)
+    assert np.allclose(x3.ravel(), xs[2], rtol=1e-8, atol=1e-11 * np.abs(xs[2]).max())
+    phi = lambda x: np.sum((us - M @ x) ** 2) + mu * x @ Lm @ x
+    assert abs(obj[3] - phi(xs[2])) <= 1e-9 * obj[3] and np.all(np.diff(obj) < 0)
+    x80, _, g80 = sph.pls_cg(w, uc, 80, mu, f0, df, nf)
+    xd = np.linalg.solve(A, b)
+    assert np.linalg.norm(x80.ravel() - xd) <= 1e-6 * np.linalg.norm(xd)
