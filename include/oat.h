@@ -156,6 +156,12 @@ int oat_sph_set(oat_geometry *geom, int32_t nf, double f0, double df, const floa
 int oat_sph_project(oat_geometry *geom, const float *d_x, float *d_u, void *cuda_stream);
 int oat_sph_backproject(oat_geometry *geom, const float *d_u, float *d_x, void *cuda_stream);
 
+/* PLS-Sph (Eq. 30): the loop of oat_pls_cg with H = H_sph (the grid of oat_sph_set) and its real-part adjoint;
+ * d_u: Q*nf complex as interleaved (re, im) fp32 pairs (read), d_x: nz*ny*nx fp32 (OVERWRITTEN), mu >= 0; h_obj / h_grad as
+ * in oat_pls_cg with ||.|| the norm of C^{Q nf}.  Synchronises the stream every iteration. */
+int oat_sph_pls_cg(oat_geometry *geom, const float *d_u, float *d_x, int n_iter, double mu,
+                   double *h_obj, double *h_grad, void *cuda_stream);
+
 /* Kernel-variant selection for measurements ("chosen by ncu", north_star).  key = "project" or
  * "backproject"; the meaning of `variant` is listed in DESIGN.md §5.  Unknown => OAT_ERR_INVALID. */
 int oat_set_variant(oat_geometry *geom, const char *key, int variant);

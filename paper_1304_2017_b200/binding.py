@@ -19,7 +19,7 @@ EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
-    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_sph_set", "oat_sph_project", "oat_sph_backproject",
+    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_sph_set", "oat_sph_project", "oat_sph_backproject", "oat_sph_pls_cg",
     "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_measure_gather_rate_ex", "oat_measure_red_rate_ex", "oat_last_error", "oat_version",
 ]
 
@@ -100,6 +100,8 @@ def load():
     lib.oat_sph_backproject.argtypes = [vp, fp, fp, vp]
     for n in ("oat_sph_set", "oat_sph_project", "oat_sph_backproject"):
         getattr(lib, n).restype = ctypes.c_int
+    lib.oat_sph_pls_cg.argtypes = [vp, fp, fp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
+    lib.oat_sph_pls_cg.restype = ctypes.c_int
     lib.oat_fbp.argtypes = [vp, fp, fp, fp, vp]
     lib.oat_fbp.restype = ctypes.c_int
     for n in ("oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply",
@@ -410,3 +412,18 @@ def oat_measure_red_rate_ex(device: int, pattern: int) -> float:
     v = ctypes.c_double(0.0)
     _check(load().oat_measure_red_rate_ex(int(device), int(pattern), ctypes.byref(v)))
     return float(v.value)
+
+
+def oat_sph_pls_cg(g, u, n_iter, mu, x=None, stream=None):
+    """n_iter CG steps on (H_sph† H_sph + mu L) x = H_sph† u from x = 0 for a complex64 tensor u (Q, nf)."""
+    import torch
+    nf = getattr(g, "sph_nf", 0)
+    if x is None:
+        x = torch.empty(g.shape, dtype=torch.float32, device=u.device)
+    obj = np.zeros(n_iter + 1, dtype=np.float64)
+    grad = np.zeros(n_iter + 1, dtype=np.float64)
+    dp = ctypes.POINTER(ctypes.c_double)
+    ur = torch.view_as_real(u)
+    _check(load().oat_sph_pls_cg(g.handle, _dev_ptr(ur, 2 * g.n_trans * nf, "u", g), _dev_ptr(x, oat_num_voxels(g), "x", g),
+                                 int(n_iter), ctypes.c_double(float(mu)), obj.ctypes.data_as(dp), grad.ctypes.data_as(dp), _stream(stream)))
+    return x, obj, grad

@@ -73,6 +73,7 @@ struct oat_geometry {
     float *d_he = nullptr;                    // EIR taps [h^e]_m, m = 0..n_he-1 (Eq. 14), NULL = no EIR
     int n_he = 0;
     float2 *d_p0 = nullptr, *d_sv = nullptr;  // row NEXT-3: p~0(f_l) (Eq. 19) and the scratch v = u conj(p~0)
+    float *d_sd = nullptr, *d_sq = nullptr;   // PLS-Sph data-space vectors (2*Q*nf floats, lazy; freed with the grid)
     int sph_nf = 0;
     double sph_f0 = 0, sph_df = 0;
     double *d_scal = nullptr;                 // a few fp64 scalars (dots)
@@ -98,7 +99,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
     cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
-    cudaFree(g->d_y4); cudaFree(g->d_he); cudaFree(g->d_p0); cudaFree(g->d_sv);
+    cudaFree(g->d_y4); cudaFree(g->d_he); cudaFree(g->d_p0); cudaFree(g->d_sv); cudaFree(g->d_sd); cudaFree(g->d_sq);
     cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
     if (g->tex) cudaDestroyTextureObject(g->tex);
     if (g->surf) cudaDestroySurfaceObject(g->surf);
@@ -780,31 +781,46 @@ int oat_backproject_eir(oat_geometry *g, const float *d_u, float *d_x, void *str
     return backproject_full(g, d_u, d_x, (cudaStream_t)stream);
 }
 
-// Row NEXT-1 (reading G22): linear CG on (H^T H + mu L) x = H^T u from x = 0, H = H^e D G.
-int oat_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double mu, double *h_obj, double *h_grad, void *stream)
+// Rows NEXT-1 / NEXT-3 (reading G22): linear CG on (H^T H + mu L) x = H^T u from x = 0.  sph = false: H = H^e D G, data =
+// Q*K floats (Eq. 29); sph = true: H = H_sph, data = Q*nf complex numbers handled as 2*Q*nf floats -- the real inner
+// product of the interleaved (re, im) pairs is Re<.,.> of C^{QL} (Eq. 30, reading G29).
+static int pls_cg_impl(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double mu, double *h_obj, double *h_grad,
+                       cudaStream_t st, bool sph)
 {
-    int rc = check_handle(g); if (rc) return rc;
-    if (!d_u || !d_x || n_iter < 0 || !(mu >= 0) || !isfinite(mu)) return fail(OAT_ERR_INVALID, "bad argument to oat_pls_cg");
-    cudaStream_t st = (cudaStream_t)stream;
-    if ((rc = ensure(&g->d_y2, g->n_dat))) return rc;     // d = u - H x
-    if ((rc = ensure(&g->d_y3, g->n_dat))) return rc;     // q = H p
+    int rc;
+    const size_t n_dat = sph ? 2 * (size_t)g->sph_nf * (size_t)g->dev.Q : g->n_dat;
+    float **pd = sph ? &g->d_sd : &g->d_y2, **pq = sph ? &g->d_sq : &g->d_y3;
+    if ((rc = ensure(pd, n_dat))) return rc;                // d = u - H x
+    if ((rc = ensure(pq, n_dat))) return rc;                // q = H p
     if ((rc = ensure(&g->d_x2, g->n_vox))) return rc;     // w = (H^T H + mu L) p, later L x
     if ((rc = ensure(&g->d_x3, g->n_vox))) return rc;     // r
     if ((rc = ensure(&g->d_x4, g->n_vox))) return rc;     // p
-    float *d = g->d_y2, *q = g->d_y3, *w = g->d_x2, *r = g->d_x3, *p = g->d_x4;
+    float *d = *pd, *q = *pq, *w = g->d_x2, *r = g->d_x3, *p = g->d_x4;
+    auto fwd = [&](const float *x, float *u) -> int {
+        if (!sph) return project_full(g, x, u, st);
+        CUDA_TRY(cudaMemsetAsync(u, 0, sizeof(float) * n_dat, st));
+        oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, x, g->d_p0, u, st);
+        return OAT_OK;
+    };
+    auto bwd = [&](const float *u, float *x) -> int {
+        if (!sph) return backproject_full(g, u, x, st);
+        oat_launch_sph_bwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, reinterpret_cast<const float2 *>(u),
+                           g->d_p0, g->d_sv, x, st);
+        return OAT_OK;
+    };
     CUDA_TRY(cudaMemsetAsync(d_x, 0, sizeof(float) * g->n_vox, st));
-    CUDA_TRY(cudaMemcpyAsync(d, d_u, sizeof(float) * g->n_dat, cudaMemcpyDeviceToDevice, st));
-    if ((rc = backproject_full(g, d_u, r, st))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(d, d_u, sizeof(float) * n_dat, cudaMemcpyDeviceToDevice, st));
+    if ((rc = bwd(d_u, r))) return rc;
     CUDA_TRY(cudaMemcpyAsync(p, r, sizeof(float) * g->n_vox, cudaMemcpyDeviceToDevice, st));
     double rr, dd;
     if ((rc = dot_sync(g, r, r, g->n_vox, &rr, st))) return rc;
-    if ((rc = dot_sync(g, d, d, g->n_dat, &dd, st))) return rc;
+    if ((rc = dot_sync(g, d, d, n_dat, &dd, st))) return rc;
     if (h_obj) h_obj[0] = dd;
     if (h_grad) h_grad[0] = sqrt(rr);
     for (int it = 0; it < n_iter; ++it) {
         double pw;
-        if ((rc = project_full(g, p, q, st))) return rc;
-        if ((rc = backproject_full(g, q, w, st))) return rc;
+        if ((rc = fwd(p, q))) return rc;
+        if ((rc = bwd(q, w))) return rc;
         if (mu > 0) oat_launch_penalty(g->dev, p, w, (float)mu, 1.f, st);          // w += mu L p
         if ((rc = dot_sync(g, p, w, g->n_vox, &pw, st))) return rc;
         if (!(pw > 0) || rr == 0) {
@@ -814,7 +830,7 @@ int oat_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double
         }
         const double alpha = rr / pw;
         oat_launch_axpy((float)alpha, p, d_x, (long long)g->n_vox, st);
-        oat_launch_axpy((float)-alpha, q, d, (long long)g->n_dat, st);
+        oat_launch_axpy((float)-alpha, q, d, (long long)n_dat, st);
         oat_launch_axpy((float)-alpha, w, r, (long long)g->n_vox, st);
         double rr_new;
         if ((rc = dot_sync(g, r, r, g->n_vox, &rr_new, st))) return rc;
@@ -823,7 +839,7 @@ int oat_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double
         oat_launch_xpay(r, (float)beta, p, (long long)g->n_vox, st);
         if (h_obj) {
             double pen = 0.0;
-            if ((rc = dot_sync(g, d, d, g->n_dat, &dd, st))) return rc;
+            if ((rc = dot_sync(g, d, d, n_dat, &dd, st))) return rc;
             if (mu > 0) {
                 oat_launch_penalty(g->dev, d_x, w, 1.f, 0.f, st);
                 if ((rc = dot_sync(g, d_x, w, g->n_vox, &pen, st))) return rc;
@@ -837,13 +853,29 @@ int oat_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double
     return OAT_OK;
 }
 
+int oat_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double mu, double *h_obj, double *h_grad, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!d_u || !d_x || n_iter < 0 || !(mu >= 0) || !isfinite(mu)) return fail(OAT_ERR_INVALID, "bad argument to oat_pls_cg");
+    return pls_cg_impl(g, d_u, d_x, n_iter, mu, h_obj, h_grad, (cudaStream_t)stream, false);
+}
+
+int oat_sph_pls_cg(oat_geometry *g, const float *d_u, float *d_x, int n_iter, double mu, double *h_obj, double *h_grad, void *stream)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!g->sph_nf) return fail(OAT_ERR_INVALID, "no frequency grid set (oat_sph_set)");
+    if (!d_u || !d_x || n_iter < 0 || !(mu >= 0) || !isfinite(mu)) return fail(OAT_ERR_INVALID, "bad argument to oat_sph_pls_cg");
+    return pls_cg_impl(g, d_u, d_x, n_iter, mu, h_obj, h_grad, (cudaStream_t)stream, true);
+}
+
 int oat_sph_set(oat_geometry *g, int32_t nf, double f0, double df, const float *h_he)
 {
     int rc = check_handle(g); if (rc) return rc;
     if (nf < 0 || nf > (1 << 20) || !(f0 >= 0) || !(df >= 0) || !isfinite(f0) || !isfinite(df))
         return fail(OAT_ERR_INVALID, "bad frequency grid (nf >= 0, f0 >= 0, df >= 0)");
     CUDA_TRY(cudaDeviceSynchronize());
-    cudaFree(g->d_p0); cudaFree(g->d_sv); g->d_p0 = nullptr; g->d_sv = nullptr; g->sph_nf = 0;
+    cudaFree(g->d_p0); cudaFree(g->d_sv); cudaFree(g->d_sd); cudaFree(g->d_sq);
+    g->d_p0 = nullptr; g->d_sv = nullptr; g->d_sd = nullptr; g->d_sq = nullptr; g->sph_nf = 0;
     if (nf == 0) return OAT_OK;
     // Eq. (19) L153 in fp64 (reading G27): p~0(f) = -j (4 pi kappa c^3 / f) [ (ds/2c) cos(pi f ds/c) - sin(pi f ds/c)/(2 pi f) ] h~e(f), p~0(0) = 0
     std::vector<float2> p0((size_t)nf);

@@ -91,3 +91,27 @@ def test_errors_and_empty(env):
     with pytest.raises(oat.OatError):
         oat.oat_sph_set(g, 8, -1.0, 0.1)
     g.close()
+
+
+@pytest.mark.parametrize("mu_rel", [0.0, 0.05])
+def test_pls_sph_cg_first_iterations_match_the_oracle(env, mu_rel):
+    """Eq. (30): 3 CG iterations on a small problem against the oracle's PLS-Sph loop; curves and iterate must match."""
+    torch, osph, oat, wl = env
+    from oracle import oat_pls as opls
+    w = wl.small(n=10, q=6, nt=8, kband=8)
+    nf, f0, df = 32, 0.05, 0.06
+    rng = np.random.default_rng(12)
+    xt = w.phantom().astype(np.float64)
+    ut = osph.project(w, xt, f0, df, nf)
+    u = (ut + 0.02 * np.abs(ut).max() * (rng.standard_normal(ut.shape) + 1j * rng.standard_normal(ut.shape))).astype(np.complex64)
+    b = osph.backproject(w, u.astype(np.complex128), f0, df, nf)
+    mu = mu_rel * float(np.linalg.norm(osph.backproject(w, osph.project(w, b, f0, df, nf), f0, df, nf)) / np.linalg.norm(opls.penalty_apply(b))) if mu_rel else 0.0
+    g = oat.oat_geometry_create(w)
+    oat.oat_sph_set(g, nf, f0, df)
+    x, obj, grad = oat.oat_sph_pls_cg(g, torch.from_numpy(u).cuda(), 3, mu)
+    g.close()
+    xo, objo, grado = osph.pls_cg(w, u.astype(np.complex128), 3, mu, f0, df, nf)
+    assert np.allclose(obj, objo, rtol=5e-4)
+    assert np.allclose(grad, grado, rtol=3e-3)
+    assert rel_l2(x.cpu().numpy(), xo) <= 1e-3
+    assert np.all(np.diff(obj) < 0)
