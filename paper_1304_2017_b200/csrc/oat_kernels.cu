@@ -1451,12 +1451,23 @@ oat_sph_bwd_kernel(const OatDev P, const OatSph S, const float2 *__restrict__ v,
                     sincospif((float)(2.0 * (pa - rint(pa))), &sr, &cr);
                     float er = amp * cr, ei = amp * sr;
                     const int ng = min(OAT_SG, nl - g0);
-                    for (int k = 0; k < ng; ++k) {
-                        const float2 vv = s_v[j][g0 + k];
-                        acc = fmaf(vv.x, er, fmaf(-vv.y, ei, acc));        // Re(v e)
-                        const float nr = fmaf(er, cz, -ei * sz);
-                        ei = fmaf(er, sz, ei * cz);
-                        er = nr;
+                    if (ng == OAT_SG) {                    // full group: unrolled
+#pragma unroll
+                        for (int k = 0; k < OAT_SG; ++k) {
+                            const float2 vv = s_v[j][g0 + k];
+                            acc = fmaf(vv.x, er, fmaf(-vv.y, ei, acc));    // Re(v e)
+                            const float nr = fmaf(er, cz, -ei * sz);
+                            ei = fmaf(er, sz, ei * cz);
+                            er = nr;
+                        }
+                    } else {
+                        for (int k = 0; k < ng; ++k) {
+                            const float2 vv = s_v[j][g0 + k];
+                            acc = fmaf(vv.x, er, fmaf(-vv.y, ei, acc));
+                            const float nr = fmaf(er, cz, -ei * sz);
+                            ei = fmaf(er, sz, ei * cz);
+                            er = nr;
+                        }
                     }
                 }
                 total += (double)acc;
