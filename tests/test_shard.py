@@ -56,7 +56,23 @@ def _worker(rank, world, port, out):
     rows = torch.zeros((w.n_trans, w.nt), dtype=torch.float64)      # only to CHECK the rows (uneven shards: 3 + 2)
     rows[lo:hi] = torch.from_numpy(hx_local)
     dist.all_reduce(rows)
+    # the same split serves the spherical-voxel pair (the paper's own multi-GPU case, Algs. 7-12): rows of H_sph are
+    # per transducer, H_sph† sums over transducers
+    from oracle import oat_sph as osph
+    nf, f0, df = 7, 0.1, 0.3
+    rng = np.random.default_rng(5)
+    u = rng.standard_normal((w.n_trans, nf)) + 1j * rng.standard_normal((w.n_trans, nf))
+    su_local = osph.project(ws, x, f0, df, nf)
+    spart = torch.from_numpy(osph.backproject(ws, u[lo:hi], f0, df, nf))
+    shard.allreduce_volume(spart)
+    srows = torch.zeros((w.n_trans, nf, 2), dtype=torch.float64)
+    srows[lo:hi] = torch.from_numpy(np.stack([su_local.real, su_local.imag], axis=-1))
+    dist.all_reduce(srows)
     if rank == 0:
+        full_su = osph.project(w, x, f0, df, nf)
+        full_sx = osph.backproject(w, u, f0, df, nf)
+        out["su"] = float(np.abs(srows.numpy()[..., 0] + 1j * srows.numpy()[..., 1] - full_su).max() / np.abs(full_su).max())
+        out["sx"] = float(np.abs(spart.numpy() - full_sx).max() / np.abs(full_sx).max())
         full_hx = orc.project(w, x)
         full_xb = orc.backproject(w, y)
         out["hx"] = float(np.abs(rows.numpy() - full_hx).max() / np.abs(full_hx).max())
@@ -69,3 +85,4 @@ def test_two_rank_gloo_sharded_operators():
     mgr = mp.Manager(); out = mgr.dict()
     mp.spawn(_worker, args=(2, port, out), nprocs=2, join=True)
     assert out["hx"] <= 1e-13 and out["xb"] <= 1e-12, dict(out)
+    assert out["su"] <= 1e-13 and out["sx"] <= 1e-12, dict(out)
