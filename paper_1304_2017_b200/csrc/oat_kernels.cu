@@ -368,7 +368,7 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
 __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
-        "@p ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
+        "@p ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"   // a record is used by one ray only
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]), "+f"(c[4]), "+f"(c[5]), "+f"(c[6]), "+f"(c[7])
         : "l"(p), "r"((int)pred));
 }
