@@ -276,13 +276,16 @@ def run_ours(args):
         # What ncu and the micro-benchmarks name as the binding unit of each kernel: H^T retires
         # vector reductions (RED.128) at the rate the L2 atomic path sustains; the peak is measured live.
         try:
-            red_peak = oat.oat_measure_red_rate(local)
+            red_scat = oat.oat_measure_red_rate(local)                 # every lane its own 32-byte sector
+            red_pack = oat.oat_measure_red_rate_ex(local, 1)           # 32 lanes fill 16 sectors: the best case
             red_lanes = RED_PER_SAMPLE * n_samples
+            ach = red_lanes / (k_t * 1e-3) if k_t > 0 else None
             roofline["limiter"] = {"kernel": "oat_march_kernel<1> (backproject)", "unit": "L2 vector reductions (RED.128 lanes/s)",
-                                   "achieved": red_lanes / (k_t * 1e-3) if k_t > 0 else None, "peak": red_peak,
-                                   "frac": (red_lanes / (k_t * 1e-3) / red_peak) if (k_t > 0 and red_peak > 0) else None,
+                                   "achieved": ach, "peak": red_pack, "frac": (ach / red_pack) if (ach and red_pack > 0) else None,
+                                   "scattered_rate": red_scat, "frac_of_scattered_rate": (ach / red_scat) if (ach and red_scat > 0) else None,
                                    "algorithmic": f"{RED_PER_SAMPLE} reductions per sample (cell crossings of the marched rays, ncu inst count) x {n_samples:.4g} samples",
-                                   "peak_source": "oat_measure_red_rate(): scattered red.global.add.v4.f32 into an L2-resident 64 MB buffer, same run"}
+                                   "peak_source": "oat_measure_red_rate_ex(pattern 1): red.global.add.v4.f32, the 32 lanes of a warp filling 16 sectors of an L2-resident "
+                                                  "64 MB buffer (the cost of a reduction is per distinct sector); scattered_rate = oat_measure_red_rate(): every lane its own sector; same run"}
         except Exception as ex:
             roofline["limiter"] = {"error": str(ex)}
         # H requests one 32-byte cell record from L2 per cell run of a ray; the peak is the measured scattered-sector rate

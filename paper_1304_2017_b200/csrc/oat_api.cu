@@ -51,7 +51,7 @@ struct oat_geometry {
     unsigned long long *d_patches = nullptr;  // schedule 1 work items (lazy)
     int *d_q_count = nullptr, *d_q_done = nullptr;
     unsigned long long patch_cap = 0;
-    int morton_shift = 4;                     // patches are sorted by the Morton code of (centre >> shift)
+    int morton_shift = 6;                     // patches are sorted by the Morton code of (centre >> shift): 64-voxel cells (measured best of 2..10)
     int schedule = 1;                         // 0 = ring-major chunks, 1 = Morton-sorted patches
     long long *d_item_prefix = nullptr;
     // scratch

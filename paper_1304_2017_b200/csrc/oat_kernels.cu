@@ -457,7 +457,7 @@ __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const PEntry 
         const float om = e.a.w;
         float L0 = 0.f, L1 = 0.f, L2 = 0.f, L3 = 0.f, H0 = 0.f, H1 = 0.f, H2 = 0.f, H3 = 0.f;
         float pr0 = 0.f, pr1 = 0.f, pr2 = 0.f;             // never equal to a rounded coordinate (those are >= 2^22)
-        float4 *cur = qb;
+        unsigned cur = 0;                                  // record index within orientation o (32-bit: one IMAD.WIDE per reduction)
         bool valid = false;
         // 8 steps per trip of a rolled loop: the fully unrolled body (32 x ~60 instructions) missed the instruction
         // cache (ncu: 21 % of the stall samples were "no instruction"); kbase + kj is exact (half-integers)
@@ -474,8 +474,8 @@ __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const PEntry 
             const bool c0 = r0 != pr0;
             const bool carry = (!c12) & (r0 == pr0 + 1.0f);    // one cell forward along the dominant axis only
             const bool full = c12 | (c0 & !carry);
-            red_add_v4_if(cur, L0, L1, L2, L3, valid & (c0 | c12));
-            red_add_v4_if(cur + sa, H0, H1, H2, H3, valid & full);
+            red_add_v4_if(qb + cur, L0, L1, L2, L3, valid & (c0 | c12));
+            red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid & full);
             L0 = full ? 0.f : (carry ? H0 : L0); L1 = full ? 0.f : (carry ? H1 : L1);
             L2 = full ? 0.f : (carry ? H2 : L2); L3 = full ? 0.f : (carry ? H3 : L3);
             const bool zh = full | carry;
@@ -483,7 +483,7 @@ __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const PEntry 
             pr0 = r0; pr1 = r1; pr2 = r2;
             const int i0 = __float_as_int(r0) + b0, i1 = __float_as_int(r1) + b1, i2 = __float_as_int(r2) + b2;
             valid = ((unsigned)i0 <= n0) & ((unsigned)i1 <= n1) & ((unsigned)i2 <= n2);
-            cur = qb + ((i0 * nc + i2) * nb + i1);
+            cur = (unsigned)((i0 * nc + i2) * nb + i1);
             const float f0 = t0 - (r0 - OAT_MAGIC), f1 = t1 - (r1 - OAT_MAGIC), f2 = t2 - (r2 - OAT_MAGIC);
             const float cwk = cp[k] * om;
             const float cw = valid ? cwk : 0.f;
@@ -494,8 +494,8 @@ __device__ __forceinline__ void consume_march_bwd(const OatDev &P, const PEntry 
             H0 = fmaf(q0, wh, H0); H1 = fmaf(q1, wh, H1); H2 = fmaf(q2, wh, H2); H3 = fmaf(q3, wh, H3);
           }
         }
-        red_add_v4_if(cur, L0, L1, L2, L3, valid);
-        red_add_v4_if(cur + sa, H0, H1, H2, H3, valid);
+        red_add_v4_if(qb + cur, L0, L1, L2, L3, valid);
+        red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid);
     }
 }
 
