@@ -37,9 +37,9 @@ RED_PER_SAMPLE = 0.63
 SECTORS_PER_SAMPLE = 0.435
 # B200 fp32 peak derived from unit counts and clocks (guide: 148 SMs x 128 fp32 lanes x 2 flop x max SM clock)
 N_SM, FP32_LANES = 148, 128
-# DRAM bytes (read + write) per in-box sample of the dominant kernel (H^T) from the ncu --set full capture in
-# profiles/r1d_ncu_full.md: (1.689 + 1.190) GB for 2.478e10 samples on the 512-transducer subset of config 3.
-DRAM_BYTES_PER_SAMPLE_HT = (1.688615e9 + 1.190443e9) / 2.4784424365e10
+# DRAM bytes (read + write) per in-box sample of the dominant kernel (H^T) from the ncu --set full capture summarised in
+# profiles/r1k_final.md: (1.825 + 1.335) GB for 2.478e10 samples on the 512-transducer subset of config 3.
+DRAM_BYTES_PER_SAMPLE_HT = (1.824808e9 + 1.335234e9) / 2.4784424365e10
 
 
 def peaks():
@@ -267,7 +267,7 @@ def run_ours(args):
                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak else None,
                     "traffic": (DRAM_BYTES_PER_SAMPLE_HT * n_samples) if dom == "backproject" else None,
                     "traffic_note": "dram__bytes_read+write of oat_march_kernel<1> per launch, ncu --set full on the 512-transducer subset "
-                                    "(profiles/r1d_ncu_full.md) scaled by samples; unit B; algorithmic unique bytes = size(x)+size(y)",
+                                    "(profiles/r1k_final.md) scaled by samples; unit B; algorithmic unique bytes = size(x)+size(y)",
                     "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_step if ms_step else None,
                     "peak_source": f"148 SM x 128 fp32 lanes x 2 flop x {peak_src}",
                     "algorithmic": f"{FLOP_PER_SAMPLE:.0f} fp32 flop per interpolation sample x {n_samples:.4g} samples per launch",
