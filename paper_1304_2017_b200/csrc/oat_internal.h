@@ -33,7 +33,7 @@
 #define OAT_MLH 512
 #endif
 #ifndef OAT_MLT
-#define OAT_MLT 512
+#define OAT_MLT 1024
 #endif
 
 struct OatBand {

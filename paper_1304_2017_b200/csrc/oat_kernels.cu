@@ -754,8 +754,13 @@ __device__ __forceinline__ bool make_entry_tab(const OatDev &P, const OatBand &b
     return hit;
 }
 
+// H^T: 6 resident blocks (80 registers, no spills) with the whole patch in one build/consume round (OAT_MLT = 1024):
+// 86.2 -> 85.4 ms on the config-3 subset; H keeps 8 blocks and two rounds (it is sensitive to occupancy and to L1 size)
+#ifndef OAT_MBLKT
+#define OAT_MBLKT 6
+#endif
 template <int MODE, int ML>
-__global__ void __launch_bounds__(OAT_MT, OAT_MBLK)
+__global__ void __launch_bounds__(OAT_MT, MODE == 0 ? OAT_MBLK : OAT_MBLKT)
 oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__restrict__ faces, float *__restrict__ y_out,
                  const float *__restrict__ coef, double *__restrict__ g)
 {
