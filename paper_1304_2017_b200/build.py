@@ -16,7 +16,7 @@ from pathlib import Path
 
 CSRC = Path(__file__).resolve().parent / "csrc"
 LIB = CSRC / "liboat.so"
-SOURCES = ["oat_api.cu", "oat_kernels.cu"]
+SOURCES = ["oat_api.cu", "oat_kernels.cu", "oat_march.cu"]
 HEADERS = ["oat_internal.h", "../../include/oat.h"]
 
 NVCC_FLAGS = [

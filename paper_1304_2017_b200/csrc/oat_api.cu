@@ -65,7 +65,7 @@ struct oat_geometry {
     float4 *d_faces = nullptr;                // face-quad accumulators of the 3 orientations (backproject variant 4, lazy)
     size_t n_faces = 0;                       // float4 records, 0 = variant unavailable for this grid
     float4 *d_cells = nullptr;                // per-cell polynomial records (project variant 4, lazy)
-    size_t n_cells = 0;                       // records incl. the trailing all-zero one (2 float4 each)
+    size_t n_cells = 0;                       // records incl. the zero margin (2 float4 each)
     double *d_g = nullptr;                    // Q*K SRT accumulator
     float *d_y2 = nullptr, *d_x2 = nullptr;   // adjoint check / CGLS / host entry points (lazy)
     float *d_x3 = nullptr, *d_y3 = nullptr, *d_x4 = nullptr;   // CGLS vectors (lazy)
@@ -306,10 +306,12 @@ int build_geometry(oat_geometry *G)
     P.qx = (d.nx + 2) / 2 + 1; P.qy = (d.ny + 2) / 2 + 1;
     P.qplane = (long long)P.qx * P.qy;
     P.oz = (d.nz + 2) / 2 + 1;
-    P.cx = ((d.nx + 1 + 3) / 4) * 4; P.cy = d.ny + 1;      // 4 records = one 128-byte line
+    // cell records with a zero margin: a ray is kept when the bounding box of its 32-sample segment meets the padded box,
+    // so its samples lie within 31 * step cells of it (+ the cull's 0.01 slack and one cell for floor)
+    P.cm = (int)ceil(31.0 * P.step) + 3;
+    P.cx = ((d.nx + 1 + 2 * P.cm + 3) / 4) * 4; P.cy = d.ny + 1 + 2 * P.cm; P.cz = d.nz + 1 + 2 * P.cm;   // 4 records = one 128-byte line
     P.cxy = (long long)P.cx * P.cy;
-    if ((unsigned long long)(d.nz + 1) * (unsigned long long)P.cxy + 1 >= (1ULL << 31)) P.cx = 0;   // variant 4 unavailable
-    else P.zero_cell = (unsigned)((long long)(d.nz + 1) * P.cxy);
+    if (P.step > 8.0 || (unsigned long long)P.cz * (unsigned long long)P.cxy >= (1ULL << 31)) P.cx = 0;    // marching H unavailable
     {   // face-quad accumulators: orientation a = x, y, z with in-plane axes (b, c) = (y,z), (z,x), (x,y)
         const long long nn[3] = {d.nx, d.ny, d.nz};
         long long tot = 0;
@@ -322,7 +324,7 @@ int build_geometry(oat_geometry *G)
         }
         G->n_faces = ok ? (size_t)tot : 0;
     }
-    G->n_cells = P.cx ? (size_t)(d.nz + 1) * (size_t)P.cxy + 1 : 0;
+    G->n_cells = P.cx ? (size_t)P.cz * (size_t)P.cxy : 0;
     {   // packed list entries: anchor node offsets in [-128, 895] (anchor = band midpoint, at most 16 samples outside the padded box)
         const int nmax = d.nx > d.ny ? (d.nx > d.nz ? d.nx : d.nz) : (d.ny > d.nz ? d.ny : d.nz);
         G->march_ok = (16.0 * P.step + 4.0 <= 128.0) && (nmax + 2 + 16.0 * P.step + 4.0 <= 895.0);

@@ -79,9 +79,10 @@ struct OatDev {
     int qx, qy;                // quad layout (variant 2): quads per row / rows per plane
     long long qplane;          // qx*qy; one parity array holds pz*qplane float4 quads
     int oz;                    // octet layout (project variant 3): bricks along z; 8 arrays of oz*qplane records of 32 B
-    int cx, cy;                // cell-record layout (variant 4): cells per row (pitch, multiple of 4) / rows per plane
-    long long cxy;             // cx*cy; record of padded cell (ix,iy,iz) = (iz*cy + iy)*cx + ix, 32 B each
-    unsigned zero_cell;        // index of an all-zero record (samples outside the padded box read / add into it)
+    int cx, cy, cz;            // cell-record layout (marching H): cells per row (pitch, multiple of 4) / rows per plane / planes,
+    int cm;                    // each = nodes + 1 + 2 cm: a zero margin of cm cells around the padded box, wide enough for every
+                               // sample of every ray whose segment meets the box (no per-sample bounds test)
+    long long cxy;             // cx*cy; record of padded cell (ix,iy,iz) = ((iz+cm)*cy + iy+cm)*cx + ix+cm, 32 B each
     // face-quad accumulators (backproject variant 4): orientation o = axis a normal to the quad, in-plane axes
     // (b, c) = (y,z), (z,x), (x,y) for a = x, y, z; record (ia, ib, ic) = float4 of padded nodes
     // {(ib,ic),(ib+1,ic),(ib,ic+1),(ib+1,ic+1)} on plane ia, at f_base[o] + (ia*f_nc[o] + ic)*f_nb[o] + ib

@@ -343,178 +343,6 @@ __device__ __forceinline__ void consume_march(const OatDev &P, const Entry *__re
     }
 }
 
-// CONSUME for H, "marching" form (project variant 4, B = 32): one THREAD per ray, stepping through the
-// band's 32 time samples in order.
-//   position   t_k = fma(u*step, k - 15.5, anchor)   (same fp64 anchor as every other variant; the
-//              immediate-operand FMA keeps one rounding at |t| < ~6 voxels)
-//   cell       floor by the round-down magic add; the cell's 32-byte record (8 polynomial coefficients of
-//              the trilinear interpolant, see oat_pad_cells_kernel) is (re)loaded with a PREDICATED 256-bit
-//              load only when the ray has entered a new cell -- ~2-3 samples share one load, and the L1
-//              data stage sees ~0.45 loads per sample instead of 8 scalar gathers
-//   value      7 FMAs (Horner in fx, fy, fz) instead of 7 lerps = 14 ops
-// acc[k] holds the thread's sum over its rays for sample k; the caller transposes/reduces over the warp.
-// Measured dead ends (B200, config-3 subset): two rays interleaved per thread, an L1 prefetch (CCTL.PF1) of the
-// next step's record, unconditional reloads, register double-buffering of the next record (ptxas hoists all 32
-// loads and spills) and cp.async staging through shared memory (LDGSTS of scattered 16-byte pieces is ~4x slower)
-// are all slower than this form at 8 resident 128-thread blocks per SM.  So are a depth-1 software pipeline of the
-// record load (8 selects per step), two rays interleaved per thread on 16 accumulators, and 6 or 5 resident blocks
-// with more registers: the kernel time does not react to occupancy or to loads in flight because it sits at the
-// rate at which an SM's L1 can send sector misses to L2 (ncu: l1tex__m_l1tex2xbar_req_cycles_active 51 %, 0.46
-// sectors per SM-cycle, L1 hit rate 5 % by construction -- every record is used by exactly one ray).  Fetching the 8
-// corner values with two predicated texture gathers (tld4 from the slice atlas) instead of the record load: 122 ms
-// against 79.5 ms.  Splitting the block into independent warp pairs with their own lists and 64-thread named
-// barriers (so that one pair's build overlaps the other's marching): 74.1 ms against 70.8 ms; two rays per thread
-// again, now with the larger L1: 85.6 ms (6 blocks, no spills).
-__device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
-{
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
-        "@p ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"   // a record is used by one ray only
-        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]), "+f"(c[4]), "+f"(c[5]), "+f"(c[6]), "+f"(c[7])
-        : "l"(p), "r"((int)pred));
-}
-
-// The 32 samples are split into two halves of 16 (K0 = 0 or 16), marched by different warps: 16 accumulators
-// per thread fit the 64-register budget of 8 resident blocks per SM (32 spilled to local memory: ncu showed
-// 0.8 LDL + 0.8 STL per warp-step and 30 % of the L2 traffic), at the price of one extra record load per ray.
-template <int NT, int K0>
-__device__ __forceinline__ void consume_march_fwd(const OatDev &P, const PEntry *__restrict__ list, int n_list, int tid,
-                                                  const float4 *__restrict__ cells, float (&acc)[16])
-{
-    const float stepf = (float)P.step;
-    for (int ei = tid; ei < n_list; ei += NT) {
-        const Entry e = unpack_entry(list[ei]);
-        const float sx = e.u.x * stepf, sy = e.u.y * stepf, sz = e.u.z * stepf;
-        float prx = 0.f, pry = 0.f, prz = 0.f;            // previous step's rounded coordinates (cell identity);
-                                                          // 0 never equals a rounded coordinate (those are >= 2^22)
-        float c[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) c[i] = 0.f;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            const float kk = (float)(K0 + k) - 15.5f;
-            const float tx = fmaf(sx, kk, e.a.x), ty = fmaf(sy, kk, e.a.y), tz = fmaf(sz, kk, e.a.z);
-            const float rx = __fadd_rd(tx, OAT_MAGIC), ry = __fadd_rd(ty, OAT_MAGIC), rz = __fadd_rd(tz, OAT_MAGIC);
-            const bool ch = (rx != prx) | (ry != pry) | (rz != prz);
-            prx = rx; pry = ry; prz = rz;
-            const int ix = __float_as_int(rx) + e.i.x, iy = __float_as_int(ry) + e.i.y, iz = __float_as_int(rz) + e.i.z;
-            // padded cell n' in [0, N] <=> xi in [-1, N): the sample touches at least one existing node (S4)
-            const bool in = ((unsigned)ix <= (unsigned)P.nx) & ((unsigned)iy <= (unsigned)P.ny) & ((unsigned)iz <= (unsigned)P.nz);
-            const unsigned idx = in ? (unsigned)((iz * P.cy + iy) * P.cx + ix) : P.zero_cell;
-            ldg256_if(c, cells + 2 * (size_t)idx, ch);
-            const float fx = tx - (rx - OAT_MAGIC), fy = ty - (ry - OAT_MAGIC), fz = tz - (rz - OAT_MAGIC);
-            const float lo = fmaf(fy, fmaf(fx, c[3], c[2]), fmaf(fx, c[1], c[0]));
-            const float hi = fmaf(fy, fmaf(fx, c[7], c[6]), fmaf(fx, c[5], c[4]));
-            acc[k] = fmaf(e.a.w, fmaf(fz, hi, lo), acc[k]);
-        }
-    }
-}
-
-// CONSUME for H^T, face-carrying marching form (backproject variant 4, B = 32).  H^T is bound by the rate at
-// which an SM can retire vector reductions (~1.5 SM-cycles per RED.128 lane on scattered sectors, measured), so
-// the aim is FEWER reductions per sample, not fewer instructions:
-//   * one THREAD per ray, local axis 0 = the ray's dominant axis a (|u_a| largest), marched in the direction in
-//     which the ray ADVANCES along a (the 32 samples are walked backwards when u_a < 0; positions are identical
-//     because fma(-s, -kk, anchor) == fma(s, kk, anchor));
-//   * the 8 corner weights of the current cell are accumulated as two quads, L on plane i_a and H on plane
-//     i_a + 1, laid out as the face-quad records of orientation a (OatDev::f_base);
-//   * when the ray steps to the next cell along a only, the finished quad L is retired with ONE reduction and H
-//     is carried over as the new L; only a step across one of the two minor axes flushes both quads.
-// About 0.65 reductions per sample instead of 0.9 for the z-only quads of variant 3.  Same positions, cells and
-// weights as consume_march_fwd, so H and H^T visit identical samples (Eq. 12 vs Eq. 23).
-
-__device__ __forceinline__ void red_add_v4_if(float4 *addr, float a, float b, float c, float d, bool pred)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t@p red.global.add.v4.f32 [%0], {%1,%2,%3,%4};\n\t}"
-                 ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d), "r"((int)pred) : "memory");
-}
-
-template <int NT>
-__device__ __forceinline__ void consume_march_bwd(const OatDev &P, const PEntry *__restrict__ list, int n_list, int tid,
-                                                  const float *__restrict__ s_coef, float4 *__restrict__ faces)
-{
-    const float stepf = (float)P.step;
-    for (int ei = tid; ei < n_list; ei += NT) {
-        const Entry e = unpack_entry(list[ei]);
-        const float mx = fabsf(e.u.x), my = fabsf(e.u.y), mz = fabsf(e.u.z);
-        const int o = (mx >= my && mx >= mz) ? 0 : (my >= mz ? 1 : 2);
-        // local axes (0, 1, 2) = (a, b, c) = (x,y,z), (y,z,x), (z,x,y)
-        const float a0 = o == 0 ? e.a.x : o == 1 ? e.a.y : e.a.z, a1 = o == 0 ? e.a.y : o == 1 ? e.a.z : e.a.x,
-                    a2 = o == 0 ? e.a.z : o == 1 ? e.a.x : e.a.y;
-        const float u0 = o == 0 ? e.u.x : o == 1 ? e.u.y : e.u.z, u1 = o == 0 ? e.u.y : o == 1 ? e.u.z : e.u.x,
-                    u2 = o == 0 ? e.u.z : o == 1 ? e.u.x : e.u.y;
-        const int b0 = o == 0 ? e.i.x : o == 1 ? e.i.y : e.i.z, b1 = o == 0 ? e.i.y : o == 1 ? e.i.z : e.i.x,
-                  b2 = o == 0 ? e.i.z : o == 1 ? e.i.x : e.i.y;
-        const unsigned n0 = o == 0 ? P.nx : o == 1 ? P.ny : P.nz, n1 = o == 0 ? P.ny : o == 1 ? P.nz : P.nx,
-                       n2 = o == 0 ? P.nz : o == 1 ? P.nx : P.ny;
-        const int nb = o == 0 ? P.f_nb[0] : o == 1 ? P.f_nb[1] : P.f_nb[2];
-        const int nc = o == 0 ? P.f_nc[0] : o == 1 ? P.f_nc[1] : P.f_nc[2];
-        float4 *const qb = faces + (o == 0 ? P.f_base[0] : o == 1 ? P.f_base[1] : P.f_base[2]);
-        const int sa = nb * nc;                            // records per plane
-        const bool flip = u0 < 0.f;
-        const float sg = flip ? -stepf : stepf;
-        const float s0 = u0 * sg, s1 = u1 * sg, s2 = u2 * sg;   // s0 >= 0: the ray advances along local axis 0
-        const float *cp = s_coef + (flip ? 32 : 0);        // [0,32): coef_k, [32,64): coef_{31-k}
-        const float om = e.a.w;
-        float L0 = 0.f, L1 = 0.f, L2 = 0.f, L3 = 0.f, H0 = 0.f, H1 = 0.f, H2 = 0.f, H3 = 0.f;
-        float pr0 = 0.f, pr1 = 0.f, pr2 = 0.f;             // never equal to a rounded coordinate (those are >= 2^22)
-        unsigned cur = 0;                                  // record index within orientation o (32-bit: one IMAD.WIDE per reduction)
-        bool valid = false;
-        // 8 steps per trip of a rolled loop: the fully unrolled body (32 x ~60 instructions) missed the instruction
-        // cache (ncu: 21 % of the stall samples were "no instruction"); kbase + kj is exact (half-integers)
-#pragma unroll 1
-        for (int kb = 0; kb < 32; kb += OAT_BU) {
-          const float kbase = (float)kb - 15.5f;
-#pragma unroll
-          for (int kj = 0; kj < OAT_BU; ++kj) {
-            const int k = kb + kj;
-            const float kk = kbase + (float)kj;
-            const float t0 = fmaf(s0, kk, a0), t1 = fmaf(s1, kk, a1), t2 = fmaf(s2, kk, a2);
-            const float r0 = __fadd_rd(t0, OAT_MAGIC), r1 = __fadd_rd(t1, OAT_MAGIC), r2 = __fadd_rd(t2, OAT_MAGIC);
-            const bool c12 = (r1 != pr1) | (r2 != pr2);
-            const bool c0 = r0 != pr0;
-            const bool carry = (!c12) & (r0 == pr0 + 1.0f);    // one cell forward along the dominant axis only
-            const bool full = c12 | (c0 & !carry);
-            red_add_v4_if(qb + cur, L0, L1, L2, L3, valid & (c0 | c12));
-            red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid & full);
-            L0 = full ? 0.f : (carry ? H0 : L0); L1 = full ? 0.f : (carry ? H1 : L1);
-            L2 = full ? 0.f : (carry ? H2 : L2); L3 = full ? 0.f : (carry ? H3 : L3);
-            const bool zh = full | carry;
-            H0 = zh ? 0.f : H0; H1 = zh ? 0.f : H1; H2 = zh ? 0.f : H2; H3 = zh ? 0.f : H3;
-            pr0 = r0; pr1 = r1; pr2 = r2;
-            const int i0 = __float_as_int(r0) + b0, i1 = __float_as_int(r1) + b1, i2 = __float_as_int(r2) + b2;
-            valid = ((unsigned)i0 <= n0) & ((unsigned)i1 <= n1) & ((unsigned)i2 <= n2);
-            cur = (unsigned)((i0 * nc + i2) * nb + i1);
-            const float f0 = t0 - (r0 - OAT_MAGIC), f1 = t1 - (r1 - OAT_MAGIC), f2 = t2 - (r2 - OAT_MAGIC);
-            const float cwk = cp[k] * om;
-            const float cw = valid ? cwk : 0.f;
-            const float e1 = 1.f - f1, e2 = 1.f - f2;
-            const float q0 = e1 * e2, q1 = f1 * e2, q2 = e1 * f2, q3 = f1 * f2;
-            const float wh = cw * f0, wl = cw - wh;
-            L0 = fmaf(q0, wl, L0); L1 = fmaf(q1, wl, L1); L2 = fmaf(q2, wl, L2); L3 = fmaf(q3, wl, L3);
-            H0 = fmaf(q0, wh, H0); H1 = fmaf(q1, wh, H1); H2 = fmaf(q2, wh, H2); H3 = fmaf(q3, wh, H3);
-          }
-        }
-        red_add_v4_if(qb + cur, L0, L1, L2, L3, valid);
-        red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid);
-    }
-}
-
-// sum acc[k] over the 32 lanes of the warp; lanes l and l + 16 return the total of sample k = l (16 shuffles)
-__device__ __forceinline__ float warp_transpose_sum(float (&acc)[16], int lane)
-{
-#pragma unroll
-    for (int s = 8; s >= 1; s >>= 1) {
-        const bool up = (lane & s) != 0;
-#pragma unroll
-        for (int i = 0; i < s; ++i) {
-            const float send = up ? acc[i] : acc[i + s];
-            const float keep = up ? acc[i + s] : acc[i];
-            acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, s);
-        }
-    }
-    return acc[0] + __shfl_xor_sync(0xffffffffu, acc[0], 16);
-}
-
 // EPILOGUE of one work item: cross-warp combine in fp64 and one fp64 atomic per time sample (S5)
 template <int MODE>
 __device__ __forceinline__ void item_epilogue(const OatDev &P, int q, const LaneCtx &L, float acc, unsigned cnt, int warp, int lane,
@@ -714,178 +542,6 @@ oat_patch_kernel(const OatDev P, const float *__restrict__ xpad, float *__restri
             }
         }
         __syncthreads();
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// Marching kernels (variant 4, B = 32): the patch schedule with everything that is not the per-sample
-// loop trimmed -- small blocks (OAT_MT threads, 8 resident per SM) so that the dependent loads at the top
-// of a patch overlap other blocks' marching; directions from the fp64 table instead of sincospi; the
-// adjoint time stencil precomputed per (q,k) by oat_coef_kernel; a patch's 32 rings built and consumed in
-// rounds of ML / 32 rings (16 KB of packed list entries per block).
-// ------------------------------------------------------------------------------------------------
-#ifndef OAT_MBLK
-#define OAT_MBLK 8
-#endif
-
-// same result as make_entry(), direction taken from the table: (dlx, dly) = sin(theta_i) (cos phi_j, sin phi_j)
-__device__ __forceinline__ bool make_entry_tab(const OatDev &P, const OatBand &band, double2 d, double ct, float omega,
-                                               const double *s_frame, Entry &e)
-{
-    float uu[3], af[3];
-    int ai[3];
-    bool hit = true;
-    const float lim[3] = {(float)P.nx + 1.01f, (float)P.ny + 1.01f, (float)P.nz + 1.01f};
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const double ua = d.x * s_frame[a] + d.y * s_frame[3 + a] + ct * s_frame[6 + a];
-        const double an = s_frame[9 + a] + band.s_mid * ua;
-        const double ar = rint(an);
-        uu[a] = (float)ua;
-        af[a] = (float)(an - ar);
-        ai[a] = (int)ar;
-        const float p0 = (float)(s_frame[9 + a] + (double)band.s_lo * ua);
-        const float p1 = (float)(s_frame[9 + a] + (double)band.s_hi * ua);
-        hit = hit && (fmaxf(p0, p1) >= -0.01f) && (fminf(p0, p1) <= lim[a]);
-    }
-    e.a = make_float4(af[0], af[1], af[2], omega);
-    e.u = make_float4(uu[0], uu[1], uu[2], 0.f);
-    e.i = make_int4(ai[0] - OAT_MAGIC_BITS, ai[1] - OAT_MAGIC_BITS, ai[2] - OAT_MAGIC_BITS, 0);
-    return hit;
-}
-
-// H^T: 6 resident blocks (80 registers, no spills) with the whole patch in one build/consume round (OAT_MLT = 1024):
-// 86.2 -> 85.4 ms on the config-3 subset; H keeps 8 blocks and two rounds (it is sensitive to occupancy and to L1 size)
-#ifndef OAT_MBLKT
-#define OAT_MBLKT 6
-#endif
-template <int MODE, int ML>
-__global__ void __launch_bounds__(OAT_MT, MODE == 0 ? OAT_MBLK : OAT_MBLKT)
-oat_march_kernel(const OatDev P, const float4 *__restrict__ cells, float4 *__restrict__ faces, float *__restrict__ y_out,
-                 const float *__restrict__ coef, double *__restrict__ g)
-{
-    __shared__ PEntry list[ML];
-    __shared__ double s_frame[12];
-    __shared__ float s_red[OAT_MT / 32][16];
-    __shared__ float s_coef[64];
-    constexpr int NR = (OAT_RI + ML / OAT_RJ - 1) / (ML / OAT_RJ);   // build/consume rounds per patch
-    __shared__ int s_count[NR];
-    __shared__ int s_flag;
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (long long item = blockIdx.x; item < P.n_patches; item += gridDim.x) {
-        int q, b, rb, sec;
-        unpack_item(P.patches[item], q, b, rb, sec);
-        if (tid < 12) s_frame[tid] = P.frame[(size_t)q * 12 + tid];
-        if (tid < NR) s_count[tid] = 0;
-        const OatBand band = P.band[b];
-        const OatRing *__restrict__ ring = P.ring + band.ring_ofs;
-        const double2 *__restrict__ dir = P.dir + band.dir_ofs;
-        const int r0 = rb * OAT_RI;
-        const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
-        const int S = P.rb_sectors[band.rb_ofs + rb];
-        if (MODE == 1 && warp == 0) {                      // B1: the band's 32 coefficients g'_k rho_k^2, forward and reversed
-            const float cf = lane < band.nk ? coef[(size_t)q * P.K + band.k0 + lane] : 0.f;
-            s_coef[lane] = cf;
-            s_coef[63 - lane] = cf;
-            const bool any = __any_sync(0xffffffffu, cf != 0.f);
-            if (lane == 0) s_flag = any ? 1 : 0;
-        }
-        float a16[16];                                     // MODE 0: warps [0, NW/2) march samples 0..15, the rest 16..31
-        if (MODE == 0) {
-#pragma unroll
-            for (int i = 0; i < 16; ++i) a16[i] = 0.f;
-        }
-        __syncthreads();
-        // a band whose 32 data values give g' = 0 contributes exactly nothing to H^T y
-        const bool live = (MODE != 1) || (s_flag != 0);
-        for (int rc = r0, round = 0; live && rc < r1; rc += ML / OAT_RJ, ++round) {
-            // ---------------------------------------------------------------- build (A2: directions -> ray anchors)
-            const int re = min(rc + ML / OAT_RJ, r1);
-            // The two table loads of a ray (ring -> direction) are dependent L2 round trips; several rays per trip keep
-            // them in flight together.  H: all 4 rays of the thread at once (67.9 -> 65.0 ms on the config-3
-            // subset); H^T, which has fewer registers to spare: two per trip (88.4 -> 86.2 ms; four: 88.0 ms).
-            if (MODE == 0) {
-            {   // all of the thread's rays of this round at once: ring loads, then direction loads, then the entries
-                constexpr int NB = ML / OAT_MT;
-                int cumj[NB]; bool ok[NB]; double ctv[NB]; float omv[NB];
-                const int jl = tid % OAT_RJ;
-#pragma unroll
-                for (int i = 0; i < NB; ++i) {
-                    const int r = rc + (tid + i * OAT_MT) / OAT_RJ;
-                    ok[i] = r < re;
-                    const OatRing R = ring[ok[i] ? r : rc];
-                    const int j0 = (int)(((long long)R.N * sec + S - 1) / S), j1 = (int)(((long long)R.N * (sec + 1) + S - 1) / S);
-                    ok[i] = ok[i] && (j0 + jl < j1);
-                    cumj[i] = R.cum + (ok[i] ? j0 + jl : 0); ctv[i] = R.ct; omv[i] = R.omega;
-                }
-                double2 dv[NB];
-#pragma unroll
-                for (int i = 0; i < NB; ++i) dv[i] = dir[cumj[i]];
-#pragma unroll
-                for (int i = 0; i < NB; ++i) {
-                    Entry e;
-                    if (ok[i] && make_entry_tab(P, band, dv[i], ctv[i], omv[i], s_frame, e)) list[atomicAdd(&s_count[round], 1)] = pack_entry(e);
-                }
-            }
-            } else {
-            // two rays per trip: the two dependent table loads (ring -> direction) of both are in flight together
-            for (int t = tid; t < ML; t += 2 * OAT_MT) {
-                const int ra = rc + t / OAT_RJ, rb2 = rc + (t + OAT_MT) / OAT_RJ, jl = t % OAT_RJ;   // OAT_MT is a multiple of OAT_RJ
-                const bool va = ra < re, vb = rb2 < re;
-                if (!va) break;
-                const OatRing Ra = ring[ra];
-                const OatRing Rb = ring[vb ? rb2 : ra];
-                const int ja0 = (int)(((long long)Ra.N * sec + S - 1) / S), ja1 = (int)(((long long)Ra.N * (sec + 1) + S - 1) / S);
-                const int jb0 = (int)(((long long)Rb.N * sec + S - 1) / S), jb1 = (int)(((long long)Rb.N * (sec + 1) + S - 1) / S);
-                const bool oa = ja0 + jl < ja1, ob = vb && (jb0 + jl < jb1);
-                const double2 da = dir[Ra.cum + (oa ? ja0 + jl : 0)];
-                const double2 db = dir[Rb.cum + (ob ? jb0 + jl : 0)];
-                Entry e;
-                if (oa && make_entry_tab(P, band, da, Ra.ct, Ra.omega, s_frame, e)) list[atomicAdd(&s_count[round], 1)] = pack_entry(e);
-                if (ob && make_entry_tab(P, band, db, Rb.ct, Rb.omega, s_frame, e)) list[atomicAdd(&s_count[round], 1)] = pack_entry(e);
-            }
-            }
-            __syncthreads();
-            // ---------------------------------------------------------------- consume (A3 / B2-B3)
-            if (MODE == 0) {
-                if (tid < OAT_MT / 2) consume_march_fwd<OAT_MT / 2, 0>(P, list, s_count[round], tid, cells, a16);
-                else consume_march_fwd<OAT_MT / 2, 16>(P, list, s_count[round], tid - OAT_MT / 2, cells, a16);
-            } else consume_march_bwd<OAT_MT>(P, list, s_count[round], tid, s_coef, faces);
-            __syncthreads();                               // the list is rebuilt by the next round / item
-        }
-        if (MODE == 0) {
-            // S5: warp sums -> fp64 cross-warp combine -> one fp64 atomic per time sample
-            const float tot = warp_transpose_sum(a16, lane);
-            if (lane < 16) s_red[warp][lane] = tot;
-            __syncthreads();
-            if (warp == 0) {
-                double sum = 0.0;                          // lane = sample k of the band; its half's warps hold the partial sums
-#pragma unroll
-                for (int w = 0; w < OAT_MT / 64; ++w) sum += (double)s_red[(lane >> 4) * (OAT_MT / 64) + w][lane & 15];
-                const int k = band.k0 + lane;
-                const double rho = P.c * (P.t0 + (double)k * P.dt);
-                if (lane < band.nk && rho > 0.0 && sum != 0.0) atomicAdd(&g[(size_t)q * P.K + k], rho * rho * sum);
-                // Fused step A4 (Eq. 3 L63 / Eq. 13): the block that completes the LAST patch of transducer q turns
-                // the finished fp64 row g[q,:] into pressure.  Every lane fences its own atomics, one lane counts.
-                __threadfence();
-                __syncwarp();
-                if (lane == 0) s_flag = (atomicAdd(&P.q_done[q], 1) + 1 == P.q_count[q]) ? 1 : 0;
-            }
-            __syncthreads();
-            if (s_flag) {
-                __threadfence();
-                const double *gq = g + (size_t)q * P.K;
-                float *yq = y_out + (size_t)q * P.K;
-                for (int k = tid; k < P.K; k += OAT_MT) {
-                    double sp = 0.0, sm = 0.0;
-                    if (k + 1 < P.K) { const double t = P.t0 + (double)(k + 1) * P.dt; if (t > 0.0) sp = __ldcg(gq + k + 1) / t; }
-                    if (k - 1 >= 0) { const double t = P.t0 + (double)(k - 1) * P.dt; if (t > 0.0) sm = __ldcg(gq + k - 1) / t; }
-                    yq[k] = (float)(P.kappa * (sp - sm) / (2.0 * P.dt));
-                }
-            }
-        }
-        __syncthreads();                                   // s_flag, s_red, s_coef reused by the next item
     }
 }
 
@@ -1129,34 +785,6 @@ __global__ void oat_pad_octs_kernel(const OatDev P, const float *__restrict__ x,
         }
         octs[2 * i] = make_float4(v[0], v[1], v[2], v[3]);
         octs[2 * i + 1] = make_float4(v[4], v[5], v[6], v[7]);
-    }
-}
-
-// cell records from x (variant 4): record of padded cell (X,Y,Z), X in [0,nx] etc. (corner nodes X-1..X in real
-// indices, zero outside the grid = reading G5), holds the coefficients of the cell's trilinear polynomial
-//   A(fx,fy,fz) = c0 + c1 fx + c2 fy + c3 fx fy + fz (c4 + c5 fx + c6 fy + c7 fx fy)        (Eq. 10 L110 expanded)
-// computed in fp64 from the 8 corner values and rounded once to fp32.
-__global__ void oat_pad_cells_kernel(const OatDev P, const float *__restrict__ x, float4 *__restrict__ cells)
-{
-    const long long n = (long long)(P.nz + 1) * P.cxy;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i <= n; i += (long long)gridDim.x * blockDim.x) {
-        double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        if (i < n) {
-            const int X = (int)(i % P.cx);
-            const long long r = i / P.cx;
-            const int Y = (int)(r % P.cy), Z = (int)(r / P.cy);
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const int xx = X - 1 + (k & 1), yy = Y - 1 + ((k >> 1) & 1), zz = Z - 1 + (k >> 2);
-                if (xx >= 0 && xx < P.nx && yy >= 0 && yy < P.ny && zz >= 0 && zz < P.nz)
-                    v[k] = (double)x[((size_t)zz * P.ny + yy) * P.nx + xx];
-            }
-        }                                                  // i == n: the all-zero record (P.zero_cell)
-        const double c1 = v[1] - v[0], c2 = v[2] - v[0], c4 = v[4] - v[0];
-        const double c3 = v[3] - v[2] - c1, c5 = v[5] - v[4] - c1, c6 = v[6] - v[4] - c2;
-        const double c7 = v[7] - v[6] - (v[5] - v[4]) - c3;
-        cells[2 * i] = make_float4((float)v[0], (float)c1, (float)c2, (float)c3);
-        cells[2 * i + 1] = make_float4((float)c4, (float)c5, (float)c6, (float)c7);
     }
 }
 
@@ -1544,12 +1172,6 @@ void oat_launch_pad_octs(const OatDev &P, const float *x, float4 *octs, cudaStre
     oat_pad_octs_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, octs);
 }
 
-void oat_launch_pad_cells(const OatDev &P, const float *x, float4 *cells, cudaStream_t st)
-{
-    const long long n = (long long)(P.nz + 1) * P.cxy + 1;
-    oat_pad_cells_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, x, cells);
-}
-
 void oat_launch_unface(const OatDev &P, const float4 *faces, float *x, cudaStream_t st)
 {
     const long long n = (long long)P.nx * P.ny * P.nz;
@@ -1605,17 +1227,6 @@ static cudaError_t launch_patch_t(const OatDev &P, const float *xpad, float *xac
     const long long cap = 0x7fffffffLL;
     const unsigned grid = (unsigned)(P.n_patches < cap ? P.n_patches : cap);
     oat_patch_kernel<MODE, VAR><<<grid, OAT_NT, smem, st>>>(P, xpad, xacc, y, g, counter);
-    return cudaGetLastError();
-}
-
-cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, float4 *faces, float *y_out,
-                             const float *coef, double *g, cudaStream_t st)
-{
-    if (P.n_patches <= 0) return cudaSuccess;
-    const long long cap = 0x7fffffffLL;
-    const unsigned grid = (unsigned)(P.n_patches < cap ? P.n_patches : cap);
-    if (mode == 0) oat_march_kernel<0, OAT_MLH><<<grid, OAT_MT, 0, st>>>(P, cells, faces, y_out, coef, g);
-    else oat_march_kernel<1, OAT_MLT><<<grid, OAT_MT, 0, st>>>(P, cells, faces, y_out, coef, g);
     return cudaGetLastError();
 }
 
