@@ -55,7 +55,7 @@ __device__ __forceinline__ void unpack_item(unsigned long long v, int &q, int &b
 // Direction (S3) of table entry d = sin(theta_i) (cos phi_j, sin phi_j) in the frame of the transducer, and the
 // ray's anchor point base' + s_mid*u, all in fp64; returns false when the bounding box of the ray segment
 // [s_lo, s_hi] cannot meet the padded node box.
-__device__ __forceinline__ bool make_ray(const OatDev &P, const OatBand &band, double2 d, double ct, float omega, float stepf,
+__device__ __forceinline__ bool make_ray(const OatDev &P, double2 d, double ct, float omega, float stepf,
                                          const double *s_frame, Ray &e)
 {
     float uu[3], af[3];
@@ -65,13 +65,13 @@ __device__ __forceinline__ bool make_ray(const OatDev &P, const OatBand &band, d
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double ua = d.x * s_frame[a] + d.y * s_frame[3 + a] + ct * s_frame[6 + a];
-        const double an = s_frame[9 + a] + band.s_mid * ua;
+        const double an = s_frame[9 + a] + s_frame[12] * ua;      // s_frame[12..14] = the band's s_mid, s_lo, s_hi
         const double ar = rint(an);
         uu[a] = (float)ua;
         af[a] = (float)(an - ar);
         ai[a] = (int)ar;
-        const float p0 = (float)(s_frame[9 + a] + (double)band.s_lo * ua);
-        const float p1 = (float)(s_frame[9 + a] + (double)band.s_hi * ua);
+        const float p0 = (float)(s_frame[9 + a] + s_frame[13] * ua);
+        const float p1 = (float)(s_frame[9 + a] + s_frame[14] * ua);
         hit = hit && (fmaxf(p0, p1) >= -0.01f) && (fminf(p0, p1) <= lim[a]);
     }
     e.ax = af[0]; e.ay = af[1]; e.az = af[2];
@@ -100,10 +100,15 @@ __device__ __forceinline__ void fill_ring_rows(const OatRing *__restrict__ ring,
     s_ring[lane] = row;
 }
 
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+#ifndef OAT_LDHINT
+#define OAT_LDHINT ".L1::no_allocate"
+#endif
 __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
-        "@p ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"   // a record is used by one ray only
+        "@p ld.global.nc" OAT_LDHINT ".v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"   // a record is used by one ray only
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]), "+f"(c[4]), "+f"(c[5]), "+f"(c[6]), "+f"(c[7])
         : "l"(p), "r"((int)pred));
 }
@@ -131,21 +136,42 @@ __device__ __forceinline__ float half_warp_transpose_sum(float (&acc)[16], int l
 }
 
 // ------------------------------------------------------------------------------------------------
-// H (projection).  A ring row (<= 32 rays, lane = azimuth) is marched in two passes of 16 rays by all 32 lanes: lanes
-// 0..15 take samples 0..15 of ray p*16 + l, lanes 16..31 samples 31..16 of the same ray walked BACKWARDS with the
-// direction negated -- fma(-s, -kk, a) == fma(s, kk, a), so both halves run the same instruction stream with the same
-// immediates kk = k' - 15.5 and the positions are bit-identical to a forward walk.  16 accumulators per lane
-// (sample k' of the lower half, 31 - k' of the upper) fit the 64-register budget of 8 resident blocks per SM.
+// Per-warp ray queue.  Only ~45 % of a patch's 1024 candidate directions survive the box cull (patches on the faces of
+// the volume), so rays are compacted before they are marched: the lanes that built a surviving ray append it to a small
+// ring buffer in shared memory owned by their warp (ballot + popc give the slot; no atomics, no block barrier), and the
+// warp marches full groups from the front.  The buffers are the only sizeable shared memory of a block (6 KB for H), so
+// the L1 carve-out stays at 64 KB per SM.
+// ------------------------------------------------------------------------------------------------
+// queue entry = two float4 kept in separate arrays (16-byte stride: conflict-free LDS.128 / STS.128):
+//   a = anchor fraction (x, y, z), omega;  s = direction * step (x, y, z), then H: record-index constant K,
+//   H^T: packed anchor node offsets
+
+#define OAT_PB 128   // bias of the 10-bit packed anchor node offsets (H^T): offsets in [-128, 895], checked at create
+
+// ------------------------------------------------------------------------------------------------
+// H (projection).  A group of 16 queued rays is marched by all 32 lanes: lanes 0..15 take samples 0..15 of ray l,
+// lanes 16..31 samples 31..16 of the same ray walked BACKWARDS with the direction negated -- fma(-s, -kk, a) ==
+// fma(s, kk, a), so both halves run the same instruction stream with the same immediates kk = k' - 15.5 and the
+// positions are bit-identical to a forward walk.  16 accumulators per lane (sample k' of the lower half, 31 - k' of the
+// upper) fit the 64-register budget of 8 resident blocks per SM.
 // Per step: 3 FFMA (position), 3 FADD.RM (floor), 1 IADD + 2 IMAD (record index), 1 ISETP (new cell?), 1 IMAD.WIDE,
 // 1 predicated 256-bit load of the cell's polynomial record -- only when the ray has entered a new cell, ~2.2 samples
 // share one load --, 6 FADD (fractions), 7 FFMA (Horner in fx, fy, fz) + 1 FFMA (quadrature weight): 26 instructions.
 // The records carry a zero margin of P.cm cells around the padded box, so no sample needs a bounds test.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(OAT_MT, 8)
+#ifndef OAT_NRH
+#define OAT_NRH 1     // rays marched together by one lane: their record loads are in flight at the same time
+#endif
+#define OAT_QNH (16 * OAT_NRH + 32)    // queue entries per warp: at most 16 NRH - 1 left over + 32 new
+#ifndef OAT_MBLKH
+#define OAT_MBLKH (OAT_NRH == 1 ? 1024 / OAT_MT : 768 / OAT_MT)
+#endif
+__global__ void __launch_bounds__(OAT_MT, OAT_MBLKH)
 oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__restrict__ y_out, double *__restrict__ g)
 {
-    __shared__ double s_frame[12];
+    __shared__ double s_frame[16];
     __shared__ RingRow s_ring[OAT_RI];
+    __shared__ float4 s_qa[OAT_MT / 32][OAT_QNH], s_qs[OAT_MT / 32][OAT_QNH];
     __shared__ float s_red[OAT_MT / 32][32];
     __shared__ int s_flag;
 
@@ -154,11 +180,14 @@ oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__
     const unsigned cx = (unsigned)P.cx, cxy = (unsigned)P.cxy;
     const unsigned kbias = (unsigned)P.cm - OAT_MAGIC_BITS;            // per axis: + margin - bias of the magic add
     const unsigned k_zero = 0u - OAT_MAGIC_BITS * (cxy + cx + 1u);     // ray (a = 0, s = 0) -> record 0 (all zero)
+    const unsigned lt_mask = (1u << lane) - 1u;
+    float4 *const qa = s_qa[warp], *const qs = s_qs[warp];
     for (long long item = blockIdx.x; item < P.n_patches; item += gridDim.x) {
         int q, b, rb, sec;
         unpack_item(P.patches[item], q, b, rb, sec);
         if (tid < 12) s_frame[tid] = P.frame[(size_t)q * 12 + tid];
         const OatBand band = P.band[b];
+        if (tid == 32) { s_frame[12] = band.s_mid; s_frame[13] = (double)band.s_lo; s_frame[14] = (double)band.s_hi; }
         const double2 *__restrict__ dir = P.dir;
         const int r0 = rb * OAT_RI;
         const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
@@ -167,51 +196,81 @@ oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__
 #pragma unroll
         for (int i = 0; i < 16; ++i) acc[i] = 0.f;
         __syncthreads();
-        // the direction of the NEXT ring row is loaded while the current one is marched
-        double2 dn = make_double2(0.0, 0.0);
-        if (warp < OAT_RI) { const RingRow rw = s_ring[warp]; if (lane < rw.nj) dn = dir[rw.dofs + lane]; }
+        // the directions of the NEXT ring row are prefetched into L1 while the current one is built and marched
+        { const RingRow rw = s_ring[warp]; if (lane < rw.nj) prefetch_l1(dir + rw.dofs + lane); }
+        int head = 0, cnt = 0;                                 // warp-uniform: first queued entry, number queued
 #pragma unroll 1
-        for (int rr = warp; rr < OAT_RI; rr += OAT_MT / 32) {
-            const RingRow row = s_ring[rr];
-            const double2 d = dn;
-            if (rr + OAT_MT / 32 < OAT_RI) { const RingRow rw = s_ring[rr + OAT_MT / 32]; if (lane < rw.nj) dn = dir[rw.dofs + lane]; }
-            if (row.nj <= 0) continue;                          // warp-uniform
-            Ray e;
-            bool ok = lane < row.nj;
-            ok = make_ray(P, band, d, row.ct, row.omega, stepf, s_frame, e) && ok;
-            unsigned K = ((unsigned)e.iz + kbias) * cxy + ((unsigned)e.iy + kbias) * cx + ((unsigned)e.ix + kbias);
-            if (!ok) { e.ax = e.ay = e.az = 0.f; e.sx = e.sy = e.sz = 0.f; e.om = 0.f; K = k_zero; }
-            const unsigned okm = __ballot_sync(0xffffffffu, ok);
+        for (int rr = warp;; rr += OAT_MT / 32) {
+            const bool last = rr >= OAT_RI;
+            if (!last) {
+                // ------------------------------------------------------------ build (A2: direction -> ray anchor)
+                const RingRow row = s_ring[rr];
+                if (rr + OAT_MT / 32 < OAT_RI) { const RingRow rw = s_ring[rr + OAT_MT / 32]; if (lane < rw.nj) prefetch_l1(dir + rw.dofs + lane); }
+                if (row.nj > 0) {                               // warp-uniform
+                    Ray e;
+                    bool ok = lane < row.nj;
+                    const double2 d = dir[row.dofs + (ok ? lane : 0)];
+                    ok = make_ray(P, d, row.ct, row.omega, stepf, s_frame, e) && ok;
+                    const unsigned m = __ballot_sync(0xffffffffu, ok);
+                    if (ok) {
+                        int slot = head + cnt + __popc(m & lt_mask);
+                        if (slot >= OAT_QNH) slot -= OAT_QNH;
+                        const unsigned K = ((unsigned)e.iz + kbias) * cxy + ((unsigned)e.iy + kbias) * cx + ((unsigned)e.ix + kbias);
+                        qa[slot] = make_float4(e.ax, e.ay, e.az, e.om);
+                        qs[slot] = make_float4(e.sx, e.sy, e.sz, __uint_as_float(K));
+                    }
+                    cnt += __popc(m);
+                    __syncwarp();
+                }
+            }
+            // ---------------------------------------------------------------- march (A3): groups of 16 * OAT_NRH rays
 #pragma unroll 1
-            for (int pass = 0; pass < 2; ++pass) {
-                if (((okm >> (16 * pass)) & 0xffffu) == 0u) continue;   // warp-uniform
-                const int src = pass * 16 + (lane & 15);
-                const float ax = __shfl_sync(0xffffffffu, e.ax, src), ay = __shfl_sync(0xffffffffu, e.ay, src),
-                            az = __shfl_sync(0xffffffffu, e.az, src), om = __shfl_sync(0xffffffffu, e.om, src);
-                float sx = __shfl_sync(0xffffffffu, e.sx, src), sy = __shfl_sync(0xffffffffu, e.sy, src),
-                      sz = __shfl_sync(0xffffffffu, e.sz, src);
-                const unsigned Kr = __shfl_sync(0xffffffffu, K, src);
-                if (lane >= 16) { sx = -sx; sy = -sy; sz = -sz; }
-                float c[8];
+            while (cnt >= 16 * OAT_NRH || (last && cnt > 0)) {
+                const int n = min(cnt, 16 * OAT_NRH);
+                float ax[OAT_NRH], ay[OAT_NRH], az[OAT_NRH], om[OAT_NRH], sx[OAT_NRH], sy[OAT_NRH], sz[OAT_NRH];
+                unsigned Kr[OAT_NRH], prev[OAT_NRH];
+                float c[OAT_NRH][8];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) c[i] = 0.f;
-                unsigned prev = 0xffffffffu;                    // never a record index (those are < 2^31)
+                for (int r = 0; r < OAT_NRH; ++r) {
+                    const int li = (lane & 15) + 16 * r;
+                    int slot = head + li;
+                    if (slot >= OAT_QNH) slot -= OAT_QNH;
+                    float4 ea = make_float4(0.f, 0.f, 0.f, 0.f), es = make_float4(0.f, 0.f, 0.f, __uint_as_float(k_zero));
+                    if (li < n) { ea = qa[slot]; es = qs[slot]; }
+                    ax[r] = ea.x; ay[r] = ea.y; az[r] = ea.z; om[r] = ea.w;
+                    sx[r] = lane >= 16 ? -es.x : es.x; sy[r] = lane >= 16 ? -es.y : es.y; sz[r] = lane >= 16 ? -es.z : es.z;
+                    Kr[r] = __float_as_uint(es.w);
+                    prev[r] = 0xffffffffu;                      // never a record index (those are < 2^31)
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) c[r][i] = 0.f;
+                }
+                __syncwarp();                                   // the slots may be refilled by the next build
+                head += n; if (head >= OAT_QNH) head -= OAT_QNH;
+                cnt -= n;
 #pragma unroll
                 for (int k = 0; k < 16; ++k) {
                     const float kk = (float)k - 15.5f;
-                    const float tx = fmaf(sx, kk, ax), ty = fmaf(sy, kk, ay), tz = fmaf(sz, kk, az);
-                    const float rx = __fadd_rd(tx, OAT_MAGIC), ry = __fadd_rd(ty, OAT_MAGIC), rz = __fadd_rd(tz, OAT_MAGIC);
-                    const unsigned idx = __float_as_uint(rz) * cxy + (__float_as_uint(ry) * cx + (__float_as_uint(rx) + Kr));
-                    const bool ch = idx != prev;
-                    prev = idx;
-                    ldg256_if(c, cells + 2 * (size_t)idx, ch);
-                    const float fx = tx - (rx - OAT_MAGIC), fy = ty - (ry - OAT_MAGIC), fz = tz - (rz - OAT_MAGIC);
-                    // record = (c0, c4, c1, c5, c2, c6, c3, c7) of A = c0 + c1 fx + c2 fy + c3 fx fy + fz (c4 + c5 fx + c6 fy + c7 fx fy)
-                    const float lo = fmaf(fy, fmaf(fx, c[6], c[4]), fmaf(fx, c[2], c[0]));
-                    const float hi = fmaf(fy, fmaf(fx, c[7], c[5]), fmaf(fx, c[3], c[1]));
-                    acc[k] = fmaf(om, fmaf(fz, hi, lo), acc[k]);
+                    float tx[OAT_NRH], ty[OAT_NRH], tz[OAT_NRH], rx[OAT_NRH], ry[OAT_NRH], rz[OAT_NRH];
+#pragma unroll
+                    for (int r = 0; r < OAT_NRH; ++r) {         // the loads of the lane's rays are in flight together
+                        tx[r] = fmaf(sx[r], kk, ax[r]); ty[r] = fmaf(sy[r], kk, ay[r]); tz[r] = fmaf(sz[r], kk, az[r]);
+                        rx[r] = __fadd_rd(tx[r], OAT_MAGIC); ry[r] = __fadd_rd(ty[r], OAT_MAGIC); rz[r] = __fadd_rd(tz[r], OAT_MAGIC);
+                        const unsigned idx = __float_as_uint(rz[r]) * cxy + (__float_as_uint(ry[r]) * cx + (__float_as_uint(rx[r]) + Kr[r]));
+                        const bool ch = idx != prev[r];
+                        prev[r] = idx;
+                        ldg256_if(c[r], cells + 2 * (size_t)idx, ch);
+                    }
+#pragma unroll
+                    for (int r = 0; r < OAT_NRH; ++r) {
+                        const float fx = tx[r] - (rx[r] - OAT_MAGIC), fy = ty[r] - (ry[r] - OAT_MAGIC), fz = tz[r] - (rz[r] - OAT_MAGIC);
+                        // record = (c0, c4, c1, c5, c2, c6, c3, c7) of A = c0 + c1 fx + c2 fy + c3 fx fy + fz (c4 + c5 fx + c6 fy + c7 fx fy)
+                        const float lo = fmaf(fy, fmaf(fx, c[r][6], c[r][4]), fmaf(fx, c[r][2], c[r][0]));
+                        const float hi = fmaf(fy, fmaf(fx, c[r][7], c[r][5]), fmaf(fx, c[r][3], c[r][1]));
+                        acc[k] = fmaf(om[r], fmaf(fz, hi, lo), acc[k]);
+                    }
                 }
             }
+            if (last) break;
         }
         // S5: half-warp sums -> fp64 cross-warp combine -> one fp64 atomic per time sample
         const float tot = half_warp_transpose_sum(acc, lane);
@@ -249,31 +308,36 @@ oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__
 // ------------------------------------------------------------------------------------------------
 // H^T (backprojection), face-carrying form.  H^T is bound by the rate at which vector reductions retire in L2
 // (~1.5 SM-cycles per RED.128 lane on scattered sectors, measured), so the aim is FEWER reductions per sample:
-//   * one lane per ray, local axis 0 = the ray's dominant axis a (|u_a| largest), marched in the direction in which
-//     the ray ADVANCES along a (backwards in k when u_a < 0; positions are identical, see above);
+//   * one lane per queued ray, local axis 0 = the ray's dominant axis a (|u_a| largest), marched in the direction in
+//     which the ray ADVANCES along a (backwards in k when u_a < 0; positions are identical, see above);
 //   * the 8 corner weights of the current cell are accumulated as two quads, L on plane i_a and H on plane i_a + 1,
 //     laid out as the face-quad records of orientation a (OatDev::f_base);
-//   * when the ray steps to the next cell along a only, the finished quad L is retired with ONE reduction and H is
-//     carried over as the new L; only a step across one of the two minor axes flushes both quads.
+//   * when the ray steps to the next cell along a only (record index + one plane), the finished quad L is retired with
+//     ONE reduction and H is carried over as the new L; any other cell change flushes both quads.
 // ------------------------------------------------------------------------------------------------
 #ifndef OAT_MBLKT
-#define OAT_MBLKT 6
+#define OAT_MBLKT 8
 #endif
+#define OAT_QNT 64    // queue entries per warp: at most 31 left over + 32 new
 __global__ void __launch_bounds__(OAT_MT, OAT_MBLKT)
 oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__restrict__ coef)
 {
-    __shared__ double s_frame[12];
+    __shared__ double s_frame[16];
     __shared__ RingRow s_ring[OAT_RI];
+    __shared__ float4 s_qa[OAT_MT / 32][OAT_QNT], s_qs[OAT_MT / 32][OAT_QNT];
     __shared__ float s_coef[64];
     __shared__ int s_flag;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const float stepf = (float)P.step;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    float4 *const qa = s_qa[warp], *const qs = s_qs[warp];
     for (long long item = blockIdx.x; item < P.n_patches; item += gridDim.x) {
         int q, b, rb, sec;
         unpack_item(P.patches[item], q, b, rb, sec);
         if (tid < 12) s_frame[tid] = P.frame[(size_t)q * 12 + tid];
         const OatBand band = P.band[b];
+        if (tid == 32) { s_frame[12] = band.s_mid; s_frame[13] = (double)band.s_lo; s_frame[14] = (double)band.s_hi; }
         const double2 *__restrict__ dir = P.dir;
         const int r0 = rb * OAT_RI;
         const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
@@ -288,79 +352,100 @@ oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__
         __syncthreads();
         // a band whose 32 data values give g' = 0 contributes exactly nothing to H^T y
         if (s_flag != 0) {
-            double2 dn = make_double2(0.0, 0.0);
-            if (warp < OAT_RI) { const RingRow rw = s_ring[warp]; if (lane < rw.nj) dn = dir[rw.dofs + lane]; }
+            { const RingRow rw = s_ring[warp]; if (lane < rw.nj) prefetch_l1(dir + rw.dofs + lane); }
+            int head = 0, cnt = 0;
 #pragma unroll 1
-            for (int rr = warp; rr < OAT_RI; rr += OAT_MT / 32) {
-                const RingRow row = s_ring[rr];
-                const double2 d = dn;
-                if (rr + OAT_MT / 32 < OAT_RI) { const RingRow rw = s_ring[rr + OAT_MT / 32]; if (lane < rw.nj) dn = dir[rw.dofs + lane]; }
-                if (row.nj <= 0) continue;                      // warp-uniform
-                Ray e;
-                bool ok = lane < row.nj;
-                ok = make_ray(P, band, d, row.ct, row.omega, stepf, s_frame, e) && ok;
-                if (!__any_sync(0xffffffffu, ok)) continue;
-                if (!ok) { e.ax = e.ay = e.az = 0.f; e.sx = e.sy = e.sz = 0.f; e.ix = e.iy = e.iz = -1000; }   // never valid: no reduction
-                const float mx = fabsf(e.sx), my = fabsf(e.sy), mz = fabsf(e.sz);
-                const int o = (mx >= my && mx >= mz) ? 0 : (my >= mz ? 1 : 2);
-                // local axes (0, 1, 2) = (a, b, c) = (x,y,z), (y,z,x), (z,x,y)
-                const float a0 = o == 0 ? e.ax : o == 1 ? e.ay : e.az, a1 = o == 0 ? e.ay : o == 1 ? e.az : e.ax,
-                            a2 = o == 0 ? e.az : o == 1 ? e.ax : e.ay;
-                const float u0 = o == 0 ? e.sx : o == 1 ? e.sy : e.sz, u1 = o == 0 ? e.sy : o == 1 ? e.sz : e.sx,
-                            u2 = o == 0 ? e.sz : o == 1 ? e.sx : e.sy;
-                const int b0 = (o == 0 ? e.ix : o == 1 ? e.iy : e.iz) - (int)OAT_MAGIC_BITS, b1 = (o == 0 ? e.iy : o == 1 ? e.iz : e.ix) - (int)OAT_MAGIC_BITS,
-                          b2 = (o == 0 ? e.iz : o == 1 ? e.ix : e.iy) - (int)OAT_MAGIC_BITS;
-                const unsigned n0 = o == 0 ? P.nx : o == 1 ? P.ny : P.nz, n1 = o == 0 ? P.ny : o == 1 ? P.nz : P.nx,
-                               n2 = o == 0 ? P.nz : o == 1 ? P.nx : P.ny;
-                const int nb = o == 0 ? P.f_nb[0] : o == 1 ? P.f_nb[1] : P.f_nb[2];
-                const int nc = o == 0 ? P.f_nc[0] : o == 1 ? P.f_nc[1] : P.f_nc[2];
-                float4 *const qb = faces + (o == 0 ? P.f_base[0] : o == 1 ? P.f_base[1] : P.f_base[2]);
-                const int sa = nb * nc;                            // records per plane
-                const bool flip = u0 < 0.f;
-                const float s0 = flip ? -u0 : u0, s1 = flip ? -u1 : u1, s2 = flip ? -u2 : u2;   // s0 >= 0: the ray advances along local axis 0
-                const float *cp = s_coef + (flip ? 32 : 0);        // [0,32): coef_k, [32,64): coef_{31-k}
-                const float om = ok ? e.om : 0.f;
-                float L0 = 0.f, L1 = 0.f, L2 = 0.f, L3 = 0.f, H0 = 0.f, H1 = 0.f, H2 = 0.f, H3 = 0.f;
-                float pr0 = 0.f, pr1 = 0.f, pr2 = 0.f;             // never equal to a rounded coordinate (those are >= 2^22)
-                unsigned cur = 0;                                  // record index within orientation o
-                bool valid = false;
-                // 8 steps per trip of a rolled loop: the fully unrolled body missed the instruction cache
-#pragma unroll 1
-                for (int kb = 0; kb < 32; kb += OAT_BU) {
-                    const float kbase = (float)kb - 15.5f;
-#pragma unroll
-                    for (int kj = 0; kj < OAT_BU; ++kj) {
-                        const int k = kb + kj;
-                        const float kk = kbase + (float)kj;
-                        const float t0 = fmaf(s0, kk, a0), t1 = fmaf(s1, kk, a1), t2 = fmaf(s2, kk, a2);
-                        const float r0f = __fadd_rd(t0, OAT_MAGIC), r1f = __fadd_rd(t1, OAT_MAGIC), r2f = __fadd_rd(t2, OAT_MAGIC);
-                        const bool c12 = (r1f != pr1) | (r2f != pr2);
-                        const bool c0 = r0f != pr0;
-                        const bool carry = (!c12) & (r0f == pr0 + 1.0f);    // one cell forward along the dominant axis only
-                        const bool full = c12 | (c0 & !carry);
-                        red_add_v4_if(qb + cur, L0, L1, L2, L3, valid & (c0 | c12));
-                        red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid & full);
-                        L0 = full ? 0.f : (carry ? H0 : L0); L1 = full ? 0.f : (carry ? H1 : L1);
-                        L2 = full ? 0.f : (carry ? H2 : L2); L3 = full ? 0.f : (carry ? H3 : L3);
-                        const bool zh = full | carry;
-                        H0 = zh ? 0.f : H0; H1 = zh ? 0.f : H1; H2 = zh ? 0.f : H2; H3 = zh ? 0.f : H3;
-                        pr0 = r0f; pr1 = r1f; pr2 = r2f;
-                        const int i0 = __float_as_int(r0f) + b0, i1 = __float_as_int(r1f) + b1, i2 = __float_as_int(r2f) + b2;
-                        // padded cell n' in [0, N] <=> xi in [-1, N): the sample touches at least one existing node (S4)
-                        valid = ((unsigned)i0 <= n0) & ((unsigned)i1 <= n1) & ((unsigned)i2 <= n2);
-                        cur = (unsigned)((i0 * nc + i2) * nb + i1);
-                        const float f0 = t0 - (r0f - OAT_MAGIC), f1 = t1 - (r1f - OAT_MAGIC), f2 = t2 - (r2f - OAT_MAGIC);
-                        const float cwk = cp[k] * om;
-                        const float cw = valid ? cwk : 0.f;
-                        const float e1 = 1.f - f1, e2 = 1.f - f2;
-                        const float q0 = e1 * e2, q1 = f1 * e2, q2 = e1 * f2, q3 = f1 * f2;
-                        const float wh = cw * f0, wl = cw - wh;
-                        L0 = fmaf(q0, wl, L0); L1 = fmaf(q1, wl, L1); L2 = fmaf(q2, wl, L2); L3 = fmaf(q3, wl, L3);
-                        H0 = fmaf(q0, wh, H0); H1 = fmaf(q1, wh, H1); H2 = fmaf(q2, wh, H2); H3 = fmaf(q3, wh, H3);
+            for (int rr = warp;; rr += OAT_MT / 32) {
+                const bool last = rr >= OAT_RI;
+                if (!last) {
+                    const RingRow row = s_ring[rr];
+                    if (rr + OAT_MT / 32 < OAT_RI) { const RingRow rw = s_ring[rr + OAT_MT / 32]; if (lane < rw.nj) prefetch_l1(dir + rw.dofs + lane); }
+                    if (row.nj > 0) {                           // warp-uniform
+                        Ray e;
+                        bool ok = lane < row.nj;
+                        const double2 d = dir[row.dofs + (ok ? lane : 0)];
+                        ok = make_ray(P, d, row.ct, row.omega, stepf, s_frame, e) && ok;
+                        const unsigned m = __ballot_sync(0xffffffffu, ok);
+                        if (ok) {
+                            const int slot = (head + cnt + __popc(m & lt_mask)) & (OAT_QNT - 1);
+                            const unsigned pk = (unsigned)(e.ix + OAT_PB) | ((unsigned)(e.iy + OAT_PB) << 10) | ((unsigned)(e.iz + OAT_PB) << 20);
+                            qa[slot] = make_float4(e.ax, e.ay, e.az, e.om);
+                            qs[slot] = make_float4(e.sx, e.sy, e.sz, __uint_as_float(pk));
+                        }
+                        cnt += __popc(m);
+                        __syncwarp();
                     }
                 }
-                red_add_v4_if(qb + cur, L0, L1, L2, L3, valid);
-                red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid);
+#pragma unroll 1
+                while (cnt >= 32 || (last && cnt > 0)) {
+                    const int n = min(cnt, 32);
+                    const int slot = (head + lane) & (OAT_QNT - 1);
+                    float4 ea = make_float4(0.f, 0.f, 0.f, 0.f), es = make_float4(1.f, 0.f, 0.f, 0.f);
+                    if (lane < n) { ea = qa[slot]; es = qs[slot]; }
+                    __syncwarp();
+                    head = (head + n) & (OAT_QNT - 1);
+                    cnt -= n;
+                    const unsigned pk = __float_as_uint(es.w);
+                    // anchor node offsets with the bias of the magic add folded in; an idle lane (lane >= n) gets -10^6: never valid
+                    const int ex = lane < n ? (int)(pk & 1023u) - (int)(OAT_PB + OAT_MAGIC_BITS) : -1000000 - (int)OAT_MAGIC_BITS;
+                    const int ey = (int)((pk >> 10) & 1023u) - (int)(OAT_PB + OAT_MAGIC_BITS), ez = (int)((pk >> 20) & 1023u) - (int)(OAT_PB + OAT_MAGIC_BITS);
+                    const float mx = fabsf(es.x), my = fabsf(es.y), mz = fabsf(es.z);
+                    const int o = (mx >= my && mx >= mz) ? 0 : (my >= mz ? 1 : 2);
+                    // local axes (0, 1, 2) = (a, b, c) = (x,y,z), (y,z,x), (z,x,y)
+                    const float a0 = o == 0 ? ea.x : o == 1 ? ea.y : ea.z, a1 = o == 0 ? ea.y : o == 1 ? ea.z : ea.x,
+                                a2 = o == 0 ? ea.z : o == 1 ? ea.x : ea.y;
+                    const float u0 = o == 0 ? es.x : o == 1 ? es.y : es.z, u1 = o == 0 ? es.y : o == 1 ? es.z : es.x,
+                                u2 = o == 0 ? es.z : o == 1 ? es.x : es.y;
+                    const int b0 = o == 0 ? ex : o == 1 ? ey : ez, b1 = o == 0 ? ey : o == 1 ? ez : ex, b2 = o == 0 ? ez : o == 1 ? ex : ey;
+                    const unsigned n0 = o == 0 ? P.nx : o == 1 ? P.ny : P.nz, n1 = o == 0 ? P.ny : o == 1 ? P.nz : P.nx,
+                                   n2 = o == 0 ? P.nz : o == 1 ? P.nx : P.ny;
+                    const int nb = o == 0 ? P.f_nb[0] : o == 1 ? P.f_nb[1] : P.f_nb[2];
+                    const int nc = o == 0 ? P.f_nc[0] : o == 1 ? P.f_nc[1] : P.f_nc[2];
+                    float4 *const qb = faces + (o == 0 ? P.f_base[0] : o == 1 ? P.f_base[1] : P.f_base[2]);
+                    const int sa = nb * nc;                            // records per plane
+                    const bool flip = u0 < 0.f;
+                    const float s0 = flip ? -u0 : u0, s1 = flip ? -u1 : u1, s2 = flip ? -u2 : u2;   // s0 >= 0: the ray advances along local axis 0
+                    const float *cp = s_coef + (flip ? 32 : 0);        // [0,32): coef_k, [32,64): coef_{31-k}
+                    const float om = ea.w;
+                    float L0 = 0.f, L1 = 0.f, L2 = 0.f, L3 = 0.f, H0 = 0.f, H1 = 0.f, H2 = 0.f, H3 = 0.f;
+                    unsigned cur = 0;                                  // record index within orientation o (32-bit: one IMAD.WIDE per reduction)
+                    bool valid = false;
+                    // 8 steps per trip of a rolled loop: the fully unrolled body missed the instruction cache
+#pragma unroll 1
+                    for (int kb = 0; kb < 32; kb += OAT_BU) {
+                        const float kbase = (float)kb - 15.5f;
+#pragma unroll
+                        for (int kj = 0; kj < OAT_BU; ++kj) {
+                            const int k = kb + kj;
+                            const float kk = kbase + (float)kj;
+                            const float t0 = fmaf(s0, kk, a0), t1 = fmaf(s1, kk, a1), t2 = fmaf(s2, kk, a2);
+                            const float r0f = __fadd_rd(t0, OAT_MAGIC), r1f = __fadd_rd(t1, OAT_MAGIC), r2f = __fadd_rd(t2, OAT_MAGIC);
+                            const int i0 = __float_as_int(r0f) + b0, i1 = __float_as_int(r1f) + b1, i2 = __float_as_int(r2f) + b2;
+                            const unsigned nxt = (unsigned)((i0 * nc + i2) * nb + i1);
+                            const unsigned dcur = nxt - cur;
+                            const bool chg = dcur != 0u;
+                            const bool carry = dcur == (unsigned)sa;       // one cell forward along the dominant axis only
+                            red_add_v4_if(qb + cur, L0, L1, L2, L3, valid & chg);
+                            red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid & chg & !carry);
+                            L0 = chg ? (carry ? H0 : 0.f) : L0; L1 = chg ? (carry ? H1 : 0.f) : L1;
+                            L2 = chg ? (carry ? H2 : 0.f) : L2; L3 = chg ? (carry ? H3 : 0.f) : L3;
+                            H0 = chg ? 0.f : H0; H1 = chg ? 0.f : H1; H2 = chg ? 0.f : H2; H3 = chg ? 0.f : H3;
+                            cur = nxt;
+                            // padded cell n' in [0, N] <=> xi in [-1, N): the sample touches at least one existing node (S4)
+                            valid = ((unsigned)i0 <= n0) & ((unsigned)i1 <= n1) & ((unsigned)i2 <= n2);
+                            const float f0 = t0 - (r0f - OAT_MAGIC), f1 = t1 - (r1f - OAT_MAGIC), f2 = t2 - (r2f - OAT_MAGIC);
+                            const float cw = valid ? cp[k] * om : 0.f;
+                            const float e1 = 1.f - f1, e2 = 1.f - f2;
+                            const float q0 = e1 * e2, q1 = f1 * e2, q2 = e1 * f2, q3 = f1 * f2;
+                            const float wh = cw * f0, wl = cw - wh;
+                            L0 = fmaf(q0, wl, L0); L1 = fmaf(q1, wl, L1); L2 = fmaf(q2, wl, L2); L3 = fmaf(q3, wl, L3);
+                            H0 = fmaf(q0, wh, H0); H1 = fmaf(q1, wh, H1); H2 = fmaf(q2, wh, H2); H3 = fmaf(q3, wh, H3);
+                        }
+                    }
+                    red_add_v4_if(qb + cur, L0, L1, L2, L3, valid);
+                    red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid);
+                }
+                if (last) break;
             }
         }
         __syncthreads();                                   // s_frame, s_ring, s_coef, s_flag are reused by the next item
