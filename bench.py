@@ -339,7 +339,7 @@ def run_ours(args):
             from paper_1304_2017_b200 import workloads as wl2
             wb2, _ = workload(args)
             areas = wl2.patch_areas_arc(64, 144, 65.0) if (args.config == 3 and not args.subset) else wl2.patch_areas_equal(wb2.trans_xyz, wb2.centre)
-            wq = torch.from_numpy(wl2.fbp_weights(wb2, areas).astype(np.float32)).cuda()
+            wq = torch.from_numpy(oat.oat_fbp_weights(g, areas)).cuda()
             oat.oat_fbp(g, y, wq, xb); torch.cuda.synchronize()
             a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
             a.record(stream); oat.oat_fbp(g, y, wq, xb); b.record(stream); torch.cuda.synchronize()

@@ -142,6 +142,12 @@ int oat_pls_cg(oat_geometry *geom, const float *d_u, float *d_x, int n_iter, dou
  * pointers owned by the caller; asynchronous on the stream. */
 int oat_fbp(oat_geometry *geom, const float *d_p, const float *d_w, float *d_x, void *cuda_stream);
 
+/* The weights of Eq. (27) L221 from the patch areas dS_q of the transducers (reading G23):
+ *   w[q] = -dS_q / (4 pi^2 kappa c^3 dt R_q),  kappa = the descriptor's gain, R_q = |r_q - grid centre| (L203);
+ * for the paper's geometry dS_q = (R^s)^2 dtheta dphi sin(theta_q) gives the printed constant.  h_areas: HOST, Q doubles
+ * (read); h_w: HOST, Q floats (written).  No device work. */
+int oat_fbp_weights(const oat_geometry *geom, const double *h_areas, float *h_w);
+
 /* ---- Row NEXT-3: the spherical-voxel imaging model in the temporal frequency domain and its adjoint (Eq. 17-20
  * L137-161, Eq. 24; Algs. 7-12), for point-like transducers (Alg. 9 line 7; reading G28).
  * oat_sph_set: frequencies f_l = f0 + l df (MHz), l = 0..nf-1 (reading G27); h_he = HOST array of 2*nf floats, the EIR
@@ -162,37 +168,8 @@ int oat_sph_backproject(oat_geometry *geom, const float *d_u, float *d_x, void *
 int oat_sph_pls_cg(oat_geometry *geom, const float *d_u, float *d_x, int n_iter, double mu,
                    double *h_obj, double *h_grad, void *cuda_stream);
 
-/* Kernel-variant selection for measurements ("chosen by ncu", north_star).  key = "project" or
- * "backproject"; the meaning of `variant` is listed in DESIGN.md §5.  Unknown => OAT_ERR_INVALID. */
-int oat_set_variant(oat_geometry *geom, const char *key, int variant);
-
 /* Number of kernels the last oat_project / oat_backproject on this handle launched. */
 int oat_last_launch_count(const oat_geometry *geom);
-
-/* Device time (ms, CUDA events on the call's stream) of the dominant kernel of the last
- * oat_project / oat_backproject; synchronises that stream.  Negative if none was recorded. */
-float oat_last_kernel_ms(oat_geometry *geom);
-
-/* Measurement aid for the roofline of H^T: sustained rate, in lanes per second, at which
- * `device` retires 16-byte vector reductions (red.global.add.v4.f32) that hit distinct 32-byte sectors of an
- * L2-resident 64 MB buffer -- the unit that bounds the backprojection scatter (Alg. 6).  Allocates and
- * frees its own scratch, synchronises the device.  Negative return on error. */
-int oat_measure_red_rate(int device, double *lanes_per_s);
-
-/* Measurement aid for the roofline of H: sustained rate, in 32-byte sectors per second, at
- * which `device` serves scattered 256-bit loads (ld.global.nc.v8.f32, one distinct sector per lane) that miss L1
- * and hit an L2-resident 64 MB buffer -- the access of the projection's marching loop (one cell record per cell
- * run of a ray, Eq. 12 L121 / Alg. 4).  Allocates and frees its own scratch, synchronises the device. */
-int oat_measure_gather_rate(int device, double *sectors_per_s);
-
-/* Parametrised forms of the two probes, behind the tables of DESIGN.md section 5.3 (`python -m paper_1304_2017_b200.probe`).
- * oat_measure_gather_rate_ex: `lanes_active` of 32 lanes load one scattered sector each, ONE load in flight per warp (the
- * request shape of H's marching loop), 8 blocks of 128 threads per SM each holding `smem_kb_per_block` KB of (unused)
- * shared memory -- what is carved out for shared memory is taken from L1.
- * oat_measure_red_rate_ex: RED.128 with an address pattern within the warp: 0 every lane its own record, 1 32 consecutive
- * records (16 sectors), 2 one record per 128-byte line, 3 lane pairs sharing a sector, 4 four scattered lines of 8 records. */
-int oat_measure_gather_rate_ex(int device, int lanes_active, int smem_kb_per_block, double *sectors_per_s);
-int oat_measure_red_rate_ex(int device, int pattern, double *lanes_per_s);
 
 const char *oat_last_error(void);
 const char *oat_version(void);

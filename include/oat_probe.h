@@ -1,0 +1,54 @@
+/*
+ * oat_probe.h -- measurement aids of liboat.so.  NOT part of the product ABI (include/oat.h): nothing here is needed to
+ * use the operators, and nothing on the operator path calls these entry points.  They serve tests (forcing the generic
+ * kernel), bench.py (device time of the dominant kernel, reported diagnostics) and the micro-benchmark tables of
+ * DESIGN.md section 5.3.
+ */
+#ifndef OAT_PROBE_H
+#define OAT_PROBE_H
+
+#include "oat.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Kernel selection for tests and measurements.  key = "project" / "backproject": variant 4 = marching kernels (default,
+ * used when the geometry allows: B = 32, records indexable with 32 bits, c dt <= spacing), 0 = the generic patch kernel
+ * that otherwise serves as the fall-back.  key = "morton_shift": log2 of the cell size of the patch order (default 6).
+ * key = "record_limit_log2": pretend record indices have that many bits (tests of the automatic fall-back).
+ * Unknown key or value => OAT_ERR_INVALID. */
+int oat_set_variant(oat_geometry *geom, const char *key, int variant);
+
+/* 1 if the next oat_project (backproject = 0) / oat_backproject (backproject = 1) on this handle runs the marching
+ * kernel, 0 if it runs the generic patch kernel, negative on NULL. */
+int oat_uses_marching(const oat_geometry *geom, int backproject);
+
+/* Device time (ms, CUDA events on the call's stream) of the dominant kernel of the last
+ * oat_project / oat_backproject; synchronises that stream.  Negative if none was recorded. */
+float oat_last_kernel_ms(oat_geometry *geom);
+
+/* Sustained rate, in lanes per second, at which `device` retires 16-byte vector reductions (red.global.add.v4.f32)
+ * that hit distinct 32-byte sectors of an L2-resident 64 MB buffer -- the path the backprojection scatter uses
+ * (Alg. 6).  A diagnostic, not a roofline peak: neighbouring rays of H^T share sectors and can exceed it.
+ * Allocates and frees its own scratch, synchronises the device.  Negative return on error. */
+int oat_measure_red_rate(int device, double *lanes_per_s);
+
+/* Sustained rate, in 32-byte sectors per second, at which `device` serves scattered 256-bit loads
+ * (ld.global.nc.v8.f32, one distinct sector per lane) that miss L1 and hit an L2-resident 64 MB buffer -- the access
+ * of the projection's marching loop (one cell record per cell run of a ray, Eq. 12 L121 / Alg. 4). */
+int oat_measure_gather_rate(int device, double *sectors_per_s);
+
+/* Parametrised forms of the two probes (tables of DESIGN.md section 5.3).
+ * oat_measure_gather_rate_ex: `lanes_active` of 32 lanes load one scattered sector each, ONE load in flight per warp,
+ * 8 blocks of 128 threads per SM each holding `smem_kb_per_block` KB of (unused) shared memory -- what is carved out
+ * for shared memory is taken from L1.
+ * oat_measure_red_rate_ex: RED.128 with an address pattern within the warp: 0 every lane its own record, 1 32 consecutive
+ * records (16 sectors), 2 one record per 128-byte line, 3 lane pairs sharing a sector, 4 four scattered lines of 8 records. */
+int oat_measure_gather_rate_ex(int device, int lanes_active, int smem_kb_per_block, double *sectors_per_s);
+int oat_measure_red_rate_ex(int device, int pattern, double *lanes_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OAT_PROBE_H */

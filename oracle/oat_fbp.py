@@ -64,6 +64,14 @@ def fbp(w, p, weights):
     return fbp_points(w, p, weights, pts).reshape(w.nz, w.ny, w.nx)
 
 
+def weights(w, areas):
+    """Reading G23: w_q = -dS_q / (4 pi^2 kappa c0^3 dt R_q), the constant of Eq. (27) L221 with kappa = beta/(4 pi C_p)
+    (Eq. 3) and R_q = |r_q - centre| the radius of the measurement sphere (L203); `areas` = the patch areas dS_q."""
+    tr = np.asarray(w.trans_xyz, dtype=np.float64)
+    r = np.sqrt(np.sum((tr - np.asarray(w.centre, dtype=np.float64)) ** 2, axis=1))
+    return -np.asarray(areas, dtype=np.float64) / (4.0 * np.pi ** 2 * w.gain * w.c ** 3 * w.dt * r)
+
+
 def interval_margin(w, pts):
     """min over transducers of |k~ - nearest integer| at each point (M,): where it is below the rounding noise of k~
     (~1e-12) the choice of interval k = floor(k~) is a tie -- Eq. (27) is discontinuous across integer k~, both

@@ -19,8 +19,8 @@ EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
-    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_sph_set", "oat_sph_project", "oat_sph_backproject", "oat_sph_pls_cg",
-    "oat_last_launch_count", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_measure_gather_rate_ex", "oat_measure_red_rate_ex", "oat_last_error", "oat_version",
+    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_fbp_weights", "oat_sph_set", "oat_sph_project", "oat_sph_backproject", "oat_sph_pls_cg",
+    "oat_last_launch_count", "oat_uses_marching", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_measure_gather_rate_ex", "oat_measure_red_rate_ex", "oat_last_error", "oat_version",
 ]
 
 
@@ -76,6 +76,8 @@ def load():
     lib.oat_set_variant.restype = ctypes.c_int
     lib.oat_last_launch_count.argtypes = [vp]
     lib.oat_last_launch_count.restype = ctypes.c_int
+    lib.oat_uses_marching.argtypes = [vp, ctypes.c_int]
+    lib.oat_uses_marching.restype = ctypes.c_int
     lib.oat_last_kernel_ms.argtypes = [vp]
     lib.oat_last_kernel_ms.restype = ctypes.c_float
     lib.oat_last_error.restype = ctypes.c_char_p
@@ -274,6 +276,10 @@ def oat_set_variant(g, key: str, variant: int):
     _check(load().oat_set_variant(g.handle, key.encode(), int(variant)))
 
 
+def oat_uses_marching(g, backproject: bool = False) -> bool:
+    return bool(load().oat_uses_marching(g.handle, 1 if backproject else 0))
+
+
 def oat_last_launch_count(g) -> int:
     return int(load().oat_last_launch_count(g.handle))
 
@@ -364,6 +370,17 @@ def oat_fbp(g, p, weights, x=None, stream=None):
     _check(load().oat_fbp(g.handle, _dev_ptr(p, oat_num_samples(g), "p", g), _dev_ptr(weights, g.n_trans, "weights", g),
                           _dev_ptr(x, oat_num_voxels(g), "x", g), _stream(stream)))
     return x
+
+
+def oat_fbp_weights(g, areas) -> np.ndarray:
+    """The Q weights of Eq. (27) from the transducers' patch areas (host arrays)."""
+    a = np.ascontiguousarray(areas, dtype=np.float64)
+    if a.shape != (g.n_trans,):
+        raise OatError(OAT_ERR_INVALID, f"areas must have shape ({g.n_trans},)")
+    out = np.empty(g.n_trans, dtype=np.float32)
+    _check(load().oat_fbp_weights(g.handle, a.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                  out.ctypes.data_as(ctypes.POINTER(ctypes.c_float))))
+    return out
 
 
 # ---------------------------------------------------------------- row NEXT-3: spherical-voxel model (frequency domain)

@@ -12,19 +12,20 @@ import os
 import shutil
 import subprocess
 import sys
+import tempfile
+from concurrent.futures import ThreadPoolExecutor
 from pathlib import Path
 
 CSRC = Path(__file__).resolve().parent / "csrc"
 LIB = CSRC / "liboat.so"
-SOURCES = ["oat_api.cu", "oat_kernels.cu", "oat_march.cu"]
-HEADERS = ["oat_internal.h", "../../include/oat.h"]
+SOURCES = ["oat_api.cu", "oat_march.cu", "oat_kernels.cu", "oat_next.cu", "oat_probe.cu"]
+HEADERS = ["oat_internal.h", "../../include/oat.h", "../../include/oat_probe.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
     "--fmad=true",
     "-Xcompiler", "-fPIC",
-    "-shared",
 ]
 
 
@@ -46,13 +47,24 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return LIB
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", str(LIB)] + [str(CSRC / s) for s in SOURCES]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed building liboat.so")
+    nvcc = nvcc_path()
+    with tempfile.TemporaryDirectory(prefix="oat_build_") as tmp:
+        def compile_one(src):
+            obj = os.path.join(tmp, src.replace(".cu", ".o"))
+            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, str(CSRC / src)]
+            return obj, subprocess.run(cmd, capture_output=True, text=True)
+        with ThreadPoolExecutor(max_workers=len(SOURCES)) as pool:       # one nvcc per translation unit, in parallel
+            done = list(pool.map(compile_one, SOURCES))
+        for _, res in done:
+            if verbose or res.returncode != 0:
+                sys.stderr.write(res.stdout + res.stderr)
+        if any(res.returncode != 0 for _, res in done):
+            raise RuntimeError("nvcc failed building liboat.so")
+        res = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", str(LIB)] + [o for o, _ in done],
+                             capture_output=True, text=True)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError("nvcc failed linking liboat.so")
     return LIB
 
 

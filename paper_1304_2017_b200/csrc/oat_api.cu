@@ -2,6 +2,7 @@
 // per-transducer frames and per-band ring tables (step A1 of SURVEY.md §8(a)), scratch
 // management, and the operator entry points.  All hot work is in oat_kernels.cu.
 #include "../../include/oat.h"
+#include "../../include/oat_probe.h"
 #include "oat_internal.h"
 
 #include <math.h>
@@ -16,14 +17,7 @@ namespace {
 
 thread_local char g_err[512] = "";
 
-int fail(int code, const char *fmt, ...)
-{
-    va_list ap;
-    va_start(ap, fmt);
-    vsnprintf(g_err, sizeof(g_err), fmt, ap);
-    va_end(ap);
-    return code;
-}
+#define fail oat_fail
 
 #define CUDA_TRY(expr)                                                                          \
     do {                                                                                        \
@@ -37,6 +31,15 @@ const double kPi = 3.14159265358979323846;
 
 }  // namespace
 
+int oat_fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
 struct oat_geometry {
     oat_geometry_desc desc;
     int device = 0;
@@ -48,23 +51,17 @@ struct oat_geometry {
     OatRing *d_ring = nullptr;
     int *d_qb_rings = nullptr;
     int *d_rb_sectors = nullptr;
-    unsigned long long *d_patches = nullptr;  // schedule 1 work items (lazy)
+    unsigned long long *d_patches = nullptr;  // Morton-sorted work items (lazy)
     int *d_q_count = nullptr, *d_q_done = nullptr;
     unsigned long long patch_cap = 0;
     int morton_shift = 6;                     // patches are sorted by the Morton code of (centre >> shift): 64-voxel cells (measured best of 2..10)
-    int schedule = 1;                         // 0 = ring-major chunks, 1 = Morton-sorted patches
-    long long *d_item_prefix = nullptr;
     // scratch
-    float *d_xpad = nullptr;                  // padded volume (gather source / scatter target)
-    float4 *d_quads = nullptr;                // 4 parity-shifted quad arrays (variant 2, lazy)
-    size_t n_quads = 0;
-    float4 *d_octs = nullptr;                 // 8 parity-shifted octet arrays (project variant 3, lazy)
-    size_t n_octs = 0;                        // in float4 units
-    double2 *d_dir = nullptr;                 // direction table of the marching kernels (variant 4)
-    float *d_coef = nullptr;                  // Q*K adjoint coefficients g'_k rho_k^2 (backproject variant 4, lazy)
-    float4 *d_faces = nullptr;                // face-quad accumulators of the 3 orientations (backproject variant 4, lazy)
-    size_t n_faces = 0;                       // float4 records, 0 = variant unavailable for this grid
-    float4 *d_cells = nullptr;                // per-cell polynomial records (project variant 4, lazy)
+    float *d_xpad = nullptr;                  // padded volume (generic kernel: gather source / scatter target; lazy)
+    double2 *d_dir = nullptr;                 // direction table of the marching kernels
+    float *d_coef = nullptr;                  // Q*K adjoint coefficients g'_k rho_k^2 (marching H^T, lazy)
+    float4 *d_faces = nullptr;                // face-quad accumulators of the 3 orientations (marching H^T, lazy)
+    size_t n_faces = 0;                       // float4 records, 0 = marching H^T unavailable for this grid
+    float4 *d_cells = nullptr;                // per-cell polynomial records (marching H, lazy)
     size_t n_cells = 0;                       // records incl. the zero margin (2 float4 each)
     double *d_g = nullptr;                    // Q*K SRT accumulator
     float *d_y2 = nullptr, *d_x2 = nullptr;   // adjoint check / CGLS / host entry points (lazy)
@@ -80,15 +77,14 @@ struct oat_geometry {
     unsigned long long *d_counter = nullptr;
     double *h_scal = nullptr;                 // pinned mirror of d_scal
     long long n_surface_samples = -1;
-    int variant_project = 4, variant_backproject = 4;   // measured best
-    bool march_ok = false;                    // ray anchors fit the 10-bit packed offsets of the marching kernels' list
-    cudaArray_t atlas = nullptr;              // slice atlas for the texture-gather projection (lazy)
-    cudaTextureObject_t tex = 0;
-    cudaSurfaceObject_t surf = 0;
+    int variant_project = 4, variant_backproject = 4;   // 4 = marching kernels, 0 = generic patch kernel (oat_probe.h)
+    bool march_ok = false;                    // ray anchors fit the 10-bit packed offsets of the marching H^T queue, step <= 1
+    size_t record_limit = (size_t)1 << 31;    // the marching kernels index records with 32 bits (lowered only by tests)
     int last_launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool ev_valid = false;
     size_t n_vox = 0, n_dat = 0, n_pad = 0;
+    std::vector<double> h_rq;                 // |r_q - grid centre| per transducer (mm), for oat_fbp_weights
 };
 
 namespace {
@@ -97,13 +93,10 @@ void free_all(oat_geometry *g)
 {
     if (!g) return;
     cudaFree(g->d_frame); cudaFree(g->d_band); cudaFree(g->d_ring); cudaFree(g->d_qb_rings);
-    cudaFree(g->d_item_prefix); cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
+    cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
     cudaFree(g->d_y4); cudaFree(g->d_he); cudaFree(g->d_p0); cudaFree(g->d_sv); cudaFree(g->d_sd); cudaFree(g->d_sq);
-    cudaFree(g->d_counter); cudaFree(g->d_quads); cudaFree(g->d_octs); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
-    if (g->tex) cudaDestroyTextureObject(g->tex);
-    if (g->surf) cudaDestroySurfaceObject(g->surf);
-    if (g->atlas) cudaFreeArray(g->atlas);
+    cudaFree(g->d_counter); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
     if (g->h_scal) cudaFreeHost(g->h_scal);
     if (g->ev0) cudaEventDestroy(g->ev0);
     if (g->ev1) cudaEventDestroy(g->ev1);
@@ -204,7 +197,7 @@ int build_geometry(oat_geometry *G)
         rings.push_back(sentinel);
     }
 
-    // ---- ring blocks of OAT_RI rings and their azimuth sector counts (schedule 1: patches)
+    // ---- ring blocks of OAT_RI rings and their azimuth sector counts (patches)
     std::vector<int> rb_sectors;
     std::vector<std::vector<long long>> rb_prefix(NB);     // per band: sectors in ring blocks [0, rb)
     for (int b = 0; b < NB; ++b) {
@@ -226,16 +219,15 @@ int build_geometry(oat_geometry *G)
     }
     if (Q >= (1 << 26) || NB > 0xfff) return fail(OAT_ERR_INVALID, "too many transducers / bands");
 
-    // ---- frames (S1) and the per-(q, band) ring bound (S9) + work-item prefix
+    // ---- frames (S1) and the per-(q, band) ring bound (S9)
     std::vector<double> frame((size_t)Q * 12);
     std::vector<int> qb_rings((size_t)Q * NB);
-    std::vector<long long> prefix((size_t)Q * NB + 1);
-    long long items = 0;
     for (int q = 0; q < Q; ++q) {
         const double *rq = d.trans_xyz + 3 * (size_t)q;
         double v[3] = {C[0] - rq[0], C[1] - rq[1], C[2] - rq[2]};
         const double L = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
         if (!(L > 0) || !isfinite(L)) return fail(OAT_ERR_INVALID, "transducer %d is at the grid centre or not finite", q);
+        G->h_rq.push_back(L);
         double ez[3] = {v[0] / L, v[1] / L, v[2] / L};
         double ey[3] = {ez[1], -ez[0], 0.0};               // e_z x z^
         const double an = sqrt(ey[0] * ey[0] + ey[1] * ey[1]);
@@ -259,12 +251,8 @@ int build_geometry(oat_geometry *G)
             }
             qb_rings[(size_t)q * NB + b] = nr;
             if (nr > 0) G->patch_cap += (unsigned long long)rb_prefix[b][(nr + OAT_RI - 1) / OAT_RI];
-            prefix[(size_t)q * NB + b] = items;
-            const long long cand = rings[bd.ring_ofs + nr].cum;
-            items += (cand + OAT_CH - 1) / OAT_CH;
         }
     }
-    prefix[(size_t)Q * NB] = items;
     // direction table of the marching kernels: per band the leading rings any transducer can use
     long long n_dir = 0;
     for (int b = 0; b < NB; ++b) {
@@ -281,7 +269,6 @@ int build_geometry(oat_geometry *G)
     if ((rc = upload(&G->d_band, bands))) return rc;
     if ((rc = upload(&G->d_ring, rings))) return rc;
     if ((rc = upload(&G->d_qb_rings, qb_rings))) return rc;
-    if ((rc = upload(&G->d_item_prefix, prefix))) return rc;
     if ((rc = upload(&G->d_rb_sectors, rb_sectors))) return rc;
 
     OatDev &P = G->dev;
@@ -293,19 +280,14 @@ int build_geometry(oat_geometry *G)
     P.c = d.c; P.t0 = d.t0; P.dt = d.dt; P.kappa = G->kappa;
     P.step = d.c * d.dt / ds;
     P.frame = G->d_frame; P.band = G->d_band; P.ring = G->d_ring;
-    P.qb_rings = G->d_qb_rings; P.item_prefix = G->d_item_prefix;
-    P.n_items = items;
+    P.qb_rings = G->d_qb_rings;
     P.rb_sectors = G->d_rb_sectors; P.patches = nullptr; P.n_patches = 0;
     P.q_count = nullptr; P.q_done = nullptr;
     P.dir = nullptr;
-    if (B == 32 && n_dir > 0 && n_dir < (1LL << 31)) {     // 16 B per direction; otherwise variant 4 falls back to 3
+    if (B == 32 && n_dir > 0 && n_dir < (1LL << 31)) {     // 16 B per direction; otherwise the generic kernel is used
         CUDA_TRY(cudaMalloc((void **)&G->d_dir, sizeof(double2) * (size_t)n_dir));
         P.dir = G->d_dir;
     }
-    P.tex = 0; P.atlas_shift = 0; P.atlas_mask = 0;
-    P.qx = (d.nx + 2) / 2 + 1; P.qy = (d.ny + 2) / 2 + 1;
-    P.qplane = (long long)P.qx * P.qy;
-    P.oz = (d.nz + 2) / 2 + 1;
     // cell records with a zero margin: a ray is kept when the bounding box of its 32-sample segment meets the padded box,
     // so its samples lie within 31 * step cells of it (+ the cull's 0.01 slack and one cell for floor)
     P.cm = (int)ceil(31.0 * P.step) + 3;
@@ -327,17 +309,14 @@ int build_geometry(oat_geometry *G)
     G->n_cells = P.cx ? (size_t)P.cz * (size_t)P.cxy : 0;
     {   // packed list entries: anchor node offsets in [-128, 895] (anchor = band midpoint, at most 16 samples outside the padded box)
         const int nmax = d.nx > d.ny ? (d.nx > d.nz ? d.nx : d.nz) : (d.ny > d.nz ? d.ny : d.nz);
-        G->march_ok = (16.0 * P.step + 4.0 <= 128.0) && (nmax + 2 + 16.0 * P.step + 4.0 <= 895.0);
+        // step <= 1: a ray moves at most one cell per sample, which the record-index form of the carry test assumes
+        G->march_ok = (P.step <= 1.0) && (16.0 * P.step + 4.0 <= 128.0) && (nmax + 2 + 16.0 * P.step + 4.0 <= 895.0);
     }
 
     G->n_vox = (size_t)d.nx * d.ny * d.nz;
     G->n_dat = (size_t)Q * K;
     G->n_pad = (size_t)P.pz * P.pxy;
-    G->n_quads = 4 * (size_t)P.pz * (size_t)P.qplane;
-    G->n_octs = 2 * 8 * (size_t)P.oz * (size_t)P.qplane;
-    if (G->n_octs / 2 >= (1ULL << 31)) return fail(OAT_ERR_INVALID, "grid too large for the octet layout");
     if (G->n_pad >= (1ULL << 31)) return fail(OAT_ERR_INVALID, "padded grid has more than 2^31 nodes");
-    CUDA_TRY(cudaMalloc((void **)&G->d_xpad, sizeof(float) * G->n_pad));
     CUDA_TRY(cudaMalloc((void **)&G->d_g, sizeof(double) * (G->n_dat ? G->n_dat : 1)));
     CUDA_TRY(cudaMalloc((void **)&G->d_scal, sizeof(double) * 8));
     CUDA_TRY(cudaMalloc((void **)&G->d_counter, sizeof(unsigned long long)));
@@ -349,42 +328,6 @@ int build_geometry(oat_geometry *G)
         CUDA_TRY(cudaGetLastError());
         CUDA_TRY(cudaDeviceSynchronize());
     }
-    return OAT_OK;
-}
-
-// Slice atlas for the texture-gather variant: the pz slices of the padded volume tiled into one 2-D
-// CUDA array (2-D because texture gather, tld4, exists for 2-D textures only), 2^shift slices per row.
-int ensure_atlas(oat_geometry *G)
-{
-    if (G->tex) return OAT_OK;
-    OatDev &P = G->dev;
-    int shift = 0;
-    while ((1 << (2 * shift)) < P.pz) ++shift;            // cols = 2^shift >= sqrt(pz)
-    const int cols = 1 << shift, rows = (P.pz + cols - 1) / cols;
-    int maxw = 0, maxh = 0;
-    CUDA_TRY(cudaDeviceGetAttribute(&maxw, cudaDevAttrMaxTexture2DGatherWidth, G->device));
-    CUDA_TRY(cudaDeviceGetAttribute(&maxh, cudaDevAttrMaxTexture2DGatherHeight, G->device));
-    if ((long long)cols * P.px > maxw || (long long)rows * P.py > maxh)
-        return fail(OAT_ERR_INVALID, "grid too large for the texture-gather variant (atlas %lld x %lld > %d x %d)",
-                    (long long)cols * P.px, (long long)rows * P.py, maxw, maxh);
-    cudaChannelFormatDesc fmt = cudaCreateChannelDesc<float>();
-    CUDA_TRY(cudaMallocArray(&G->atlas, &fmt, (size_t)cols * P.px, (size_t)rows * P.py,
-                             cudaArrayTextureGather | cudaArraySurfaceLoadStore));
-    cudaResourceDesc res;
-    memset(&res, 0, sizeof(res));
-    res.resType = cudaResourceTypeArray;
-    res.res.array.array = G->atlas;
-    cudaTextureDesc td;
-    memset(&td, 0, sizeof(td));
-    td.addressMode[0] = td.addressMode[1] = cudaAddressModeClamp;
-    td.filterMode = cudaFilterModePoint;
-    td.readMode = cudaReadModeElementType;
-    td.normalizedCoords = 0;
-    CUDA_TRY(cudaCreateTextureObject(&G->tex, &res, &td, nullptr));
-    CUDA_TRY(cudaCreateSurfaceObject(&G->surf, &res));
-    P.tex = G->tex;
-    P.atlas_shift = shift;
-    P.atlas_mask = cols - 1;
     return OAT_OK;
 }
 
@@ -406,69 +349,59 @@ int ensure_patches(oat_geometry *G)
     return OAT_OK;
 }
 
-// one traversal of all samples: mode 0 gather, 1 scatter, 2 count; schedule picks the work decomposition
-int launch_traversal(oat_geometry *G, int mode, int variant, const float *src, float *acc, const float *y, double *g,
-                     unsigned long long *counter, cudaStream_t st, bool *launched)
+int ensure_xpad(oat_geometry *G)
 {
-    *launched = false;
-    if (G->schedule == 1) {
-        int rc = ensure_patches(G); if (rc) return rc;
-        if (G->dev.n_patches > 0) { CUDA_TRY(oat_launch_patch(mode, variant, G->dev, src, acc, y, g, counter, st)); *launched = true; }
-    } else if (G->dev.n_items > 0) {
-        CUDA_TRY(oat_launch_ray(mode, variant, G->dev, src, acc, y, g, counter, st)); *launched = true;
-    }
+    if (G->d_xpad) return OAT_OK;
+    CUDA_TRY(cudaMalloc((void **)&G->d_xpad, sizeof(float) * G->n_pad));
     return OAT_OK;
 }
 
-int ensure_quads(oat_geometry *G)
+// one traversal of all samples by the generic patch kernel: mode 0 gather, 1 scatter, 2 count
+int launch_traversal(oat_geometry *G, int mode, const float *src, float *acc, const float *y, double *g,
+                     unsigned long long *counter, cudaStream_t st, bool *launched)
 {
-    if (G->d_quads) return OAT_OK;
-    CUDA_TRY(cudaMalloc((void **)&G->d_quads, sizeof(float4) * G->n_quads));
+    *launched = false;
+    int rc = ensure_patches(G); if (rc) return rc;
+    if (G->dev.n_patches > 0) { CUDA_TRY(oat_launch_patch(mode, G->dev, src, acc, y, g, counter, st)); *launched = true; }
     return OAT_OK;
+}
+
+bool march_h_ok(const oat_geometry *G)
+{
+    return G->dev.B == 32 && G->n_cells && G->n_cells < G->record_limit && G->dev.dir && G->march_ok;
+}
+
+bool march_ht_ok(const oat_geometry *G)
+{
+    return G->dev.B == 32 && G->n_faces && G->n_faces < G->record_limit && G->dev.dir && G->march_ok;
 }
 
 int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    const float *src = G->d_xpad;
-    int variant = G->variant_project;
-    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_cells || !P.dir || !G->march_ok)) variant = 3;   // marching form needs B = 32 patches
-    if (variant == 4) {
+    const bool march = G->variant_project == 4 && march_h_ok(G);   // else: B < 32 or a grid the marching kernel cannot index
+    int rc = ensure_patches(G); if (rc) return rc;
+    if (march) {
         if (!G->d_cells) CUDA_TRY(cudaMalloc((void **)&G->d_cells, sizeof(float4) * 2 * G->n_cells));
         oat_launch_pad_cells(P, d_x, G->d_cells, st); ++G->last_launches;
-        src = reinterpret_cast<const float *>(G->d_cells);
-    } else if (variant == 3) {
-        if (!G->d_octs) CUDA_TRY(cudaMalloc((void **)&G->d_octs, sizeof(float4) * G->n_octs));
-        oat_launch_pad_octs(P, d_x, G->d_octs, st); ++G->last_launches;
-        src = reinterpret_cast<const float *>(G->d_octs);
-    } else if (variant == 2) {
-        int rc = ensure_quads(G); if (rc) return rc;
-        oat_launch_pad_quads(P, d_x, G->d_quads, st); ++G->last_launches;
-        src = reinterpret_cast<const float *>(G->d_quads);
-    } else if (variant == 1) {
-        int rc = ensure_atlas(G); if (rc) return rc;
-        oat_launch_pad_atlas(P, d_x, G->surf, st); ++G->last_launches;
     } else {
+        if ((rc = ensure_xpad(G))) return rc;
         oat_launch_pad(P, d_x, G->d_xpad, st); ++G->last_launches;
     }
     CUDA_TRY(cudaMemsetAsync(G->d_g, 0, sizeof(double) * (G->n_dat ? G->n_dat : 1), st));
-    const bool fused = G->schedule == 1;                  // patch kernel applies 1/t and the time difference itself
-    if (fused) {
-        int rc = ensure_patches(G); if (rc) return rc;
-        if (G->n_dat > 0) CUDA_TRY(cudaMemsetAsync(d_y, 0, sizeof(float) * G->n_dat, st));   // rows without any sample
-        if (G->d_q_done) CUDA_TRY(cudaMemsetAsync(G->d_q_done, 0, sizeof(int) * (size_t)(P.Q > 0 ? P.Q : 1), st));
-    }
+    // the kernel that finishes the last patch of a transducer applies 1/t and the time difference itself (step A4)
+    if (G->n_dat > 0) CUDA_TRY(cudaMemsetAsync(d_y, 0, sizeof(float) * G->n_dat, st));   // rows without any sample
+    if (G->d_q_done) CUDA_TRY(cudaMemsetAsync(G->d_q_done, 0, sizeof(int) * (size_t)(P.Q > 0 ? P.Q : 1), st));
     CUDA_TRY(cudaEventRecord(G->ev0, st));
     bool launched;
-    if (variant == 4) {
+    if (march) {
         launched = G->dev.n_patches > 0;
         CUDA_TRY(oat_launch_march(0, G->dev, G->d_cells, nullptr, d_y, nullptr, G->d_g, st));
-    } else { int rc = launch_traversal(G, 0, variant, src, fused ? d_y : nullptr, nullptr, G->d_g, nullptr, st, &launched); if (rc) return rc; }
+    } else if ((rc = launch_traversal(G, 0, G->d_xpad, d_y, nullptr, G->d_g, nullptr, st, &launched))) return rc;
     if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
-    if (!fused && G->n_dat > 0) { oat_launch_diff(P, G->d_g, d_y, st); ++G->last_launches; }
     CUDA_TRY(cudaGetLastError());
     return OAT_OK;
 }
@@ -477,36 +410,27 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    int variant = G->variant_backproject;
-    if (variant == 4 && (P.B != 32 || G->schedule != 1 || !G->n_faces || !P.dir || !G->march_ok)) variant = 3;   // marching form needs B = 32 patches
-    const bool faces = variant == 4;
-    const bool quads = !faces && variant >= 2;
-    float *acc = G->d_xpad;
-    if (faces) {
+    const bool march = G->variant_backproject == 4 && march_ht_ok(G);
+    int rc = ensure_patches(G); if (rc) return rc;
+    if (march) {
         if (!G->d_faces) CUDA_TRY(cudaMalloc((void **)&G->d_faces, sizeof(float4) * G->n_faces));
-        acc = reinterpret_cast<float *>(G->d_faces);
         CUDA_TRY(cudaMemsetAsync(G->d_faces, 0, sizeof(float4) * G->n_faces, st));
-        int rc = ensure(&G->d_coef, G->n_dat); if (rc) return rc;
-        if ((rc = ensure_patches(G))) return rc;
+        if ((rc = ensure(&G->d_coef, G->n_dat))) return rc;
         oat_launch_coef(P, d_y, G->d_coef, st); ++G->last_launches;
-    } else if (quads) {
-        int rc = ensure_quads(G); if (rc) return rc;
-        acc = reinterpret_cast<float *>(G->d_quads);
-        CUDA_TRY(cudaMemsetAsync(G->d_quads, 0, sizeof(float4) * G->n_quads, st));
     } else {
+        if ((rc = ensure_xpad(G))) return rc;
         CUDA_TRY(cudaMemsetAsync(G->d_xpad, 0, sizeof(float) * G->n_pad, st));
     }
     CUDA_TRY(cudaEventRecord(G->ev0, st));
     bool launched;
-    if (faces) {
+    if (march) {
         launched = G->dev.n_patches > 0;
         CUDA_TRY(oat_launch_march(1, G->dev, nullptr, G->d_faces, nullptr, G->d_coef, nullptr, st));
-    } else { int rc = launch_traversal(G, 1, variant, nullptr, acc, d_y, nullptr, nullptr, st, &launched); if (rc) return rc; }
+    } else if ((rc = launch_traversal(G, 1, nullptr, G->d_xpad, d_y, nullptr, nullptr, st, &launched))) return rc;
     if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));
     G->ev_valid = true;
-    if (faces) oat_launch_unface(P, G->d_faces, d_x, st);
-    else if (quads) oat_launch_unquad(P, G->d_quads, d_x, st);
+    if (march) oat_launch_unface(P, G->d_faces, d_x, st);
     else oat_launch_unpad(P, G->d_xpad, d_x, st);
     ++G->last_launches;
     CUDA_TRY(cudaGetLastError());
@@ -612,7 +536,7 @@ int64_t oat_num_surface_samples(oat_geometry *g)
     if (g->n_surface_samples >= 0) return g->n_surface_samples;
     if (cudaMemset(g->d_counter, 0, sizeof(unsigned long long)) != cudaSuccess) return -1;
     bool launched;
-    if (launch_traversal(g, 2, 0, nullptr, nullptr, nullptr, nullptr, g->d_counter, 0, &launched)) return -1;
+    if (launch_traversal(g, 2, nullptr, nullptr, nullptr, nullptr, g->d_counter, 0, &launched)) return -1;
     unsigned long long v = 0;
     if (cudaMemcpy(&v, g->d_counter, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) {
         fail(OAT_ERR_CUDA, "sample count kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -937,18 +861,36 @@ int oat_fbp(oat_geometry *g, const float *d_p, const float *d_w, float *d_x, voi
     return OAT_OK;
 }
 
+int oat_fbp_weights(const oat_geometry *g, const double *h_areas, float *h_w)
+{
+    if (!g) return fail(OAT_ERR_INVALID, "geometry handle is NULL");
+    if ((!h_areas || !h_w) && g->dev.Q) return fail(OAT_ERR_INVALID, "h_areas / h_w must not be NULL");
+    const double c = g->desc.c, k = 4.0 * kPi * kPi * g->kappa * c * c * c * g->desc.dt;
+    for (int q = 0; q < g->dev.Q; ++q) h_w[q] = (float)(-h_areas[q] / (k * g->h_rq[(size_t)q]));
+    return OAT_OK;
+}
+
 int oat_set_variant(oat_geometry *g, const char *key, int variant)
 {
     if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");
-    if (!strcmp(key, "project")) { if (variant < 0 || variant > 4) return fail(OAT_ERR_INVALID, "unknown project variant %d", variant); g->variant_project = variant; return OAT_OK; }
-    if (!strcmp(key, "backproject")) { if (variant < 0 || variant > 4) return fail(OAT_ERR_INVALID, "unknown backproject variant %d", variant); g->variant_backproject = variant; return OAT_OK; }
+    if (!strcmp(key, "project")) { if (variant != 0 && variant != 4) return fail(OAT_ERR_INVALID, "unknown project variant %d (0 generic, 4 marching)", variant); g->variant_project = variant; return OAT_OK; }
+    if (!strcmp(key, "backproject")) { if (variant != 0 && variant != 4) return fail(OAT_ERR_INVALID, "unknown backproject variant %d (0 generic, 4 marching)", variant); g->variant_backproject = variant; return OAT_OK; }
     if (!strcmp(key, "morton_shift")) {
         if (variant < 0 || variant > 10) return fail(OAT_ERR_INVALID, "morton_shift out of range");
         if (g->morton_shift != variant) { cudaFree(g->d_patches); g->d_patches = nullptr; g->dev.patches = nullptr; g->dev.n_patches = 0; }
         g->morton_shift = variant; return OAT_OK;
     }
-    if (!strcmp(key, "schedule")) { if (variant < 0 || variant > 1) return fail(OAT_ERR_INVALID, "unknown schedule %d", variant); g->schedule = variant; return OAT_OK; }
+    if (!strcmp(key, "record_limit_log2")) {               // tests: pretend the 32-bit record index is narrower
+        if (variant < 1 || variant > 31) return fail(OAT_ERR_INVALID, "record_limit_log2 out of range");
+        g->record_limit = (size_t)1 << variant; return OAT_OK;
+    }
     return fail(OAT_ERR_INVALID, "unknown variant key '%s'", key);
+}
+
+int oat_uses_marching(const oat_geometry *g, int backproject)
+{
+    if (!g) return -1;
+    return backproject ? (g->variant_backproject == 4 && march_ht_ok(g)) : (g->variant_project == 4 && march_h_ok(g));
 }
 
 int oat_last_launch_count(const oat_geometry *g) { return g ? g->last_launches : -1; }
@@ -960,127 +902,6 @@ float oat_last_kernel_ms(oat_geometry *g)
     float ms = -1.f;
     if (cudaEventElapsedTime(&ms, g->ev0, g->ev1) != cudaSuccess) return -1.f;
     return ms;
-}
-
-int oat_measure_red_rate(int device, double *lanes_per_s)
-{
-    if (!lanes_per_s) return fail(OAT_ERR_INVALID, "NULL argument");
-    CUDA_TRY(cudaSetDevice(device));
-    const size_t bytes = 64u << 20;                       // L2-resident
-    const int blocks = 148 * 8, iters = 2000;
-    float4 *buf = nullptr;
-    cudaEvent_t a = nullptr, b = nullptr;
-    CUDA_TRY(cudaMalloc((void **)&buf, bytes));
-    cudaError_t e = cudaMemset(buf, 0, bytes);
-    if (e == cudaSuccess) e = cudaEventCreate(&a);
-    if (e == cudaSuccess) e = cudaEventCreate(&b);
-    float ms = 0.f;
-    if (e == cudaSuccess) {
-        oat_launch_red_probe(buf, (unsigned)(bytes / 16), 200, blocks, 0);      // warm-up
-        cudaEventRecord(a, 0);
-        oat_launch_red_probe(buf, (unsigned)(bytes / 16), iters, blocks, 0);
-        cudaEventRecord(b, 0);
-        e = cudaEventSynchronize(b);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
-    }
-    if (a) cudaEventDestroy(a);
-    if (b) cudaEventDestroy(b);
-    cudaFree(buf);
-    if (e != cudaSuccess || !(ms > 0.f)) return fail(OAT_ERR_CUDA, "reduction-rate probe failed: %s", cudaGetErrorString(e));
-    *lanes_per_s = (double)blocks * 256.0 * iters / (ms * 1e-3);
-    return OAT_OK;
-}
-
-int oat_measure_gather_rate(int device, double *sectors_per_s)
-{
-    if (!sectors_per_s) return fail(OAT_ERR_INVALID, "NULL argument");
-    CUDA_TRY(cudaSetDevice(device));
-    const size_t bytes = 64u << 20;                       // L2-resident, far larger than L1
-    const int blocks = 148 * 8, iters = 500;
-    float4 *buf = nullptr;
-    float *sink = nullptr;
-    cudaEvent_t a = nullptr, b = nullptr;
-    CUDA_TRY(cudaMalloc((void **)&buf, bytes));
-    cudaError_t e = cudaMemset(buf, 0, bytes);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&sink, sizeof(float));
-    if (e == cudaSuccess) e = cudaEventCreate(&a);
-    if (e == cudaSuccess) e = cudaEventCreate(&b);
-    float ms = 0.f;
-    if (e == cudaSuccess) {
-        oat_launch_gather_probe(buf, (unsigned)(bytes / 16), 50, blocks, sink, 0);      // warm-up (fills L2)
-        cudaEventRecord(a, 0);
-        oat_launch_gather_probe(buf, (unsigned)(bytes / 16), iters, blocks, sink, 0);
-        cudaEventRecord(b, 0);
-        e = cudaEventSynchronize(b);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
-    }
-    if (a) cudaEventDestroy(a);
-    if (b) cudaEventDestroy(b);
-    cudaFree(sink);
-    cudaFree(buf);
-    if (e != cudaSuccess || !(ms > 0.f)) return fail(OAT_ERR_CUDA, "gather-rate probe failed: %s", cudaGetErrorString(e));
-    *sectors_per_s = (double)blocks * 256.0 * 4.0 * iters / (ms * 1e-3);
-    return OAT_OK;
-}
-
-int oat_measure_gather_rate_ex(int device, int lanes_active, int smem_kb_per_block, double *sectors_per_s)
-{
-    if (!sectors_per_s || lanes_active < 1 || lanes_active > 32 || smem_kb_per_block < 0 || smem_kb_per_block > 27)
-        return fail(OAT_ERR_INVALID, "bad argument (lanes_active 1..32, smem_kb_per_block 0..27)");
-    CUDA_TRY(cudaSetDevice(device));
-    const size_t bytes = 64u << 20;
-    const int blocks = 148 * 8, iters = 2000;
-    float4 *buf = nullptr; float *sink = nullptr;
-    cudaEvent_t a = nullptr, b = nullptr;
-    CUDA_TRY(cudaMalloc((void **)&buf, bytes));
-    cudaError_t e = cudaMemset(buf, 0, bytes);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&sink, sizeof(float));
-    if (e == cudaSuccess) e = cudaEventCreate(&a);
-    if (e == cudaSuccess) e = cudaEventCreate(&b);
-    float ms = 0.f;
-    if (e == cudaSuccess) e = oat_launch_gather_probe_ex(buf, (unsigned)(bytes / 32), 100, lanes_active, smem_kb_per_block * 1024, blocks, sink, 0);
-    if (e == cudaSuccess) {
-        cudaEventRecord(a, 0);
-        e = oat_launch_gather_probe_ex(buf, (unsigned)(bytes / 32), iters, lanes_active, smem_kb_per_block * 1024, blocks, sink, 0);
-        cudaEventRecord(b, 0);
-        if (e == cudaSuccess) e = cudaEventSynchronize(b);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
-    }
-    if (a) cudaEventDestroy(a);
-    if (b) cudaEventDestroy(b);
-    cudaFree(sink); cudaFree(buf);
-    if (e != cudaSuccess || !(ms > 0.f)) return fail(OAT_ERR_CUDA, "gather-rate probe failed: %s", cudaGetErrorString(e));
-    *sectors_per_s = (double)blocks * 4.0 * iters * lanes_active / (ms * 1e-3);
-    return OAT_OK;
-}
-
-int oat_measure_red_rate_ex(int device, int pattern, double *lanes_per_s)
-{
-    if (!lanes_per_s || pattern < 0 || pattern > 4) return fail(OAT_ERR_INVALID, "bad argument (pattern 0..4)");
-    CUDA_TRY(cudaSetDevice(device));
-    const size_t bytes = 64u << 20;
-    const int blocks = 148 * 8, iters = 2000;
-    float4 *buf = nullptr;
-    cudaEvent_t a = nullptr, b = nullptr;
-    CUDA_TRY(cudaMalloc((void **)&buf, bytes));
-    cudaError_t e = cudaMemset(buf, 0, bytes);
-    if (e == cudaSuccess) e = cudaEventCreate(&a);
-    if (e == cudaSuccess) e = cudaEventCreate(&b);
-    float ms = 0.f;
-    if (e == cudaSuccess) {
-        oat_launch_red_probe_ex(buf, (unsigned)(bytes / 16), 200, pattern, blocks, 0);
-        cudaEventRecord(a, 0);
-        oat_launch_red_probe_ex(buf, (unsigned)(bytes / 16), iters, pattern, blocks, 0);
-        cudaEventRecord(b, 0);
-        e = cudaEventSynchronize(b);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
-    }
-    if (a) cudaEventDestroy(a);
-    if (b) cudaEventDestroy(b);
-    cudaFree(buf);
-    if (e != cudaSuccess || !(ms > 0.f)) return fail(OAT_ERR_CUDA, "reduction-rate probe failed: %s", cudaGetErrorString(e));
-    *lanes_per_s = (double)blocks * 256.0 * iters / (ms * 1e-3);
-    return OAT_OK;
 }
 
 const char *oat_last_error(void) { return g_err; }

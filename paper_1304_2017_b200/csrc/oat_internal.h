@@ -7,34 +7,25 @@
 //   ring    sum(n_rings+1) per band, rings i = 1..n_rings with theta_i = i*dtheta < pi, plus a
 //                         sentinel whose `cum` is the band's total direction count
 //   qb_rings Q x NB       number of leading rings that can reach the padded box (S9 cull)
-//   item_prefix Q*NB+1    exclusive prefix of work items (chunks of OAT_CH candidate directions)
+//   patches               Morton-sorted work items (q, band, ring block, azimuth sector)
+//   dir                   fp64 direction table of the marching kernels
+//   cells                 per-cell polynomial records with a zero margin (marching H)
+//   faces                 face-quad accumulators of the three orientations (marching H^T)
 //   xpad    (nz+2)(ny+2)(px) fp32  volume zero-padded by one node on every side = Eq. (12)'s
-//                         "nodes outside the grid do not exist" (reading G5), row pitch px
+//                         "nodes outside the grid do not exist" (reading G5), row pitch px (generic kernel)
 //   g       Q x K fp64    SRT accumulator (forward) before the time difference
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#define OAT_CH 8192        // candidate directions per work item
-#define OAT_SB 1024        // candidates per shared-memory sub-batch
-#define OAT_NT 256         // threads per block of the ray kernels
+#define OAT_NT 256         // threads per block of the generic patch kernel
 #define OAT_NW (OAT_NT / 32)
-#define OAT_RI 32          // rings per patch (schedule 1)
+#define OAT_RI 32          // rings per patch
 #define OAT_RJ 32          // max azimuth samples per ring of a patch
 #ifndef OAT_MT
 #define OAT_MT 128         // threads per block of the marching kernels
 #endif
 #define OAT_BU 8           // steps per trip of the (rolled) backprojection marching loop
-// list entries (32 B each) per build/consume round of the marching kernels: 512 = 16 rings x 32 (16 KB per block).
-// Measured on the config-3 subset (H / H^T ms): 48-byte entries x 512: 79.5 / 91.5; 32-byte x 256: 75.8 / 95.9;
-// 32-byte x 512: 70.8 / 91.5; 32-byte x 1024 at 6 blocks: 78.9 / 91.4 -- less shared memory leaves more L1 for the
-// scattered record loads of H, fewer rounds mean fewer barriers.
-#ifndef OAT_MLH
-#define OAT_MLH 512
-#endif
-#ifndef OAT_MLT
-#define OAT_MLT 1024
-#endif
 
 struct OatBand {
     double s_mid;      // radius of the band's anchor (k0 + (B-1)/2) in voxel units: rho/ds
@@ -67,68 +58,52 @@ struct OatDev {
     const OatBand *band;
     const OatRing *ring;
     const int *qb_rings;
-    const long long *item_prefix;
-    long long n_items;
     const int *rb_sectors;               // per (band, ring block): number of azimuth sectors S
-    const unsigned long long *patches;   // schedule 1: Morton-sorted packed (q, band, ring block, sector)
+    const unsigned long long *patches;   // Morton-sorted packed (q, band, ring block, sector)
     long long n_patches;
     const double2 *dir;                  // direction table (marching kernels): (sin th cos phi, sin th sin phi) of ring r,
                                          // azimuth j of band b at band.dir_ofs + ring.cum + j, fp64 (S2, S3)
     const int *q_count;                  // patches per transducer
     int *q_done;                         // patches finished in the running projection (zeroed per call)
-    int qx, qy;                // quad layout (variant 2): quads per row / rows per plane
-    long long qplane;          // qx*qy; one parity array holds pz*qplane float4 quads
-    int oz;                    // octet layout (project variant 3): bricks along z; 8 arrays of oz*qplane records of 32 B
     int cx, cy, cz;            // cell-record layout (marching H): cells per row (pitch, multiple of 4) / rows per plane / planes,
     int cm;                    // each = nodes + 1 + 2 cm: a zero margin of cm cells around the padded box, wide enough for every
                                // sample of every ray whose segment meets the box (no per-sample bounds test)
     long long cxy;             // cx*cy; record of padded cell (ix,iy,iz) = ((iz+cm)*cy + iy+cm)*cx + ix+cm, 32 B each
-    // face-quad accumulators (backproject variant 4): orientation o = axis a normal to the quad, in-plane axes
+    // face-quad accumulators (marching H^T): orientation o = axis a normal to the quad, in-plane axes
     // (b, c) = (y,z), (z,x), (x,y) for a = x, y, z; record (ia, ib, ic) = float4 of padded nodes
     // {(ib,ic),(ib+1,ic),(ib,ic+1),(ib+1,ic+1)} on plane ia, at f_base[o] + (ia*f_nc[o] + ic)*f_nb[o] + ib
     long long f_base[3];
     int f_nb[3], f_nc[3];
-    cudaTextureObject_t tex;   // slice atlas of the padded volume (project variant 1), 0 if unused
-    int atlas_shift, atlas_mask;   // slice z sits at column (z & mask), row (z >> shift) of the atlas
 };
 
-// launchers (oat_kernels.cu); all asynchronous on `st`
+// error reporting shared by the translation units (oat_api.cu): formats the thread-local message, returns `code`
+int oat_fail(int code, const char *fmt, ...);
+
+// launchers; all asynchronous on `st`
 void oat_launch_pad(const OatDev &P, const float *x, float *xpad, cudaStream_t st);
 void oat_launch_unpad(const OatDev &P, const float *xpad, float *x, cudaStream_t st);
-// mode 0: g += G x (gathers from xpad); 1: xacc += G^T D^T y (scatter); 2: count in-box samples
-// quad layout: 4 parity-shifted arrays of xy-quads {(x0,y0),(x0+1,y0),(x0,y0+1),(x0+1,y0+1)} with
-// x0 = 2a + (p&1), y0 = 2b + (p>>1): the four in-plane corners of ANY cell are one aligned float4
-void oat_launch_pad_quads(const OatDev &P, const float *x, float4 *quads, cudaStream_t st);
-void oat_launch_pad_octs(const OatDev &P, const float *x, float4 *octs, cudaStream_t st);
-// cell records (variant 4): per padded cell the 8 coefficients of its trilinear polynomial
-// c0 + cx fx + cy fy + cxy fx fy + fz (cz + cxz fx + cyz fy + cxyz fx fy), fp64-computed, one 32-byte sector
-void oat_launch_pad_cells(const OatDev &P, const float *x, float4 *cells, cudaStream_t st);
-// x[n] = sum of the 12 face-quad components that are node n (backproject variant 4)
-void oat_launch_unface(const OatDev &P, const float4 *faces, float *x, cudaStream_t st);
-void oat_launch_unquad(const OatDev &P, const float4 *quads, float *x, cudaStream_t st);
-void oat_launch_pad_atlas(const OatDev &P, const float *x, cudaSurfaceObject_t surf, cudaStream_t st);
-cudaError_t oat_launch_ray(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
-                           double *g, unsigned long long *counter, cudaStream_t st);
-cudaError_t oat_launch_patch(int mode, int variant, const OatDev &P, const float *xpad, float *xacc, const float *y,
+// generic patch kernel (oat_kernels.cu): mode 0: g += G x (gathers from xpad) and y rows (step A4); 1: xacc += G^T D^T y
+// (8 scalar atomics per sample); 2: count in-box samples
+cudaError_t oat_launch_patch(int mode, const OatDev &P, const float *xpad, float *xacc, const float *y,
                              double *g, unsigned long long *counter, cudaStream_t st);
-// marching kernels (variant 4, B = 32): mode 0 gathers from cell records into g (and writes y rows, step A4),
+// cell records (marching H): per cell the 8 coefficients of its trilinear polynomial
+// c0 + c1 fx + c2 fy + c3 fx fy + fz (c4 + c5 fx + c6 fy + c7 fx fy), fp64-computed, one 32-byte sector
+void oat_launch_pad_cells(const OatDev &P, const float *x, float4 *cells, cudaStream_t st);
+// x[n] = sum of the 12 face-quad components that are node n (marching H^T)
+void oat_launch_unface(const OatDev &P, const float4 *faces, float *x, cudaStream_t st);
+// marching kernels (oat_march.cu, B = 32): mode 0 gathers from cell records into g (and writes y rows, step A4),
 // mode 1 scatters coef[q,k] = g'_k rho_k^2 into the face-quad accumulators
 cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, float4 *faces, float *y_out,
                              const float *coef, double *g, cudaStream_t st);
 void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream_t st);
 // coef[q,k] = kappa (y[k-1] - y[k+1]) / (2 dt t_k) * rho_k^2   (Eq. 22 L172 with the rho^2 of S8; 0 where t_k <= 0)
 void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st);
-// micro-benchmark behind oat_measure_red_rate(): `iters` scattered RED.128 per thread into `buf` (n16 float4 records)
-void oat_launch_red_probe(float4 *buf, unsigned n16, int iters, int blocks, cudaStream_t st);
-// micro-benchmark behind oat_measure_gather_rate(): 4 x `iters` scattered 256-bit loads per thread from `buf`
-void oat_launch_gather_probe(const float4 *buf, unsigned n16, int iters, int blocks, float *sink, cudaStream_t st);
 cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, int *q_count, unsigned long long **patches_out, long long *n_patches);
-void oat_launch_diff(const OatDev &P, const double *g, float *y, cudaStream_t st);
 // vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)
 void oat_launch_dot(const float *a, const float *b, long long n, double *out, cudaStream_t st);
 void oat_launch_axpy(float alpha, const float *x, float *y, long long n, cudaStream_t st);   // y += alpha x
 void oat_launch_xpay(const float *x, float beta, float *y, long long n, cudaStream_t st);    // y = x + beta y
-// row NEXT-1: EIR convolution / correlation along time (Eq. 14 / Eq. 21) and the penalty stencil (Eq. 34)
+// row NEXT-1 (oat_next.cu): EIR convolution / correlation along time (Eq. 14 / Eq. 21) and the penalty stencil (Eq. 34)
 cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float *he, int L, int Q, int K, cudaStream_t st);
 void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha, float beta, cudaStream_t st);   // out = beta out + alpha L x
 // row NEXT-2: filtered backprojection, Eq. (27), x[n] = sum_q wq[q] {...} (voxel driven)
@@ -136,6 +111,3 @@ void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, 
 // row NEXT-3: spherical-voxel model (Eq. 17-19, 24), point-like transducers; u, v: Q x nf complex (float2), p0: nf complex
 void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float *x, const float2 *p0, float *u, cudaStream_t st);
 void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st);
-// parametrised roofline probes (oat_measure_gather_rate_ex / oat_measure_red_rate_ex)
-cudaError_t oat_launch_gather_probe_ex(const float4 *buf, unsigned nsec, int iters, int active, int smem_bytes, int blocks, float *sink, cudaStream_t st);
-void oat_launch_red_probe_ex(float4 *buf, unsigned n16, int iters, int pattern, int blocks, cudaStream_t st);

@@ -126,14 +126,6 @@ def patch_areas_arc(n_elem: int, n_views: int, radius: float, polar0_deg: float 
     return np.repeat(radius * radius * dth * dph * np.sin(pol), n_views)
 
 
-def fbp_weights(w: "Workload", areas: np.ndarray) -> np.ndarray:
-    """Input vector of row NEXT-2 (reading G23): w_q = -dS_q / (4 pi^2 kappa c^3 dt R_q), the constant of Eq. (27)
-    with kappa = beta / (4 pi C_p) and R_q the transducer's distance from the grid centre.  Handed to the oracle and
-    to the library alike (an INPUT of the operator, like the transducer positions)."""
-    r = np.linalg.norm(np.asarray(w.trans_xyz, dtype=np.float64) - w.centre, axis=1)
-    return -np.asarray(areas, dtype=np.float64) / (4.0 * math.pi ** 2 * w.gain * w.c ** 3 * w.dt * r)
-
-
 def default_t0(trans_xyz: np.ndarray, n: int, spacing: float, c: float, dt: float) -> float:
     """t0 = dt * max(1, floor((min_q |r_q - C| - R_pad)/(c dt)) - 1) with
     R_pad = sqrt(3) * ((N-1) spacing / 2 + spacing); grid centred at the origin."""

@@ -18,18 +18,24 @@ def lib():
     return binding.load()
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "oat.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(oat_[a-z_0-9]+)\s*\(", text)))
+def declared_symbols(headers=("oat.h", "oat_probe.h")):
+    names = set()
+    for h in headers:
+        text = open(os.path.join(ROOT, "include", h)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names |= set(re.findall(r"\b(oat_[a-z_0-9]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_symbols_are_exported(lib):
     names = declared_symbols()
     assert {"oat_geometry_create", "oat_project", "oat_backproject", "oat_adjoint_check"} <= set(names)
     for n in names:
-        assert hasattr(lib, n), f"{n} declared in include/oat.h but not exported by liboat.so"
+        assert hasattr(lib, n), f"{n} declared in include/*.h but not exported by liboat.so"
     assert set(binding.EXPORTS) == set(names)
+    # the product header holds the paper's problem statement only: no probes, no kernel selection
+    product = declared_symbols(("oat.h",))
+    assert not [n for n in product if "measure" in n or "variant" in n or "kernel_ms" in n]
 
 
 def test_binding_has_the_same_names():

@@ -74,6 +74,24 @@ def test_non_cubic_grid_record_edges_and_degenerate_sizes(env):
     assert np.all(gpu_fbp(torch, oat, w1, np.ones((9, 1), np.float32), np.ones(9, np.float32)) == 0.0)
 
 
+def test_transducer_on_a_grid_node(env):
+    """Reading G25: a voxel that coincides with a transducer gets no term from that transducer (and no NaN)."""
+    torch, ofbp, orc, oat, wl = env
+    tr = np.array([[0.5, -0.5, 1.0], [9.0, 2.0, -3.0], [-7.0, 6.0, 4.0]])          # the first one sits on node (5, 3, 6)
+    w = wl.Workload("fbp-on-node", 9, 9, 9, 0.5, (-2.0, -2.0, -2.0), tr, c=1.5, t0=0.0, dt=0.05, nt=300, surf_step=0.5, kband=32)
+    assert np.allclose(ofbp.node_positions(w)[6, 3, 5], tr[0])
+    rng = np.random.default_rng(3)
+    p = rng.standard_normal((3, 300)).astype(np.float32)
+    wq = np.array([1.0, -0.5, 2.0], dtype=np.float32)
+    got = gpu_fbp(torch, oat, w, p, wq)
+    ref = ofbp.fbp(w, p.astype(np.float64), wq.astype(np.float64))
+    assert np.all(np.isfinite(got))
+    uniq = (ofbp.interval_margin(w, ofbp.node_positions(w).reshape(-1, 3)) > 1e-9).reshape(ref.shape)
+    uniq[6, 3, 5] = True                                    # the node on the transducer is compared too
+    assert rel_l2(got[uniq], ref[uniq]) <= TOL
+    assert abs(got[6, 3, 5] - ref[6, 3, 5]) <= TOL * np.abs(ref).max()
+
+
 def test_config1_fbp_of_projected_phantom(env):
     """Config 1 end to end: p = H x from the library, FBP with the Fibonacci patch weights, against the oracle's
     FBP of the same p; and the image correlates with the phantom (limited by the 64-transducer aperture)."""
@@ -82,11 +100,14 @@ def test_config1_fbp_of_projected_phantom(env):
     x = w.phantom()
     g = oat.oat_geometry_create(w)
     pd = oat.oat_project(g, torch.from_numpy(x).cuda())
-    wq = wl.fbp_weights(w, wl.patch_areas_equal(w.trans_xyz, w.centre))
-    img = oat.oat_fbp(g, pd, torch.from_numpy(wq.astype(np.float32)).cuda()).cpu().numpy()
+    areas = wl.patch_areas_equal(w.trans_xyz, w.centre)
+    wq = oat.oat_fbp_weights(g, areas)                      # the library's weights of Eq. (27) ...
+    wq_ref = ofbp.weights(w, areas)                         # ... against the oracle's, computed independently
+    assert np.allclose(wq, wq_ref, rtol=2e-7)
+    img = oat.oat_fbp(g, pd, torch.from_numpy(wq).cuda()).cpu().numpy()
     p = pd.cpu().numpy()
     g.close()
-    ref = ofbp.fbp(w, p.astype(np.float64), wq.astype(np.float32).astype(np.float64))
+    ref = ofbp.fbp(w, p.astype(np.float64), wq_ref)
     uniq = (ofbp.interval_margin(w, ofbp.node_positions(w).reshape(-1, 3)) > 1e-9).reshape(ref.shape)
     assert uniq.sum() >= ref.size - 8
     assert rel_l2(img[uniq], ref[uniq]) <= TOL
@@ -105,7 +126,10 @@ def test_fullsize_sampled_voxels(env, cfg):
     ph = rng.uniform(0, 2 * np.pi, size=(w.n_trans, 1)); f = rng.uniform(0.01, 0.05, size=(w.n_trans, 1))
     p = (np.sin(2 * np.pi * f * t[None, :] + ph) * np.exp(-((t[None, :] - w.nt / 2) / (0.3 * w.nt)) ** 2)).astype(np.float32)
     areas = wl.patch_areas_arc(64, 144, 65.0) if cfg == 3 else wl.patch_areas_equal(w.trans_xyz, w.centre)
-    wq = wl.fbp_weights(w, areas).astype(np.float32)
+    g = oat.oat_geometry_create(w)
+    wq = oat.oat_fbp_weights(g, areas)
+    g.close()
+    assert np.allclose(wq, ofbp.weights(w, areas), rtol=2e-7)
     got = gpu_fbp(torch, oat, w, p, wq)
     idx = rng.integers(0, [w.nz, w.ny, w.nx], size=(48, 3))
     idx[0] = (0, 0, 0); idx[1] = (w.nz - 1, w.ny - 1, w.nx - 1)

@@ -64,9 +64,9 @@ def check_pair(env, w, x=None, y=None, tol=TOL):
     e1, e2 = rel_l2(hx, ref_hx), rel_l2(hty, ref_hty)
     assert e1 <= tol, f"H rel-L2 {e1:.3e}"
     assert e2 <= tol, f"H^T rel-L2 {e2:.3e}"
-    # element by element: no single output is off by more than a few 1e-4 of the vector's scale
-    assert np.max(np.abs(hx - ref_hx)) <= 10 * tol * np.max(np.abs(ref_hx))
-    assert np.max(np.abs(hty - ref_hty)) <= 10 * tol * np.max(np.abs(ref_hty))
+    # element by element: no single output is off by more than 3e-4 of the vector's peak
+    assert np.max(np.abs(hx - ref_hx)) <= 3 * tol * np.max(np.abs(ref_hx))
+    assert np.max(np.abs(hty - ref_hty)) <= 3 * tol * np.max(np.abs(ref_hty))
     lhs, rhs, rel = oat.oat_adjoint_check(g, torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda())
     assert rel <= tol, f"adjoint mismatch {rel:.3e}"
     assert abs(lhs - float(np.vdot(ref_hx, y))) <= 10 * tol * abs(lhs) + 1e-12
@@ -97,12 +97,34 @@ def test_non_cubic_grid_and_offset_origin(env):
 
 def test_coarse_time_sampling_falls_back_from_the_marching_kernels(env):
     """c dt = 9 voxels per sample: the ray anchors of a 32-sample band lie up to 144 voxels outside the box and do not
-    fit the packed list entries of the marching kernels, so the library must fall back to the
-    lane-per-sample kernels -- same operator, same tolerance."""
+    fit the packed queue entries of the marching kernels, so the library must fall back to the
+    generic lane-per-sample kernel -- same operator, same tolerance."""
     torch, orc, oat, wl = env
     w = wl.small(n=14, q=4, nt=40, spacing=0.05, radius=6.0, kband=32, dt=0.3)
     assert w.c * w.dt / w.spacing > 7.8
+    g = oat.oat_geometry_create(w)
+    assert not oat.oat_uses_marching(g) and not oat.oat_uses_marching(g, backproject=True)
+    g.close()
     check_pair(env, w)
+
+
+def test_record_index_limit_falls_back_from_the_marching_kernels(env):
+    """The marching kernels index cell records and face quads with 32 bits; a grid with more records must take the
+    generic kernel.  The limit is lowered here (oat_probe.h, "record_limit_log2") so that a small grid exceeds it:
+    the same selection branch as for a > 2^31-record grid, on a problem the oracle can check."""
+    torch, orc, oat, wl = env
+    w = wl.small(n=18, q=5, nt=75, kband=32, h=0.2)
+    x, y = w.phantom(), w.data_noise()
+    g = oat.oat_geometry_create(w)
+    assert oat.oat_uses_marching(g) and oat.oat_uses_marching(g, backproject=True)
+    oat.oat_set_variant(g, "record_limit_log2", 10)
+    assert not oat.oat_uses_marching(g) and not oat.oat_uses_marching(g, backproject=True)
+    assert rel_l2(gpu_project(torch, oat, w, x, g), orc.project(w, x.astype(np.float64))) <= TOL
+    assert rel_l2(gpu_backproject(torch, oat, w, y, g), orc.backproject(w, y.astype(np.float64))) <= TOL
+    oat.oat_set_variant(g, "record_limit_log2", 31)
+    assert oat.oat_uses_marching(g)
+    assert rel_l2(gpu_project(torch, oat, w, x, g), orc.project(w, x.astype(np.float64))) <= TOL
+    g.close()
 
 
 def test_config1_tiny_full(env):
@@ -219,28 +241,67 @@ def test_host_entry_points(env):
     g.close()
 
 
-# ------------------------------------------------------------------ larger configs
-def test_config2_transducer_subset(env):
-    """BASELINE.json config 2 on a seeded subset of 16 transducers (rows of H are independent;
-    H^T is a sum over transducers)."""
+# ------------------------------------------------------------------ larger configs: 2 and 4 at their full size
+@pytest.fixture(scope="module")
+def config2_full(env):
+    """BASELINE.json configs 2 / 4 share one geometry (128^3, 1,024 transducers); the oracle's H of the phantom on ALL
+    transducers is computed once (about a minute on 16 cores) and serves both tests."""
     torch, orc, oat, wl = env
     w = wl.config(2)
-    idx, ws = w.seeded_subset(16)
     x = w.phantom()
-    y = ws.data_noise()
-    g = oat.oat_geometry_create(ws)
-    hx = gpu_project(torch, oat, ws, x, g)
-    hty = gpu_backproject(torch, oat, ws, y, g)
+    return w, x, orc.project(w, x.astype(np.float64))
+
+
+def test_config2_full(env, config2_full):
+    """BASELINE.json config 2 in full: one H and one H^T on the 1,024-transducer geometry (its patch list, Morton order and
+    fused-A4 row counters), every output compared with the oracle."""
+    torch, orc, oat, wl = env
+    w, x, ref_hx = config2_full
+    y = w.data_noise()
+    g = oat.oat_geometry_create(w)
+    assert oat.oat_uses_marching(g) and oat.oat_uses_marching(g, backproject=True)
+    hx = gpu_project(torch, oat, w, x, g)
+    hty = gpu_backproject(torch, oat, w, y, g)
+    cnt = oat.oat_num_surface_samples(g)
     g.close()
-    e1 = rel_l2(hx, orc.project(ws, x.astype(np.float64)))
-    e2 = rel_l2(hty, orc.backproject(ws, y.astype(np.float64)))
-    print(f"config2[16]: H {e1:.2e}  H^T {e2:.2e}")
+    ref_hty = orc.backproject(w, y.astype(np.float64))
+    e1, e2 = rel_l2(hx, ref_hx), rel_l2(hty, ref_hty)
+    print(f"config2 full: H {e1:.2e}  H^T {e2:.2e}")
     assert e1 <= TOL and e2 <= TOL
+    assert np.max(np.abs(hx - ref_hx)) <= 3 * TOL * np.max(np.abs(ref_hx))
+    assert np.max(np.abs(hty - ref_hty)) <= 3 * TOL * np.max(np.abs(ref_hty))
+    ref_cnt = orc.count_samples(w)
+    assert abs(cnt - ref_cnt) <= max(2, 1e-6 * ref_cnt), (cnt, ref_cnt)
+
+
+def test_config4_cgls_full_geometry(env, config2_full):
+    """BASELINE.json config 4 on the full 1,024-transducer geometry: y = H A_true + 5 % noise (the oracle's H), 3 CGLS
+    iterations on the GPU.  The oracle's CGLS on the full problem would take ~8 operator applications; instead the
+    GPU iterate is checked with TWO oracle applications that pin the loop's arithmetic: (i) the first search direction
+    s_0 = H^T y and its norm (h_grad[0]) against the oracle's H^T y, (ii) the residual the GPU reports after 3 iterations
+    against ||y - H_oracle x_3|| / ||y|| evaluated by the oracle on the GPU's iterate."""
+    torch, orc, oat, wl = env
+    w, xt, ytrue = config2_full
+    rng = np.random.default_rng(4)
+    y = (ytrue + rng.standard_normal(ytrue.shape) * 0.05 * np.abs(ytrue).max()).astype(np.float32)
+    g = oat.oat_geometry_create(w)
+    yd = torch.from_numpy(y).cuda()
+    x3, res, grad = oat.oat_cgls(g, yd, 3)
+    hty = gpu_backproject(torch, oat, w, y, g)
+    g.close()
+    ref_hty = orc.backproject(w, y.astype(np.float64))
+    assert rel_l2(hty, ref_hty) <= TOL
+    assert abs(grad[0] - np.linalg.norm(ref_hty)) <= 1e-4 * np.linalg.norm(ref_hty)
+    r3 = y.astype(np.float64) - orc.project(w, x3.cpu().numpy().astype(np.float64))
+    res3 = np.linalg.norm(r3) / np.linalg.norm(y.astype(np.float64))
+    print(f"config4 full: residual after 3 CGLS iterations {res[3]:.6f} (GPU) vs {res3:.6f} (oracle H on the GPU iterate)")
+    assert abs(res[3] - res3) <= 2e-4 * res3
+    assert np.all(np.diff(res) <= 1e-6)
 
 
 def test_config4_cgls_first_iterations(env):
     """Row C1: first 3 CGLS iterations on a config-2-shaped problem (reduced transducer count so the
-    oracle finishes in seconds) against the oracle's CGLS; residual curve must match."""
+    oracle's own CGLS finishes in seconds) against the oracle's CGLS; the whole residual curve must match."""
     torch, orc, oat, wl = env
     w = wl.config(4)
     idx, ws = w.seeded_subset(6)
@@ -259,18 +320,17 @@ def test_config4_cgls_first_iterations(env):
     g.close()
 
 
-# ------------------------------------------------------------------ kernel variants
-@pytest.mark.parametrize("schedule", [0, 1])
-@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 1), ("project", 2), ("project", 3), ("project", 4),
-                                         ("backproject", 0), ("backproject", 1), ("backproject", 2), ("backproject", 3), ("backproject", 4)])
-def test_every_kernel_variant_matches_the_oracle(env, key, variant, schedule):
-    """each selectable kernel variant / work schedule computes the same operator."""
+# ------------------------------------------------------------------ the generic kernel (fall-back) on its own
+@pytest.mark.parametrize("key,variant", [("project", 0), ("project", 4), ("backproject", 0), ("backproject", 4)])
+def test_generic_and_marching_kernels_match_the_oracle(env, key, variant):
+    """the marching kernels (4) and the generic patch kernel (0: the fall-back and the sample counter)
+    compute the same operator."""
     torch, orc, oat, wl = env
     w = wl.small(n=18, q=5, nt=75, kband=32, h=0.2)        # h < spacing: several patches per ring block
     x, y = w.phantom(), w.data_noise()
     g = oat.oat_geometry_create(w)
-    oat.oat_set_variant(g, "schedule", schedule)
     oat.oat_set_variant(g, key, variant)
+    assert oat.oat_uses_marching(g, backproject=(key == "backproject")) == (variant == 4)
     if key == "project":
         e = rel_l2(gpu_project(torch, oat, w, x, g), orc.project(w, x.astype(np.float64)))
     else:
@@ -278,19 +338,17 @@ def test_every_kernel_variant_matches_the_oracle(env, key, variant, schedule):
     _, _, rel = oat.oat_adjoint_check(g, torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda())
     cnt = oat.oat_num_surface_samples(g)
     g.close()
-    assert e <= TOL and rel <= TOL, (key, variant, schedule, e, rel)
+    assert e <= TOL and rel <= TOL, (key, variant, e, rel)
     assert abs(cnt - orc.count_samples(w)) <= 2
 
 
-def test_both_schedules_on_config1(env):
+def test_generic_kernel_on_config1(env):
     torch, orc, oat, wl = env
     w = wl.config(1)
     x, y = w.phantom(), w.data_noise()
-    ref_hx, ref_hty, ref_cnt = orc.project(w, x.astype(np.float64)), orc.backproject(w, y.astype(np.float64)), orc.count_samples(w)
-    for schedule in (0, 1):
-        g = oat.oat_geometry_create(w)
-        oat.oat_set_variant(g, "schedule", schedule)
-        assert rel_l2(gpu_project(torch, oat, w, x, g), ref_hx) <= TOL
-        assert rel_l2(gpu_backproject(torch, oat, w, y, g), ref_hty) <= TOL
-        assert abs(oat.oat_num_surface_samples(g) - ref_cnt) <= max(2, 1e-6 * ref_cnt)
-        g.close()
+    g = oat.oat_geometry_create(w)
+    oat.oat_set_variant(g, "project", 0)
+    oat.oat_set_variant(g, "backproject", 0)
+    assert rel_l2(gpu_project(torch, oat, w, x, g), orc.project(w, x.astype(np.float64))) <= TOL
+    assert rel_l2(gpu_backproject(torch, oat, w, y, g), orc.backproject(w, y.astype(np.float64))) <= TOL
+    g.close()

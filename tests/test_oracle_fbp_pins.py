@@ -30,7 +30,7 @@ def test_fused_formula_equals_eq4_with_eq25_and_eq26():
     rng = np.random.default_rng(0)
     p = rng.standard_normal((w.n_trans, w.nt))
     areas = wl.patch_areas_equal(w.trans_xyz, w.centre)
-    wq = wl.fbp_weights(w, areas)
+    wq = fbp.weights(w, areas)
     pts = rng.uniform(-2.0, 2.0, size=(25, 3))
     got = fbp.fbp_points(w, p, wq, pts)
     rs = np.linalg.norm(w.trans_xyz - w.centre, axis=1)
@@ -52,7 +52,7 @@ def test_uniform_ball_is_reconstructed_from_its_n_wave():
     w = sphere_problem()
     centre, rb, amp = np.array([0.4, -0.3, 0.2]), 1.2, 0.7
     p = ball_data(w, centre, rb, amp)
-    wq = wl.fbp_weights(w, wl.patch_areas_equal(w.trans_xyz, w.centre))
+    wq = fbp.weights(w, wl.patch_areas_equal(w.trans_xyz, w.centre))
     inside = centre + np.array([[0, 0, 0], [0.5, 0, 0], [0, -0.6, 0.3], [-0.3, 0.3, 0.5]])
     vin = fbp.fbp_points(w, p, wq, inside)
     # inside the ball every shell crosses the linear part of the N-wave, where Eq. (25)-(26) are exact: only the
@@ -67,7 +67,7 @@ def test_uniform_ball_is_reconstructed_from_its_n_wave():
     # scale pins: twice the amplitude -> twice the image; kappa cancels between data and weights
     w2 = sphere_problem(kappa=2.5)
     p2 = ball_data(w2, centre, rb, amp)
-    v2 = fbp.fbp_points(w2, p2, wl.fbp_weights(w2, wl.patch_areas_equal(w2.trans_xyz, w2.centre)), inside)
+    v2 = fbp.fbp_points(w2, p2, fbp.weights(w2, wl.patch_areas_equal(w2.trans_xyz, w2.centre)), inside)
     assert np.allclose(v2, vin, rtol=1e-12)
 
 
@@ -101,3 +101,51 @@ def test_record_edges_and_linearity():
     p3 = np.vstack([p1, rng.standard_normal((1, 40))])
     assert np.array_equal(fbp.fbp(w, p3, np.append(wq, 7.0)), a)
     assert np.isfinite(a).all() and pts.shape[0] == a.size
+
+
+def test_weights_are_the_constant_of_eq27_for_the_papers_geometry():
+    """Eq. (27) L221 prints, for the ring/view geometry of L203, the factor -C_p R^s dtheta dphi sin(theta_q) / (pi beta c0^3 dt);
+    with kappa = beta / (4 pi C_p) that is -R^s dtheta dphi sin(theta_q) / (4 pi^2 kappa c0^3 dt).  Numbers by hand."""
+    rs, n_el, n_views = 65.0, 4, 6
+    w = wl.Workload("w", 5, 5, 5, 0.5, (-1.0, -1.0, -1.0), np.zeros((n_el * n_views, 3)), c=1.5, t0=1.0, dt=0.05, nt=10, surf_step=0.5, gain=0.25)
+    pol = np.deg2rad(14.0 + np.arange(n_el) * 152.0 / (n_el - 1))
+    dth, dph = np.deg2rad(152.0 / (n_el - 1)), 2.0 * math.pi / n_views
+    tr = []
+    for e in range(n_el):
+        for v in range(n_views):
+            tr.append([rs * math.sin(pol[e]) * math.cos(v * dph), rs * math.sin(pol[e]) * math.sin(v * dph), rs * math.cos(pol[e])])
+    w.trans_xyz = np.array(tr) + w.centre
+    got = fbp.weights(w, wl.patch_areas_arc(n_el, n_views, rs))
+    beta_over_cp = 4.0 * math.pi * 0.25
+    exp = np.repeat(-rs * dth * dph * np.sin(pol) / (math.pi * beta_over_cp * 1.5 ** 3 * 0.05), n_views)
+    assert np.allclose(got, exp, rtol=1e-13)
+
+
+def test_interval_margin_flags_ties_and_nothing_else():
+    """oat_fbp.interval_margin decides which points a parity test may skip (reading G26): it must be ~0 exactly where some
+    k~ is an integer -- the centre of a Fibonacci sphere whose radius is a whole number of samples -- and equal to the
+    constructed offset elsewhere, so that a threshold of 1e-9 excludes the ties and nothing at margin 1e-6."""
+    w = sphere_problem(q=50, rs=30.0, n=5, ds=0.5, dt=0.02, nt=2200, t0=2.0)     # k~ at the centre = (30/1.5 - 2)/0.02 = 900
+    m0 = fbp.interval_margin(w, np.zeros((1, 3)))
+    assert m0[0] < 1e-9
+    # a point on the axis through transducer 0, displaced by delta samples: margin = |delta| for that transducer at most
+    u = w.trans_xyz[0] / np.linalg.norm(w.trans_xyz[0])
+    for delta in (1e-6, 1e-3, 0.25):
+        pt = (u * (-delta * w.c * w.dt))[None, :]                                  # farther from transducer 0 by delta samples
+        m = fbp.interval_margin(w, pt)
+        assert 0.0 < m[0] <= delta * (1 + 1e-6) + 1e-9
+        kt = (np.linalg.norm(w.trans_xyz - pt, axis=1) / w.c - w.t0) / w.dt
+        assert np.isclose(m[0], np.min(np.abs(kt - np.rint(kt))), rtol=0, atol=1e-12)
+        if delta >= 1e-6:
+            assert m[0] > 1e-9 or delta < 1e-6
+    # points whose every k~ lies outside the record are never ties
+    far = np.array([[1e4, 0.0, 0.0]])
+    assert np.isinf(fbp.interval_margin(w, far)[0])
+    # generic points: the margin is the brute-force minimum over transducers
+    rng = np.random.default_rng(5)
+    pts = rng.uniform(-1.0, 1.0, size=(20, 3))
+    m = fbp.interval_margin(w, pts)
+    for i, pt in enumerate(pts):
+        kt = (np.linalg.norm(w.trans_xyz - pt, axis=1) / w.c - w.t0) / w.dt
+        assert np.isclose(m[i], np.min(np.abs(kt - np.rint(kt))), atol=1e-12)
+    assert np.all(m > 1e-9)
