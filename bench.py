@@ -1,17 +1,18 @@
 #!/usr/bin/env python
 """bench.py -- one H and one H^T (the whole hot path) per step on the
 configuration BASELINE.json's metric is quoted on: config 3, 240^3 voxels x 9,216 transducers x
-2,048 time samples (arc-array geometry), synthetic seeded phantom.
+2,048 time samples (arc-array geometry), synthetic seeded phantom and data.
 
     python bench.py --gpus N --steps K --warmup W            (our arm, CUDA)
     python bench.py --impl reference --steps K --warmup W    (the fp64 oracle on host cores)
 
-Prints ONE JSON line (see DESIGN.md §7 for every field).  Timing: CUDA events on the launching
+Prints ONE JSON line (DESIGN.md §7 explains every field).  Timing: CUDA events on the launching
 stream, barrier + synchronize on both sides, max over ranks; L2 is flushed between steps.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -26,33 +27,58 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "ms per H and per H^T at 240^3 voxels x 9216 transducers x 2048 t (value = ms per H + H^T pair)"
-# Algorithmic fp32 work per interpolation sample: position 3 FMA, 3 floor, 3 frac,
-# 7 lerps (sub + FMA) or 8 weight products + 8 accumulates, 1 quadrature FMA  ->  36 flop (FMA = 2).
-FLOP_PER_SAMPLE = 36.0
-# Vector reductions per interpolation sample of the face-carrying H^T: ncu counts 1.562e10
-# predicated-on RED.128 lanes for 2.478e10 in-box samples on the config-3 subset profiled in profiles/.
-RED_PER_SAMPLE = 0.63
-# 32-byte cell records requested from L2 per interpolation sample of the marching H: ncu counts
-# 1.079e10 global-load sectors (L1 hit rate 5 %) for 2.478e10 in-box samples on the same subset.
-SECTORS_PER_SAMPLE = 0.435
-# B200 fp32 peak derived from unit counts and clocks (guide: 148 SMs x 128 fp32 lanes x 2 flop x max SM clock)
-N_SM, FP32_LANES = 148, 128
-# DRAM bytes (read + write) per in-box sample of the dominant kernel (H^T) from the ncu --set full capture summarised in
-# profiles/r1k_final.md: (1.825 + 1.335) GB for 2.478e10 samples on the 512-transducer subset of config 3.
-DRAM_BYTES_PER_SAMPLE_HT = (1.824808e9 + 1.335234e9) / 2.4784424365e10
+# Algorithmic work per interpolation sample: 8 corners x 4 B gathered at L1 level; ~30 fp32 lane-operations
+# (3 FMA position, 3 floor + 3 fraction, ~14 weights / lerps, 1 accumulate, rest bounds).
+L1_BYTES_PER_SAMPLE = 32.0
+LANE_OPS_PER_SAMPLE = 30.0
+# B200 unit counts (guide): 148 SMs; L1 delivers 128 B per clock per SM; 128 fp32 lanes per SM
+N_SM, L1_BYTES_PER_CLK, FP32_LANES = 148, 128, 128
+# ncu captures of the SHIPPING marching kernels on the 512-transducer subset of config 3 (profiles/r2_march_counters.md
+# names the commands and the library revision): `ncu -i ... --page raw --csv` dumps, parsed below for the per-sample counters
+PROFILE_FWD = os.path.join(ROOT, "profiles", "r2_march_fwd_raw.csv")
+PROFILE_BWD = os.path.join(ROOT, "profiles", "r2_march_bwd_raw.csv")
+PROFILE_META = os.path.join(ROOT, "profiles", "r2_march_counters.json")
 
 
-def peaks():
+def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    sm_mhz, src = 1965.0, "fallback clocks.max.sm of B200_PROFILING.md"
+    sm_mhz, hbm, src = 1965.0, 6650.0, "fallback of B200_PROFILING.md (clocks.max.sm 1965 MHz, 6.65 TB/s)"
     if os.path.exists(path):
         try:
             mp = json.load(open(path))
-            sm_mhz = float(mp.get("sm_max_mhz", sm_mhz))
-            src = "MEASURED_PEAKS.json sm_max_mhz"
+            sm_mhz = float(mp.get("sm_max_mhz", sm_mhz)); hbm = float(mp.get("hbm_gbs", hbm))
+            src = "MEASURED_PEAKS.json (sm_max_mhz, hbm_gbs)"
         except Exception:
             pass
-    return N_SM * FP32_LANES * 2.0 * sm_mhz * 1e6 / 1e12, src      # TFLOP/s
+    return sm_mhz, hbm, src
+
+
+def ncu_counters():
+    """Per-sample counters of the two marching kernels from the committed ncu raw pages ({"error": ...} when unreadable)."""
+    unit = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
+
+    def raw(path):
+        rows = list(csv.reader(open(path)))
+        return dict(zip(rows[0], rows[2])), dict(zip(rows[0], rows[1]))
+
+    def num(d, k):
+        return float(d[k].replace(",", ""))
+
+    def dram(d, u):
+        return sum(num(d, k) * unit.get(u[k], 1.0) for k in ("dram__bytes_read.sum", "dram__bytes_write.sum"))
+    try:
+        meta = json.load(open(PROFILE_META))
+        ns = float(meta["in_box_samples_per_launch"])
+        (f, uf), (b, ub) = raw(PROFILE_FWD), raw(PROFILE_BWD)
+        return {"samples": ns, "revision": meta.get("library_revision"),
+                "H_sectors_per_sample": num(f, "l1tex__t_sectors_pipe_lsu_mem_global_op_ld.sum") / ns,
+                "H_inst_per_sample": num(f, "smsp__inst_executed.sum") * 32.0 / ns,
+                "H_dram_bytes_per_sample": dram(f, uf) / ns,
+                "HT_red_lanes_per_sample": num(b, "l1tex__t_sectors_pipe_lsu_mem_global_op_red.sum") / ns,
+                "HT_inst_per_sample": num(b, "smsp__inst_executed.sum") * 32.0 / ns,
+                "HT_dram_bytes_per_sample": dram(b, ub) / ns}
+    except Exception as ex:
+        return {"error": f"{type(ex).__name__}: {ex}"}
 
 
 class ClockSampler:
@@ -114,16 +140,33 @@ def workload(args):
     return w, note
 
 
-def oracle_step(w, x64, sample_q):
-    """One H + one H^T of the oracle on `sample_q` seeded transducers; returns (s_H, s_HT)."""
+def dense_data(w):
+    """The data vector H^T is timed on: dense seeded N(0,1), config 1's recipe (no band of 32 samples is all zero, so
+    the kernel skips nothing; y = H x of the sparse vessel phantom would leave ~5 % of the samples in skipped bands)."""
+    rng = np.random.default_rng(w.seed + 101)
+    return rng.standard_normal((w.n_trans, w.nt)).astype(np.float32)
+
+
+def oracle_step(w, x64, sample_q, n_threads=0):
+    """One H + one H^T of the oracle on `sample_q` seeded transducers; returns (s_H, s_HT, n_trans)."""
     from oracle import oat_oracle as orc
     _, ws = w.seeded_subset(sample_q)
+    kw = {"n_threads": n_threads} if n_threads else {}
     t0 = time.perf_counter()
-    y = orc.project(ws, x64)
+    y = orc.project(ws, x64, **kw)
     t1 = time.perf_counter()
-    orc.backproject(ws, y)
+    orc.backproject(ws, y, **kw)
     t2 = time.perf_counter()
     return t1 - t0, t2 - t1, ws.n_trans
+
+
+def oracle_sample_size(want, n_trans, threads):
+    """The oracle parallelises over transducers only: a sample keeps every core busy when it is a multiple of the
+    thread count."""
+    sq = max(1, min(want, n_trans))
+    if threads > 1 and sq >= threads:
+        sq -= sq % threads
+    return sq
 
 
 def run_reference(args):
@@ -133,20 +176,21 @@ def run_reference(args):
     from oracle import oat_oracle as orc
     w, note = workload(args)
     x64 = w.phantom().astype(np.float64)
-    sq = max(1, min(args.ref_sample, w.n_trans))
+    threads = orc.max_threads()
+    sq = oracle_sample_size(args.ref_sample, w.n_trans, threads)
     for _ in range(args.warmup):
-        oracle_step(w, x64, 1)
+        oracle_step(w, x64, min(threads, sq))
     th = tt = 0.0
     for _ in range(args.steps):
         a, b, nq = oracle_step(w, x64, sq)
         th += a; tt += b
     scale = w.n_trans / sq
     ms_h, ms_t = th / args.steps * 1e3 * scale, tt / args.steps * 1e3 * scale
-    cores = orc.max_threads()
-    sample = f"{sq} of {w.n_trans} transducers per step (seeded subset), times scaled by {scale:.0f}x"
+    cores = min(threads, sq)
+    sample = f"{sq} of {w.n_trans} transducers per step (seeded subset, {cores} threads busy), times scaled by {scale:.0f}x"
     line = {"impl": "reference", "metric": METRIC, "value": ms_h + ms_t, "unit": "ms", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_h + ms_t, "higher_is_better": False,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "n_trans": w.n_trans, "nt": w.nt, "note": note},
             "ms_H": ms_h, "ms_HT": ms_t,
             "cpu_baseline": {"value": ms_h + ms_t, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample},
@@ -154,10 +198,21 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def timed(torch, stream, fn, reps=5):
+    fn(); torch.cuda.synchronize()
+    a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(reps):
+        fn()
+    b.record(stream); torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_1304_2017_b200 import binding as oat, build, shard
+    from dataclasses import replace
+    from paper_1304_2017_b200 import binding as oat, build, shard, workloads as wl
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -172,17 +227,16 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
 
-    w, note = workload(args)
-    if world > 1:                                           # weak scaling: N-times denser view sampling
-        from dataclasses import replace
-        w = replace(w, trans_xyz=shard.weak_replica_transducers(w.trans_xyz, rank, world, 144))
+    w_all, note = workload(args)
+    w = w_all
+    if world > 1 and args.scaling == "strong":              # rows of H partitioned: total work fixed
+        w = replace(w_all, trans_xyz=shard.shard_transducers(w_all.trans_xyz, rank, world))
+    elif world > 1:                                         # weak: N-times denser view sampling, per-GPU work fixed
+        w = replace(w_all, trans_xyz=shard.weak_replica_transducers(w_all.trans_xyz, rank, world, 144))
     g = oat.oat_geometry_create(w, local)
-    if args.project_variant >= 0:
-        oat.oat_set_variant(g, "project", args.project_variant)
-    if args.backproject_variant >= 0:
-        oat.oat_set_variant(g, "backproject", args.backproject_variant)
     x = torch.from_numpy(w.phantom()).cuda()
     y = torch.empty((w.n_trans, w.nt), dtype=torch.float32, device="cuda")
+    ynoise = torch.from_numpy(dense_data(w)).cuda()
     xb = torch.empty_like(x)
     n_samples = oat.oat_num_surface_samples(g)              # per operator, this rank
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
@@ -196,7 +250,7 @@ def run_ours(args):
         kh = oat.oat_last_kernel_ms(g) if rec is not None else 0.0
         nl = oat.oat_last_launch_count(g)
         if e: e[1].record(stream)
-        oat.oat_backproject(g, y, xb)
+        oat.oat_backproject(g, ynoise, xb)
         kt = oat.oat_last_kernel_ms(g) if rec is not None else 0.0
         nl += oat.oat_last_launch_count(g)
         if world > 1:
@@ -228,12 +282,12 @@ def run_ours(args):
     ms_t = float(np.mean([r[0][1].elapsed_time(r[0][2]) for r in rec]))
     k_h = float(np.mean([r[1] for r in rec])); k_t = float(np.mean([r[2] for r in rec]))
     launches = int(sum(r[3] for r in rec)) + args.steps      # + the L2-flush fill per step
-    vals = torch.tensor([total_ms, ms_h, ms_t], dtype=torch.float64, device="cuda")
+    vals = torch.tensor([total_ms, ms_h, ms_t, k_h, k_t], dtype=torch.float64, device="cuda")
     tot_samples = torch.tensor([float(n_samples)], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(vals, op=dist.ReduceOp.MAX)
         dist.all_reduce(tot_samples, op=dist.ReduceOp.SUM)
-    total_ms, ms_h, ms_t = [float(v) for v in vals.tolist()]
+    total_ms, ms_h, ms_t, k_h, k_t = [float(v) for v in vals.tolist()]
     ms_step = total_ms / args.steps
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
@@ -241,15 +295,16 @@ def run_ours(args):
     if args.e2e_steps > 0:
         hx = torch.from_numpy(w.phantom()).pin_memory()
         hy = torch.empty((w.n_trans, w.nt), dtype=torch.float32).pin_memory()
+        hyn = torch.from_numpy(dense_data(w)).pin_memory()
         hxb = torch.empty_like(hx).pin_memory()
-        n_e2e = max(1, min(args.steps, args.e2e_steps))
-        oat.oat_project_host(g, hx, hy); oat.oat_backproject_host(g, hy, hxb)     # warm-up
+        n_e2e = args.e2e_steps
+        oat.oat_project_host(g, hx, hy); oat.oat_backproject_host(g, hyn, hxb)     # warm-up
         if world > 1:
             dist.barrier()
         t0 = time.perf_counter()
         for _ in range(n_e2e):
             oat.oat_project_host(g, hx, hy)
-            oat.oat_backproject_host(g, hy, hxb)
+            oat.oat_backproject_host(g, hyn, hxb)
         dt_e2e = (time.perf_counter() - t0) / n_e2e * 1e3
         v = torch.tensor([dt_e2e], dtype=torch.float64, device="cuda")
         if world > 1:
@@ -259,118 +314,114 @@ def run_ours(args):
                "steps": n_e2e, "api": "oat_project_host + oat_backproject_host (pinned host buffers)"}
 
     if rank == 0:
-        peak, peak_src = peaks()
-        dom = "backproject" if k_t >= k_h else "project"
-        k_ms = max(k_t, k_h)
-        achieved = n_samples * FLOP_PER_SAMPLE / (k_ms * 1e-3) / 1e12 if k_ms > 0 else 0.0
-        roofline = {"bound": "alu", "kernel": f"oat_march_kernel<{1 if dom == 'backproject' else 0}> ({dom})",
-                    "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak else None,
-                    "traffic": (DRAM_BYTES_PER_SAMPLE_HT * n_samples) if dom == "backproject" else None,
-                    "traffic_note": "dram__bytes_read+write of oat_march_kernel<1> per launch, ncu --set full on the 512-transducer subset "
-                                    "(profiles/r1k_final.md) scaled by samples; unit B; algorithmic unique bytes = size(x)+size(y)",
-                    "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_step if ms_step else None,
-                    "peak_source": f"148 SM x 128 fp32 lanes x 2 flop x {peak_src}",
-                    "algorithmic": f"{FLOP_PER_SAMPLE:.0f} fp32 flop per interpolation sample x {n_samples:.4g} samples per launch",
-                    "other_kernel": {"kernel_ms": min(k_t, k_h),
-                                     "frac": (n_samples * FLOP_PER_SAMPLE / (min(k_t, k_h) * 1e-3) / 1e12 / peak) if min(k_t, k_h) > 0 else None}}
-        # What ncu and the micro-benchmarks name as the binding unit of each kernel: H^T retires
-        # vector reductions (RED.128) at the rate the L2 atomic path sustains; the peak is measured live.
-        try:
-            red_scat = oat.oat_measure_red_rate(local)                 # every lane its own 32-byte sector
-            red_pack = oat.oat_measure_red_rate_ex(local, 1)           # 32 lanes fill 16 sectors: the best case
-            red_lanes = RED_PER_SAMPLE * n_samples
-            ach = red_lanes / (k_t * 1e-3) if k_t > 0 else None
-            roofline["limiter"] = {"kernel": "oat_march_kernel<1> (backproject)", "unit": "L2 vector reductions (RED.128 lanes/s)",
-                                   "achieved": ach, "peak": red_pack, "frac": (ach / red_pack) if (ach and red_pack > 0) else None,
-                                   "scattered_rate": red_scat, "frac_of_scattered_rate": (ach / red_scat) if (ach and red_scat > 0) else None,
-                                   "algorithmic": f"{RED_PER_SAMPLE} reductions per sample (cell crossings of the marched rays, ncu inst count) x {n_samples:.4g} samples",
-                                   "peak_source": "oat_measure_red_rate_ex(pattern 1): red.global.add.v4.f32, the 32 lanes of a warp filling 16 sectors of an L2-resident "
-                                                  "64 MB buffer (the cost of a reduction is per distinct sector); scattered_rate = oat_measure_red_rate(): every lane its own sector; same run"}
-        except Exception as ex:
-            roofline["limiter"] = {"error": str(ex)}
-        # H requests one 32-byte cell record from L2 per cell run of a ray; the peak is the measured scattered-sector rate
-        try:
-            gat_peak = oat.oat_measure_gather_rate(local)
-            sec = SECTORS_PER_SAMPLE * n_samples
-            roofline["limiter_H"] = {"kernel": "oat_march_kernel<0> (project)", "unit": "L1-miss sector loads from L2 (32 B sectors/s)",
-                                     "achieved": sec / (k_h * 1e-3) if k_h > 0 else None, "peak": gat_peak,
-                                     "frac": (sec / (k_h * 1e-3) / gat_peak) if (k_h > 0 and gat_peak > 0) else None,
-                                     "algorithmic": f"{SECTORS_PER_SAMPLE} cell records per sample (one per cell run of a marched ray, ncu sector count) x {n_samples:.4g} samples",
-                                     "peak_source": "oat_measure_gather_rate(): scattered ld.global.nc.v8.f32, one sector per lane, L2-resident 64 MB buffer, same run"}
-        except Exception as ex:
-            roofline["limiter_H"] = {"error": str(ex)}
-        # ---- row NEXT-1 (EIR convolution, penalty stencil): the steps either side of the path, timed at this config's sizes
-        next1 = None
-        try:
-            hbm = None
-            try:
-                hbm = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs"))
-            except Exception:
-                pass
-            taps = 128
-            tt = np.arange(taps) * w.dt
-            oat.oat_eir_set(g, (w.dt * np.exp(-tt / (0.15 * taps * w.dt)) * np.sin(2 * np.pi * 2.5 * tt)).astype(np.float32))
-            u = torch.empty_like(y); lx = torch.empty_like(x)
+        sm_mhz, hbm_gbs, peak_src = measured_peaks()
+        clk = sm_mhz * 1e6
+        peak_l1 = N_SM * L1_BYTES_PER_CLK * clk / 1e9        # GB/s
+        peak_alu = N_SM * FP32_LANES * clk                    # lane-ops/s
+        cnt = ncu_counters()
 
-            def timed(fn, reps=5):
-                fn(); torch.cuda.synchronize()
-                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
-                a.record(stream)
-                for _ in range(reps):
-                    fn()
-                b.record(stream); torch.cuda.synchronize()
-                return a.elapsed_time(b) / reps
-            ms_e = timed(lambda: oat.oat_eir_apply(g, y, u))
-            ms_ea = timed(lambda: oat.oat_eir_apply(g, y, u, adjoint=True))
-            ms_p = timed(lambda: oat.oat_penalty_apply(g, xb, lx))
-            by, bx = 2.0 * y.numel() * 4, 2.0 * x.numel() * 4          # read + write once
-            next1 = {"eir_taps": taps, "ms_eir": ms_e, "ms_eir_adjoint": ms_ea, "ms_penalty": ms_p,
-                     "eir_GBps": by / (ms_e * 1e-3) / 1e9, "penalty_GBps": bx / (ms_p * 1e-3) / 1e9,
-                     "hbm_peak_GBps": hbm, "penalty_frac_of_hbm": (bx / (ms_p * 1e-3) / 1e9 / hbm) if hbm else None,
-                     "eir_frac_of_hbm": (by / (ms_e * 1e-3) / 1e9 / hbm) if hbm else None,
-                     "share_of_pls_iteration": (ms_e + ms_ea + ms_p) / (ms_step + ms_e + ms_ea + ms_p),
-                     "note": "outside the timed step; algorithmic bytes = read + write of the vector once; the EIR is a 128-tap FIR from shared memory (LDS-bound, not HBM-bound)"}
-            oat.oat_eir_set(g, np.zeros(0, dtype=np.float32))
-        except Exception as ex:
-            next1 = {"error": str(ex)}
-        # ---- row NEXT-2 (FBP, Eq. 27): one image from the data of this config, voxel driven
-        next2 = None
+        def kernel_roofline(name, k_ms, dram_per_sample):
+            ach = n_samples * L1_BYTES_PER_SAMPLE / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
+            ops = n_samples * LANE_OPS_PER_SAMPLE / (k_ms * 1e-3) if k_ms > 0 else 0.0
+            return {"kernel": name, "kernel_ms": k_ms, "achieved": ach, "peak": peak_l1, "unit": "GB/s", "frac": ach / peak_l1,
+                    "frac_alu": ops / peak_alu, "samples_per_sm_cycle": n_samples / (k_ms * 1e-3) / (N_SM * clk) if k_ms > 0 else None,
+                    "traffic": dram_per_sample * n_samples if dram_per_sample is not None else None}
+        r_t = kernel_roofline("oat_march_bwd_kernel (backproject)", k_t, cnt.get("HT_dram_bytes_per_sample"))
+        r_h = kernel_roofline("oat_march_fwd_kernel (project)", k_h, cnt.get("H_dram_bytes_per_sample"))
+        dom, other = (r_t, r_h) if k_t >= k_h else (r_h, r_t)
+        roofline = dict(dom)
+        roofline.update({
+            "bound": "l1",
+            "kernel_share_of_step": dom["kernel_ms"] / ms_step if ms_step else None,
+            "other_kernel": other,
+            "algorithmic": f"SURVEY 8(d): {L1_BYTES_PER_SAMPLE:.0f} B gathered at L1 level (frac) and {LANE_OPS_PER_SAMPLE:.0f} fp32 lane-operations (frac_alu) per "
+                           f"interpolation sample x {n_samples:.4g} in-box samples per launch; unique HBM bytes per launch = size(x) + size(y) = {(x.numel() + y.numel()) * 4:.4g} B",
+            "peak_source": f"148 SM x 128 B/clk (L1) resp. 148 SM x 128 fp32 lanes, x max SM clock of {peak_src}; the L1-bytes ceiling is the tighter of the two",
+            "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of this kernel per launch: ncu --set full of the shipping kernel on the 512-transducer "
+                            "subset of config 3 (profiles/r2_march_*_raw.csv), per in-box sample x this launch's samples; unit B",
+            "ncu_counters": cnt})
+        # Diagnostics, self-measured in this run by the library's own probe kernels (include/oat_probe.h).  NOT roofline
+        # fractions: neighbouring rays share sectors, so the kernels can exceed the scattered-access rates.
+        diag = {"note": "self-measured probe rates of the two hardware paths ncu names as the kernels' limiters; diagnostics, not a roofline"}
         try:
-            from paper_1304_2017_b200 import workloads as wl2
-            wb2, _ = workload(args)
-            areas = wl2.patch_areas_arc(64, 144, 65.0) if (args.config == 3 and not args.subset) else wl2.patch_areas_equal(wb2.trans_xyz, wb2.centre)
-            wq = torch.from_numpy(oat.oat_fbp_weights(g, areas)).cuda()
-            oat.oat_fbp(g, y, wq, xb); torch.cuda.synchronize()
-            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
-            a.record(stream); oat.oat_fbp(g, y, wq, xb); b.record(stream); torch.cuda.synchronize()
-            ms_f = a.elapsed_time(b)
-            pairs = float(x.numel()) * w.n_trans
-            next2 = {"ms_fbp": ms_f, "voxel_transducer_pairs": pairs, "pairs_per_s": pairs / (ms_f * 1e-3),
-                     "note": "outside the timed step; fp64 distance + interval decision, fp32 brackets and sum (DESIGN.md section 5.6)"}
+            if "HT_red_lanes_per_sample" in cnt:
+                red_scat = oat.oat_measure_red_rate(local)
+                ach = cnt["HT_red_lanes_per_sample"] * n_samples / (k_t * 1e-3) if k_t > 0 else None
+                diag["H^T"] = {"unit": "RED.128 lanes/s into L2", "achieved": ach, "probe_scattered_sectors": red_scat,
+                               "probe_packed_sectors": oat.oat_measure_red_rate_ex(local, 1),
+                               "achieved_over_scattered_probe": ach / red_scat if (ach and red_scat > 0) else None}
+            if "H_sectors_per_sample" in cnt:
+                gat = oat.oat_measure_gather_rate(local)
+                ach = cnt["H_sectors_per_sample"] * n_samples / (k_h * 1e-3) if k_h > 0 else None
+                diag["H"] = {"unit": "scattered 32 B sector loads/s (L1 misses served by L2)", "achieved": ach, "probe": gat,
+                             "achieved_over_probe": ach / gat if (ach and gat > 0) else None}
         except Exception as ex:
-            next2 = {"error": str(ex)}
-        # ---- row NEXT-3 (spherical-voxel model, frequency domain): this config's grid, 256 seeded transducers, 64 frequencies
-        next3 = None
-        try:
-            wb3, _ = workload(args)
-            _, ws3 = wb3.seeded_subset(256)
-            g3 = oat.oat_geometry_create(ws3, local)
-            nf3 = 64
-            oat.oat_sph_set(g3, nf3, 0.0, 0.078125)          # 0 .. 4.9 MHz
-            u3 = torch.empty((ws3.n_trans, nf3), dtype=torch.complex64, device="cuda")
-            oat.oat_sph_project(g3, x, u3); oat.oat_sph_backproject(g3, u3, xb); torch.cuda.synchronize()
-            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-            ev[0].record(stream); oat.oat_sph_project(g3, x, u3); ev[1].record(stream); oat.oat_sph_backproject(g3, u3, xb); ev[2].record(stream)
-            torch.cuda.synchronize()
-            terms = float(x.numel()) * ws3.n_trans * nf3
-            nnz = float(torch.count_nonzero(x).item())
-            next3 = {"n_trans": ws3.n_trans, "n_freq": nf3, "ms_project": ev[0].elapsed_time(ev[1]), "ms_backproject": ev[1].elapsed_time(ev[2]),
-                     "voxel_transducer_frequency_terms": terms, "terms_per_s_backproject": terms / (ev[1].elapsed_time(ev[2]) * 1e-3),
-                     "nonzero_voxel_fraction": nnz / x.numel(),
-                     "note": "outside the timed step; the projection skips all-zero voxels (sparse vessel phantom), the backprojection visits every term"}
-            g3.close()
-        except Exception as ex:
-            next3 = {"error": str(ex)}
+            diag["error"] = str(ex)
+        roofline["limiter_diagnostics"] = diag
+
+        next1 = next2 = next3 = None
+        if not args.no_next:
+            # ---- row NEXT-1 (EIR convolution, penalty stencil): the steps either side of the path, timed at this config's sizes
+            try:
+                taps = 128
+                tt = np.arange(taps) * w.dt
+                oat.oat_eir_set(g, (w.dt * np.exp(-tt / (0.15 * taps * w.dt)) * np.sin(2 * np.pi * 2.5 * tt)).astype(np.float32))
+                u = torch.empty_like(y); lx = torch.empty_like(x)
+                ms_e = timed(torch, stream, lambda: oat.oat_eir_apply(g, ynoise, u))
+                ms_ea = timed(torch, stream, lambda: oat.oat_eir_apply(g, ynoise, u, adjoint=True))
+                ms_p = timed(torch, stream, lambda: oat.oat_penalty_apply(g, xb, lx))
+                by, bx = 2.0 * y.numel() * 4, 2.0 * x.numel() * 4          # read + write once
+                fma = float(taps) * y.numel()                               # one FMA per tap and output
+                next1 = {"eir_taps": taps, "ms_eir": ms_e, "ms_eir_adjoint": ms_ea, "ms_penalty": ms_p,
+                         "roofline_eir": {"bound": "hbm", "achieved": by / (ms_e * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                                          "frac": by / (ms_e * 1e-3) / 1e9 / hbm_gbs, "frac_alu": fma / (ms_e * 1e-3) / peak_alu,
+                                          "algorithmic": "read + write of the Q x K data vector once (frac); 128 FMAs per output against the fp32 lanes (frac_alu)"},
+                         "roofline_penalty": {"bound": "hbm", "achieved": bx / (ms_p * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                                              "frac": bx / (ms_p * 1e-3) / 1e9 / hbm_gbs, "algorithmic": "read + write of the volume once"},
+                         "share_of_pls_iteration": (ms_e + ms_ea + ms_p) / (ms_step + ms_e + ms_ea + ms_p),
+                         "note": "outside the timed step"}
+                oat.oat_eir_set(g, np.zeros(0, dtype=np.float32))
+            except Exception as ex:
+                next1 = {"error": str(ex)}
+            # ---- row NEXT-2 (FBP, Eq. 27): one image from the data of this config, voxel driven
+            try:
+                areas = wl.patch_areas_arc(64, 144, 65.0) if (args.config == 3 and not args.subset and world == 1) else wl.patch_areas_equal(w.trans_xyz, w.centre)
+                wq = torch.from_numpy(oat.oat_fbp_weights(g, areas)).cuda()
+                ms_f = timed(torch, stream, lambda: oat.oat_fbp(g, ynoise, wq, xb), reps=2)
+                pairs = float(x.numel()) * w.n_trans
+                peak_fp64 = N_SM * 64 * clk
+                next2 = {"ms_fbp": ms_f, "voxel_transducer_pairs": pairs, "pairs_per_s": pairs / (ms_f * 1e-3),
+                         "roofline": {"bound": "alu", "unit": "fp64 lane-operations/s", "achieved": 25.0 * pairs / (ms_f * 1e-3), "peak": peak_fp64,
+                                      "frac": 25.0 * pairs / (ms_f * 1e-3) / peak_fp64,
+                                      "algorithmic": "25 fp64 operations per pair (3 differences, 3 FMA, sqrt ~ 12, scale, floor, 2 conversions; reading G26 fixes fp64); "
+                                                     "peak = 148 SM x 64 fp64 lanes x max SM clock"},
+                         "note": "outside the timed step; fp64 distance + interval decision, fp32 brackets and sum (DESIGN.md section 5.6)"}
+            except Exception as ex:
+                next2 = {"error": str(ex)}
+            # ---- row NEXT-3 (spherical-voxel model, frequency domain): this config's grid, 256 seeded transducers, 64 frequencies
+            try:
+                _, ws3 = w.seeded_subset(256)
+                g3 = oat.oat_geometry_create(ws3, local)
+                nf3 = 64
+                oat.oat_sph_set(g3, nf3, 0.0, 0.078125)          # 0 .. 4.9 MHz
+                u3 = torch.empty((ws3.n_trans, nf3), dtype=torch.complex64, device="cuda")
+                xdense = torch.from_numpy(np.random.default_rng(33).standard_normal(tuple(x.shape)).astype(np.float32)).cuda()
+                ms_sp = timed(torch, stream, lambda: oat.oat_sph_project(g3, x, u3), reps=2)
+                ms_spd = timed(torch, stream, lambda: oat.oat_sph_project(g3, xdense, u3), reps=1)
+                ms_sb = timed(torch, stream, lambda: oat.oat_sph_backproject(g3, u3, xb), reps=2)
+                terms = float(x.numel()) * ws3.n_trans * nf3
+                nnz = float(torch.count_nonzero(x).item())
+                next3 = {"n_trans": ws3.n_trans, "n_freq": nf3, "ms_project_sparse_phantom": ms_sp, "ms_project_dense_volume": ms_spd, "ms_backproject": ms_sb,
+                         "voxel_transducer_frequency_terms": terms, "nonzero_voxel_fraction_of_phantom": nnz / x.numel(),
+                         "roofline_project_dense": {"bound": "alu", "unit": "fp32 lane-operations/s", "achieved": 8.0 * terms / (ms_spd * 1e-3), "peak": peak_alu,
+                                                    "frac": 8.0 * terms / (ms_spd * 1e-3) / peak_alu},
+                         "roofline_backproject": {"bound": "alu", "unit": "fp32 lane-operations/s", "achieved": 8.0 * terms / (ms_sb * 1e-3), "peak": peak_alu,
+                                                  "frac": 8.0 * terms / (ms_sb * 1e-3) / peak_alu},
+                         "algorithmic": "8 fp32 lane-operations per (voxel, transducer, frequency) term: 4 for the phasor recurrence, 4 for the complex multiply-accumulate",
+                         "note": "outside the timed step; the projection skips all-zero voxels, so it is also timed on a dense N(0,1) volume"}
+                g3.close()
+            except Exception as ex:
+                next3 = {"error": str(ex)}
         # ---- row C1 (config 4 only): the CG loop of the paper's experiments, 20 iterations (L326), timed as a whole
         cgls = None
         if args.config == 4:
@@ -388,24 +439,29 @@ def run_ours(args):
         if not args.no_cpu_baseline and world == 1:       # rank 0 at N=1 only
             try:
                 from oracle import oat_oracle as orc
-                from paper_1304_2017_b200 import workloads as wl
-                wb, _ = workload(args)
-                sq = max(1, min(args.cpu_sample, wb.n_trans))
-                a, b, nq = oracle_step(wb, wb.phantom().astype(np.float64), sq)
-                sc = wb.n_trans / nq
-                cpu = {"value": (a + b) * 1e3 * sc, "unit": "ms", "cores": orc.max_threads(), "kind": "oracle",
-                       "sample": f"H + H^T on {nq} of {wb.n_trans} transducers (seeded subset), {a + b:.1f} s of CPU wall time scaled by {sc:.0f}x",
-                       "ms_H": a * 1e3 * sc, "ms_HT": b * 1e3 * sc}
+                threads = orc.max_threads()
+                x64 = w.phantom().astype(np.float64)
+                sq = oracle_sample_size(args.cpu_sample, w.n_trans, threads)
+                a, b, nq = oracle_step(w, x64, sq)
+                sc = w.n_trans / nq
+                a1, b1, n1 = oracle_step(w, x64, 1, n_threads=1)           # the 1-thread figure of SURVEY 8(d)
+                cpu = {"value": (a + b) * 1e3 * sc, "unit": "ms", "cores": min(threads, nq), "kind": "oracle",
+                       "sample": f"H + H^T on {nq} of {w.n_trans} transducers (seeded subset), {a + b:.1f} s of CPU wall time scaled by {sc:.0f}x",
+                       "ms_H": a * 1e3 * sc, "ms_HT": b * 1e3 * sc,
+                       "one_thread": {"value": (a1 + b1) * 1e3 * w.n_trans, "unit": "ms", "cores": 1,
+                                      "sample": f"H + H^T on 1 of {w.n_trans} transducers, {a1 + b1:.1f} s scaled by {w.n_trans}x"}}
             except Exception as ex:                          # the baseline must never sink the bench line
                 cpu = {"value": None, "unit": "ms", "cores": None, "kind": "oracle", "sample": f"failed: {ex}"}
-        metric = METRIC if (args.config == 3 and not args.subset) else f"ms per H and per H^T on {w.name} (value = ms per H + H^T pair)"
+        metric = METRIC if (args.config == 3 and not args.subset) else f"ms per H and per H^T on {w_all.name} (value = ms per H + H^T pair)"
+        par = "1 GPU" if world == 1 else (f"{world} GPUs, transducers sharded ({args.scaling}" +
+                                          (f": {world}x denser views" if args.scaling == "weak" else ": rows of H partitioned") +
+                                          "), H^T partial volumes all-reduced over NCCL")
         line = {"metric": metric, "value": ms_step, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+                "ms_per_step": ms_step, "higher_is_better": False, "scaling": args.scaling, "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
                 "config": {"workload": f"{w.name}: {w.nx}x{w.ny}x{w.nz} voxels @ {w.spacing} mm, {w.n_trans} transducers/GPU, nt={w.nt}, h={w.surf_step}, B={w.kband}",
-                           "step": "one H (x -> y) followed by one H^T (y -> x), inputs resident in HBM",
-                           "l2": "flushed between steps (256 MB fill)", "note": note,
-                           "parallelism": "1 GPU" if world == 1 else f"{world} GPUs, transducers sharded (weak: {world}x denser views), H^T partial volumes all-reduced over NCCL"},
+                           "step": "one H (phantom x -> y) followed by one H^T (dense seeded N(0,1) data -> x), inputs resident in HBM",
+                           "l2": "flushed between steps (256 MB fill)", "note": note, "parallelism": par},
                 "ms_H": ms_h, "ms_HT": ms_t,
                 "samples_per_operator": int(n_samples), "samples_per_s": 2.0 * float(tot_samples.item()) / (ms_step * 1e-3),
                 "samples_per_s_H": float(tot_samples.item()) / (ms_h * 1e-3), "samples_per_s_HT": float(tot_samples.item()) / (ms_t * 1e-3),
@@ -425,12 +481,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number (1-5); 3 is the metric's")
     ap.add_argument("--subset", type=int, default=0, help="debug only: use a seeded subset of transducers")
-    ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--cpu-sample", type=int, default=8, help="transducers in the oracle's timed sample")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank a rotated copy of the array (per-GPU work fixed), strong = rows of H partitioned")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--cpu-sample", type=int, default=64, help="transducers in the oracle's timed sample (SURVEY 8(d): 64)")
     ap.add_argument("--ref-sample", type=int, default=8, help="transducers per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--project-variant", type=int, default=-1, help="kernel variant (DESIGN.md §5); -1 = library default")
-    ap.add_argument("--backproject-variant", type=int, default=-1)
+    ap.add_argument("--no-next", action="store_true", help="skip the NEXT-row legs after the timed region")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
