@@ -159,6 +159,15 @@ int oat_fbp_weights(const oat_geometry *geom, const double *h_areas, float *h_w)
  * d_x: nz*ny*nx fp32; d_u: Q*nf complex as interleaved (re, im) fp32 pairs, index q*nf + l; device pointers owned by the
  * caller; the output is OVERWRITTEN; asynchronous on the stream. */
 int oat_sph_set(oat_geometry *geom, int32_t nf, double f0, double df, const float *h_he);
+
+/* Finite transducer aperture: the spatial impulse response of Eq. (18), (1/S_q) h~_q(r_n, f) = (1/S_q) int_{S_q}
+ * exp(-j 2 pi f |r^s - r_n|/c) / (2 pi |r^s - r_n|) dr^s, which the paper names as the reason for this model (L243; its
+ * elements are 2 x 2 mm^2, L291).  Reading G30: S_q is a flat square of side `side` (mm) centred on r_q, normal towards
+ * the grid centre, sides along the x^tr / y^tr axes of the transducer's frame (Appendix); the integral is the m x m
+ * midpoint rule, i.e. the mean of the point responses at the sub-element centres.  side = 0 or m = 1: point-like
+ * (the default).  Applies to oat_sph_project / oat_sph_backproject / oat_sph_pls_cg of this handle; cost grows with
+ * m^2.  Synchronises the device. */
+int oat_sph_set_aperture(oat_geometry *geom, double side, int32_t m);
 int oat_sph_project(oat_geometry *geom, const float *d_x, float *d_u, void *cuda_stream);
 int oat_sph_backproject(oat_geometry *geom, const float *d_u, float *d_x, void *cuda_stream);
 

@@ -19,7 +19,7 @@ EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
-    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_fbp_weights", "oat_sph_set", "oat_sph_project", "oat_sph_backproject", "oat_sph_pls_cg",
+    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_fbp_weights", "oat_sph_set", "oat_sph_set_aperture", "oat_sph_project", "oat_sph_backproject", "oat_sph_pls_cg",
     "oat_last_launch_count", "oat_uses_marching", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_measure_gather_rate_ex", "oat_measure_red_rate_ex", "oat_last_error", "oat_version",
 ]
 
@@ -100,7 +100,7 @@ def load():
     lib.oat_sph_set.argtypes = [vp, ctypes.c_int32, ctypes.c_double, ctypes.c_double, fp]
     lib.oat_sph_project.argtypes = [vp, fp, fp, vp]
     lib.oat_sph_backproject.argtypes = [vp, fp, fp, vp]
-    for n in ("oat_sph_set", "oat_sph_project", "oat_sph_backproject"):
+    for n in ("oat_sph_set", "oat_sph_set_aperture", "oat_sph_project", "oat_sph_backproject"):
         getattr(lib, n).restype = ctypes.c_int
     lib.oat_sph_pls_cg.argtypes = [vp, fp, fp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
     lib.oat_sph_pls_cg.restype = ctypes.c_int
@@ -370,6 +370,14 @@ def oat_fbp(g, p, weights, x=None, stream=None):
     _check(load().oat_fbp(g.handle, _dev_ptr(p, oat_num_samples(g), "p", g), _dev_ptr(weights, g.n_trans, "weights", g),
                           _dev_ptr(x, oat_num_voxels(g), "x", g), _stream(stream)))
     return x
+
+
+def oat_sph_set_aperture(g, side: float, m: int):
+    """Square transducer surface of side `side` (mm), integrated with m x m sub-elements (Eq. 18); 0 / 1 = point-like."""
+    lib = load()
+    lib.oat_sph_set_aperture.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int32]
+    lib.oat_sph_set_aperture.restype = ctypes.c_int
+    _check(lib.oat_sph_set_aperture(g.handle, ctypes.c_double(float(side)), ctypes.c_int32(int(m))))
 
 
 def oat_fbp_weights(g, areas) -> np.ndarray:

@@ -73,6 +73,8 @@ struct oat_geometry {
     float *d_sd = nullptr, *d_sq = nullptr;   // PLS-Sph data-space vectors (2*Q*nf floats, lazy; freed with the grid)
     int sph_nf = 0;
     double sph_f0 = 0, sph_df = 0;
+    double sph_aperture = 0;                  // side of the square transducer surface (mm), 0 = point-like (reading G30)
+    int sph_m = 1;                            // sub-elements per side of the aperture quadrature
     double *d_scal = nullptr;                 // a few fp64 scalars (dots)
     unsigned long long *d_counter = nullptr;
     double *h_scal = nullptr;                 // pinned mirror of d_scal
@@ -725,13 +727,13 @@ static int pls_cg_impl(oat_geometry *g, const float *d_u, float *d_x, int n_iter
     auto fwd = [&](const float *x, float *u) -> int {
         if (!sph) return project_full(g, x, u, st);
         CUDA_TRY(cudaMemsetAsync(u, 0, sizeof(float) * n_dat, st));
-        oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, x, g->d_p0, u, st);
+        oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m, x, g->d_p0, u, st);
         return OAT_OK;
     };
     auto bwd = [&](const float *u, float *x) -> int {
         if (!sph) return backproject_full(g, u, x, st);
-        oat_launch_sph_bwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, reinterpret_cast<const float2 *>(u),
-                           g->d_p0, g->d_sv, x, st);
+        oat_launch_sph_bwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m,
+                           reinterpret_cast<const float2 *>(u), g->d_p0, g->d_sv, x, st);
         return OAT_OK;
     };
     CUDA_TRY(cudaMemsetAsync(d_x, 0, sizeof(float) * g->n_vox, st));
@@ -828,6 +830,15 @@ int oat_sph_set(oat_geometry *g, int32_t nf, double f0, double df, const float *
     return OAT_OK;
 }
 
+int oat_sph_set_aperture(oat_geometry *g, double side, int32_t m)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!(side >= 0) || !isfinite(side) || m < 1 || m > 64) return fail(OAT_ERR_INVALID, "bad aperture (side >= 0, 1 <= m <= 64)");
+    CUDA_TRY(cudaDeviceSynchronize());
+    g->sph_aperture = side; g->sph_m = m;
+    return OAT_OK;
+}
+
 int oat_sph_project(oat_geometry *g, const float *d_x, float *d_u, void *stream)
 {
     int rc = check_handle(g); if (rc) return rc;
@@ -835,7 +846,7 @@ int oat_sph_project(oat_geometry *g, const float *d_x, float *d_u, void *stream)
     if (!d_x || (!d_u && g->dev.Q)) return fail(OAT_ERR_INVALID, "d_x / d_u must not be NULL");
     cudaStream_t st = (cudaStream_t)stream;
     if (g->dev.Q > 0) CUDA_TRY(cudaMemsetAsync(d_u, 0, sizeof(float2) * (size_t)g->sph_nf * (size_t)g->dev.Q, st));
-    oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, d_x, g->d_p0, d_u, st);
+    oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m, d_x, g->d_p0, d_u, st);
     CUDA_TRY(cudaGetLastError());
     return OAT_OK;
 }
@@ -845,8 +856,8 @@ int oat_sph_backproject(oat_geometry *g, const float *d_u, float *d_x, void *str
     int rc = check_handle(g); if (rc) return rc;
     if (!g->sph_nf) return fail(OAT_ERR_INVALID, "no frequency grid set (oat_sph_set)");
     if (!d_x || (!d_u && g->dev.Q)) return fail(OAT_ERR_INVALID, "d_x / d_u must not be NULL");
-    oat_launch_sph_bwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, reinterpret_cast<const float2 *>(d_u),
-                       g->d_p0, g->d_sv, d_x, (cudaStream_t)stream);
+    oat_launch_sph_bwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m,
+                       reinterpret_cast<const float2 *>(d_u), g->d_p0, g->d_sv, d_x, (cudaStream_t)stream);
     CUDA_TRY(cudaGetLastError());
     return OAT_OK;
 }

@@ -108,6 +108,7 @@ cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float
 void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha, float beta, cudaStream_t st);   // out = beta out + alpha L x
 // row NEXT-2: filtered backprojection, Eq. (27), x[n] = sum_q wq[q] {...} (voxel driven)
 void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, cudaStream_t st);
-// row NEXT-3: spherical-voxel model (Eq. 17-19, 24), point-like transducers; u, v: Q x nf complex (float2), p0: nf complex
-void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float *x, const float2 *p0, float *u, cudaStream_t st);
-void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st);
+// row NEXT-3: spherical-voxel model (Eq. 17-19, 24); point-like transducers or square apertures of side `aperture` (mm)
+// integrated with m x m sub-elements (Eq. 18, reading G30); u, v: Q x nf complex (float2), p0: nf complex
+void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float *x, const float2 *p0, float *u, cudaStream_t st);
+void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st);

@@ -127,7 +127,8 @@ oat_fbp_kernel(const OatDev P, const float *__restrict__ p, const float *__restr
 // other frequencies of the group by complex recurrence (OAT_SG - 1 fp32 rotations, error ~ OAT_SG eps).
 #define OAT_SG 16          // frequencies per thread (forward) / per re-seeded group (adjoint)
 #define OAT_SV 2048        // voxels per block chunk (forward)
-struct OatSph { int nf, n_lg; double f0, df, ds_over_c, ds; };   // ds_over_c: microseconds per node unit of distance
+struct OatSph { int nf, n_lg; double f0, df, ds_over_c, ds; int m; double a_nodes; };   // ds_over_c: microseconds per node unit of distance;
+                                                                                   // m x m sub-elements of a square aperture of side a_nodes (node units), reading G30
 
 __global__ void __launch_bounds__(128)
 oat_sph_fwd_kernel(const OatDev P, const OatSph S, const float *__restrict__ x, const float2 *__restrict__ p0, float *__restrict__ u)
@@ -145,6 +146,12 @@ oat_sph_fwd_kernel(const OatDev P, const OatSph S, const float *__restrict__ x, 
     const int l0 = lg * OAT_SG;
     const double *f = P.frame + (size_t)q * 12;
     const double tx = f[9] - 1.0, ty = f[10] - 1.0, tz = f[11] - 1.0;       // node coordinates (frames hold padded ones)
+    // finite aperture (Eq. 18, reading G30): the m x m sub-element midpoints t + u_i A e_x + u_j A e_y, u = (i + 1/2)/m - 1/2
+    const double Ax = S.a_nodes * f[0], Ay = S.a_nodes * f[1], Az = S.a_nodes * f[2];
+    const double Bx = S.a_nodes * f[3], By = S.a_nodes * f[4], Bz = S.a_nodes * f[5];
+    const int m = S.m;
+    const double rm = 1.0 / (double)m;
+    const float wsub = (float)(rm * rm);                                    // (1/S_q) x sub-element area
     const double fa = S.f0 + (double)l0 * S.df;
     float ar[OAT_SG], ai[OAT_SG];
 #pragma unroll
@@ -153,22 +160,29 @@ oat_sph_fwd_kernel(const OatDev P, const OatSph S, const float *__restrict__ x, 
     for (int i = 0; i < nv; ++i) {
         const float xv = s_x[i];                           // same address for the whole block: a broadcast
         if (xv != 0.f) {                                   // block-uniform branch
-            const double dx = (double)ix - tx, dy = (double)iy - ty, dz = (double)iz - tz;
-            const double d = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
-            if (d > 0.0) {
-                const double td = d * S.ds_over_c;         // |r_q - r_n| / c
-                const double pa = fa * td, pd = S.df * td; // cycles
-                float sr, cr, sz, cz;
-                sincospif((float)(-2.0 * (pa - rint(pa))), &sr, &cr);
-                sincospif((float)(-2.0 * (pd - rint(pd))), &sz, &cz);
-                const float amp = xv / (float)(6.283185307179586 * d * S.ds);
-                float er = amp * cr, ei = amp * sr;
+            for (int si = 0; si < m; ++si) {
+                const double ui = ((double)si + 0.5) * rm - 0.5;
+                for (int sj = 0; sj < m; ++sj) {
+                    const double uj = ((double)sj + 0.5) * rm - 0.5;
+                    const double dx = (double)ix - (tx + ui * Ax + uj * Bx), dy = (double)iy - (ty + ui * Ay + uj * By),
+                                 dz = (double)iz - (tz + ui * Az + uj * Bz);
+                    const double d = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
+                    if (d > 0.0) {
+                        const double td = d * S.ds_over_c;         // |r^s - r_n| / c
+                        const double pa = fa * td, pd = S.df * td; // cycles
+                        float sr, cr, sz, cz;
+                        sincospif((float)(-2.0 * (pa - rint(pa))), &sr, &cr);
+                        sincospif((float)(-2.0 * (pd - rint(pd))), &sz, &cz);
+                        const float amp = xv * wsub / (float)(6.283185307179586 * d * S.ds);
+                        float er = amp * cr, ei = amp * sr;
 #pragma unroll
-                for (int j = 0; j < OAT_SG; ++j) {
-                    ar[j] += er; ai[j] += ei;
-                    const float nr = fmaf(er, cz, -ei * sz);
-                    ei = fmaf(er, sz, ei * cz);
-                    er = nr;
+                        for (int j = 0; j < OAT_SG; ++j) {
+                            ar[j] += er; ai[j] += ei;
+                            const float nr = fmaf(er, cz, -ei * sz);
+                            ei = fmaf(er, sz, ei * cz);
+                            er = nr;
+                        }
+                    }
                 }
             }
         }
@@ -204,7 +218,7 @@ __global__ void __launch_bounds__(128)
 oat_sph_bwd_kernel(const OatDev P, const OatSph S, const float2 *__restrict__ v, float *__restrict__ x)
 {
     __shared__ float2 s_v[OAT_SQ][OAT_SL];
-    __shared__ double s_t[OAT_SQ][3];
+    __shared__ double s_t[OAT_SQ][9];                     // per staged transducer: position, A e_x, A e_y (node units)
     const long long n_vox = (long long)P.nx * P.ny * P.nz;
     const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool inside = n < n_vox;
@@ -216,44 +230,55 @@ oat_sph_bwd_kernel(const OatDev P, const OatSph S, const float2 *__restrict__ v,
             const int nl = min(OAT_SL, S.nf - lb);
             __syncthreads();
             for (int t = threadIdx.x; t < nq * nl; t += blockDim.x) s_v[t / nl][t % nl] = v[(size_t)(q0 + t / nl) * S.nf + lb + t % nl];
-            if (threadIdx.x < nq * 3) s_t[threadIdx.x / 3][threadIdx.x % 3] = P.frame[(size_t)(q0 + threadIdx.x / 3) * 12 + 9 + threadIdx.x % 3] - 1.0;
+            if (threadIdx.x < nq * 9) {
+                const int j = threadIdx.x / 9, c = threadIdx.x % 9;
+                const double *fr = P.frame + (size_t)(q0 + j) * 12;
+                s_t[j][c] = c < 3 ? fr[9 + c] - 1.0 : S.a_nodes * fr[c - 3];
+            }
             __syncthreads();
             if (!inside) continue;
+            const int m = S.m;
+            const double rm = 1.0 / (double)m;
             for (int j = 0; j < nq; ++j) {
-                const double dx = (double)ix - s_t[j][0], dy = (double)iy - s_t[j][1], dz = (double)iz - s_t[j][2];
-                const double d = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
-                if (!(d > 0.0)) continue;
-                const double td = d * S.ds_over_c, pd = S.df * td;
-                float sz, cz;
-                sincospif((float)(2.0 * (pd - rint(pd))), &sz, &cz);
-                const float amp = 1.f / (float)(6.283185307179586 * d * S.ds);
-                float acc = 0.f;
-                for (int g0 = 0; g0 < nl; g0 += OAT_SG) {
-                    const double pa = (S.f0 + (double)(lb + g0) * S.df) * td;
-                    float sr, cr;
-                    sincospif((float)(2.0 * (pa - rint(pa))), &sr, &cr);
-                    float er = amp * cr, ei = amp * sr;
-                    const int ng = min(OAT_SG, nl - g0);
-                    if (ng == OAT_SG) {                    // full group: unrolled
+                for (int sub = 0; sub < m * m; ++sub) {    // sub-elements of the aperture (reading G30); m = 1: the point-like model
+                    const double ui = ((double)(sub / m) + 0.5) * rm - 0.5, uj = ((double)(sub % m) + 0.5) * rm - 0.5;
+                    const double dx = (double)ix - (s_t[j][0] + ui * s_t[j][3] + uj * s_t[j][6]),
+                                 dy = (double)iy - (s_t[j][1] + ui * s_t[j][4] + uj * s_t[j][7]),
+                                 dz = (double)iz - (s_t[j][2] + ui * s_t[j][5] + uj * s_t[j][8]);
+                    const double d = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
+                    if (!(d > 0.0)) continue;
+                    const double td = d * S.ds_over_c, pd = S.df * td;
+                    float sz, cz;
+                    sincospif((float)(2.0 * (pd - rint(pd))), &sz, &cz);
+                    const float amp = (float)(rm * rm) / (float)(6.283185307179586 * d * S.ds);
+                    float acc = 0.f;
+                    for (int g0 = 0; g0 < nl; g0 += OAT_SG) {
+                        const double pa = (S.f0 + (double)(lb + g0) * S.df) * td;
+                        float sr, cr;
+                        sincospif((float)(2.0 * (pa - rint(pa))), &sr, &cr);
+                        float er = amp * cr, ei = amp * sr;
+                        const int ng = min(OAT_SG, nl - g0);
+                        if (ng == OAT_SG) {                    // full group: unrolled
 #pragma unroll
-                        for (int k = 0; k < OAT_SG; ++k) {
-                            const float2 vv = s_v[j][g0 + k];
-                            acc = fmaf(vv.x, er, fmaf(-vv.y, ei, acc));    // Re(v e)
-                            const float nr = fmaf(er, cz, -ei * sz);
-                            ei = fmaf(er, sz, ei * cz);
-                            er = nr;
-                        }
-                    } else {
-                        for (int k = 0; k < ng; ++k) {
-                            const float2 vv = s_v[j][g0 + k];
-                            acc = fmaf(vv.x, er, fmaf(-vv.y, ei, acc));
-                            const float nr = fmaf(er, cz, -ei * sz);
-                            ei = fmaf(er, sz, ei * cz);
-                            er = nr;
+                            for (int k = 0; k < OAT_SG; ++k) {
+                                const float2 vv = s_v[j][g0 + k];
+                                acc = fmaf(vv.x, er, fmaf(-vv.y, ei, acc));    // Re(v e)
+                                const float nr = fmaf(er, cz, -ei * sz);
+                                ei = fmaf(er, sz, ei * cz);
+                                er = nr;
+                            }
+                        } else {
+                            for (int k = 0; k < ng; ++k) {
+                                const float2 vv = s_v[j][g0 + k];
+                                acc = fmaf(vv.x, er, fmaf(-vv.y, ei, acc));
+                                const float nr = fmaf(er, cz, -ei * sz);
+                                ei = fmaf(er, sz, ei * cz);
+                                er = nr;
+                            }
                         }
                     }
+                    total += (double)acc;
                 }
-                total += (double)acc;
             }
         }
     }
@@ -283,18 +308,20 @@ void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, 
     oat_fbp_kernel<<<grid, 256, 0, st>>>(P, p, wq, x);
 }
 
-void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float *x, const float2 *p0, float *u, cudaStream_t st)
+void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float *x, const float2 *p0, float *u, cudaStream_t st)
 {
     OatSph S; S.nf = nf; S.n_lg = (nf + OAT_SG - 1) / OAT_SG; S.f0 = f0; S.df = df; S.ds = ds; S.ds_over_c = ds / c;
+    S.m = (aperture > 0.0 && m > 1) ? m : 1; S.a_nodes = S.m > 1 ? aperture / ds : 0.0;
     const long long n_vox = (long long)P.nx * P.ny * P.nz, work = (long long)P.Q * S.n_lg;
     if (n_vox <= 0 || work <= 0) return;
     const dim3 grid((unsigned)((work + 127) / 128), (unsigned)((n_vox + OAT_SV - 1) / OAT_SV));
     oat_sph_fwd_kernel<<<grid, 128, 0, st>>>(P, S, x, p0, u);
 }
 
-void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st)
+void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st)
 {
     OatSph S; S.nf = nf; S.n_lg = (nf + OAT_SG - 1) / OAT_SG; S.f0 = f0; S.df = df; S.ds = ds; S.ds_over_c = ds / c;
+    S.m = (aperture > 0.0 && m > 1) ? m : 1; S.a_nodes = S.m > 1 ? aperture / ds : 0.0;
     const long long n_vox = (long long)P.nx * P.ny * P.nz, n = (long long)P.Q * nf;
     if (n > 0) oat_sph_prep_kernel<<<grid_for(n, 256), 256, 0, st>>>(S, P.Q, u, p0, v);
     if (n_vox > 0) oat_sph_bwd_kernel<<<(unsigned)((n_vox + 127) / 128), 128, 0, st>>>(P, S, v, x);

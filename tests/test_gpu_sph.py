@@ -28,7 +28,7 @@ def rel_l2(a, b):
     return float(np.linalg.norm(a - b) / nb) if nb > 0 else float(np.linalg.norm(a))
 
 
-def run_pair(env, w, nf, f0, df, he=None, seed=0, sparse=False):
+def run_pair(env, w, nf, f0, df, he=None, seed=0, sparse=False, aperture=0.0, m=1):
     torch, osph, oat, wl = env
     rng = np.random.default_rng(seed)
     x = rng.standard_normal((w.nz, w.ny, w.nx)).astype(np.float32)
@@ -37,12 +37,14 @@ def run_pair(env, w, nf, f0, df, he=None, seed=0, sparse=False):
     u = (rng.standard_normal((w.n_trans, nf)) + 1j * rng.standard_normal((w.n_trans, nf))).astype(np.complex64)
     g = oat.oat_geometry_create(w)
     oat.oat_sph_set(g, nf, f0, df, he)
+    if aperture:
+        oat.oat_sph_set_aperture(g, aperture, m)
     hx = oat.oat_sph_project(g, torch.from_numpy(x).cuda()).cpu().numpy()
     htu = oat.oat_sph_backproject(g, torch.from_numpy(u).cuda()).cpu().numpy()
     g.close()
     he128 = None if he is None else np.asarray(he, dtype=np.complex64).astype(np.complex128)
-    rx = osph.project(w, x.astype(np.float64), f0, df, nf, he128)
-    ru = osph.backproject(w, u.astype(np.complex128), f0, df, nf, he128)
+    rx = osph.project(w, x.astype(np.float64), f0, df, nf, he128, aperture, m)
+    ru = osph.backproject(w, u.astype(np.complex128), f0, df, nf, he128, aperture, m)
     e1, e2 = rel_l2(hx, rx), rel_l2(htu, ru)
     lhs = float(np.real(np.vdot(u.astype(np.complex128), hx.astype(np.complex128))))
     rhs = float(np.vdot(x.astype(np.float64), htu.astype(np.float64)))
@@ -115,3 +117,52 @@ def test_pls_sph_cg_first_iterations_match_the_oracle(env, mu_rel):
     assert np.allclose(grad, grado, rtol=3e-3)
     assert rel_l2(x.cpu().numpy(), xo) <= 1e-3
     assert np.all(np.diff(obj) < 0)
+
+
+# ---------------------------------------------------------------- finite aperture (Eq. 18, reading G30)
+@pytest.mark.parametrize("n,q,nf,aperture,m", [(9, 5, 40, 2.0, 2), (12, 3, 23, 2.0, 3), (7, 6, 16, 0.7, 4)])
+def test_finite_aperture(env, n, q, nf, aperture, m):
+    torch, osph, oat, wl = env
+    w = wl.small(n=n, q=q, nt=8, kband=8)
+    e1, e2, adj = run_pair(env, w, nf, 0.05, 0.07, seed=n * m, aperture=aperture, m=m)
+    assert e1 <= TOL and e2 <= TOL and adj <= 1e-4, (e1, e2, adj)
+    # the aperture changes the operator (the test would also pass for a kernel that ignored it otherwise)
+    rng = np.random.default_rng(n * m)
+    x = rng.standard_normal((w.nz, w.ny, w.nx)).astype(np.float32)
+    g = oat.oat_geometry_create(w)
+    oat.oat_sph_set(g, nf, 0.05, 0.07)
+    a = oat.oat_sph_project(g, torch.from_numpy(x).cuda()).cpu().numpy()
+    oat.oat_sph_set_aperture(g, aperture, m)
+    b = oat.oat_sph_project(g, torch.from_numpy(x).cuda()).cpu().numpy()
+    oat.oat_sph_set_aperture(g, 0.0, 1)
+    c = oat.oat_sph_project(g, torch.from_numpy(x).cuda()).cpu().numpy()
+    g.close()
+    assert rel_l2(b, a) > 1e-3 and np.array_equal(a, c)
+
+
+@pytest.mark.parametrize("aperture,m", [(0.0, 1), (2.0, 2)])
+def test_bench_shape_sampled_rows_and_voxels(env, aperture, m):
+    """The shape bench.py times (config 3's 240^3 grid, 256 seeded transducers, 64 frequencies), in full on the GPU;
+    the oracle evaluates 2 sampled rows of H_sph x (dense N(0,1) volume) and 24 sampled voxels of H_sph† u."""
+    torch, osph, oat, wl = env
+    w = wl.config(3)
+    _, ws = w.seeded_subset(256)
+    nf, f0, df = 64, 0.0, 0.078125
+    rng = np.random.default_rng(77)
+    x = rng.standard_normal((ws.nz, ws.ny, ws.nx)).astype(np.float32)
+    u = (rng.standard_normal((ws.n_trans, nf)) + 1j * rng.standard_normal((ws.n_trans, nf))).astype(np.complex64)
+    g = oat.oat_geometry_create(ws)
+    oat.oat_sph_set(g, nf, f0, df)
+    oat.oat_sph_set_aperture(g, aperture, m)
+    hx = oat.oat_sph_project(g, torch.from_numpy(x).cuda()).cpu().numpy()
+    htu = oat.oat_sph_backproject(g, torch.from_numpy(u).cuda()).cpu().numpy()
+    g.close()
+    rows = [5, 200] if m == 1 else [131]
+    ref_rows = osph.project_rows(ws, x.astype(np.float64), rows, f0, df, nf, None, aperture, m)
+    idx = rng.integers(0, [ws.nz, ws.ny, ws.nx], size=(24, 3))
+    pts = np.asarray(ws.origin)[None, :] + ws.spacing * idx[:, ::-1].astype(np.float64)
+    ref_vox = osph.backproject_points(ws, u.astype(np.complex128), pts, f0, df, nf, None, aperture, m)
+    e1 = rel_l2(hx[rows], ref_rows)
+    e2 = rel_l2(htu[idx[:, 0], idx[:, 1], idx[:, 2]], ref_vox)
+    print(f"H_sph at 240^3 x 256 x 64 (aperture {aperture} mm, m = {m}): rows {e1:.2e}, voxels {e2:.2e}")
+    assert e1 <= 2 * TOL and e2 <= TOL, (e1, e2)

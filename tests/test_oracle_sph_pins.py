@@ -123,3 +123,99 @@ def test_pls_sph_cg_matches_the_dense_real_system():
     x80, _, g80 = sph.pls_cg(w, uc, 80, mu, f0, df, nf)
     xd = np.linalg.solve(A, b)
     assert np.linalg.norm(x80.ravel() - xd) <= 1e-6 * np.linalg.norm(xd)
+
+
+# ---------------------------------------------------------------- finite aperture (Eq. 18, reading G30)
+def test_aperture_with_one_sub_element_is_the_point_like_model():
+    w = problem(n=4, q=3)
+    rng = np.random.default_rng(11)
+    x = rng.standard_normal((w.nz, w.ny, w.nx))
+    u = rng.standard_normal((w.n_trans, 12)) + 1j * rng.standard_normal((w.n_trans, 12))
+    a = sph.project(w, x, 0.1, 0.3, 12)
+    assert np.array_equal(a, sph.project(w, x, 0.1, 0.3, 12, aperture=2.0, m=1))
+    assert np.array_equal(a, sph.project(w, x, 0.1, 0.3, 12, aperture=0.0, m=4))
+    b = sph.backproject(w, u, 0.1, 0.3, 12)
+    assert np.array_equal(b, sph.backproject(w, u, 0.1, 0.3, 12, aperture=2.0, m=1))
+
+
+def test_sub_elements_tile_a_square_facing_the_grid_centre():
+    """Reading G30: the m x m midpoints lie in the plane through r_q normal to (centre - r_q), inside a square of side a
+    whose sides follow e_x, e_y of reading S1; their mean is r_q and their second moments are those of the midpoint rule."""
+    w = problem(n=3, q=3)
+    a, m = 2.0, 4
+    for q in range(w.n_trans):
+        pts = sph.element_points(w, q, a, m)
+        assert pts.shape == (m * m, 3)
+        rq = w.trans_xyz[q]
+        n = (w.centre - rq) / np.linalg.norm(w.centre - rq)
+        assert np.allclose((pts - rq) @ n, 0.0, atol=1e-12)                 # in the plane facing the centre
+        assert np.allclose(pts.mean(axis=0), rq, atol=1e-12)
+        ex, ey, ez = sph.element_frame(w, q)
+        assert np.allclose(ez, n) and abs(ex @ ey) < 1e-12 and abs(ex @ ez) < 1e-12 and np.isclose(np.linalg.norm(ex), 1.0)
+        assert abs(ey[2]) < 1e-12                                             # y^tr is horizontal (e_z x z^)
+        lx, ly = (pts - rq) @ ex, (pts - rq) @ ey
+        assert np.all(np.abs(lx) < a / 2) and np.all(np.abs(ly) < a / 2)
+        assert np.isclose(np.mean(lx ** 2), a * a / 12.0 * (1.0 - 1.0 / m ** 2))   # midpoint rule on [-a/2, a/2]
+        assert np.isclose(np.mean(ly ** 2), a * a / 12.0 * (1.0 - 1.0 / m ** 2))
+
+
+def test_far_field_of_the_aperture_is_the_sinc_pattern():
+    """Fraunhofer limit of Eq. (18): for a source far from a flat a x a element, (1/S_q) h~_q = G(d) sinc(k a s_x / 2)
+    sinc(k a s_y / 2), k = 2 pi f / c, (s_x, s_y) = components of the unit vector element -> source along the element's
+    sides.  The element (2 mm, m = 24 sub-elements per side) faces the centre of a coarse 3^3 grid 400 mm away, so the
+    grid's off-centre nodes sample the pattern well off its axis (|k a s / 2| up to ~5); the residual is the Fresnel term
+    ~ k a^2 / (8 d) <= 1.6e-2 rad, hence the 1.2e-2 gate.  The voxel size enters only through the common factor p~0."""
+    ds, a, m = 150.0, 2.0, 24
+    tr = np.array([[400.0, 30.0, -20.0]])
+    o = -1.0 * ds
+    w = wl.Workload("sph-ff", 3, 3, 3, ds, (o, o, o), tr, c=1.5, t0=0.0, dt=0.05, nt=8, surf_step=ds, kband=8, gain=1.0)
+    f0, df, nf = 0.5, 0.5, 6                                       # 0.5 .. 3 MHz: lambda 3 .. 0.5 mm
+    f = sph.freqs(f0, df, nf)
+    ex, ey, ez = sph.element_frame(w, 0)
+    p0 = sph.p0_tilde(w, f)
+    k = 2.0 * np.pi * f / w.c
+    strongest = 1.0
+    for (iz, iy, ix) in [(1, 1, 1), (1, 2, 1), (0, 1, 1), (2, 2, 0), (0, 0, 2)]:
+        x = np.zeros((3, 3, 3)); x[iz, iy, ix] = 1.0
+        node = np.asarray(w.origin) + ds * np.array([ix, iy, iz])
+        u = sph.project(w, x, f0, df, nf, aperture=a, m=m)[0]
+        v = node - tr[0]
+        d = np.linalg.norm(v)
+        sx, sy = (v / d) @ ex, (v / d) @ ey
+        pat = np.sinc(k * a * sx / 2.0 / np.pi) * np.sinc(k * a * sy / 2.0 / np.pi)      # np.sinc(t) = sin(pi t)/(pi t)
+        exp = p0 * np.exp(-1j * k * d) / (2.0 * np.pi * d) * pat
+        scale = np.abs(p0 / (2.0 * np.pi * d))
+        assert np.all(np.abs(u - exp) <= 1.2e-2 * scale), ((iz, iy, ix), np.abs(u - exp) / scale)
+        strongest = min(strongest, np.abs(pat).min())
+        if (iz, iy, ix) != (1, 1, 1):                              # off axis the point-like response is clearly different
+            up = sph.project(w, x, f0, df, nf)[0]
+            assert np.abs(up - u).max() > 0.2 * np.abs(up).max()
+    assert strongest < 0.1                                         # the pattern was sampled down to its side lobes
+
+
+def test_adjoint_identity_with_aperture():
+    w = problem(n=4, q=3)
+    rng = np.random.default_rng(12)
+    x = rng.standard_normal((w.nz, w.ny, w.nx))
+    u = rng.standard_normal((w.n_trans, 9)) + 1j * rng.standard_normal((w.n_trans, 9))
+    he = rng.standard_normal(9) + 1j * rng.standard_normal(9)
+    hx = sph.project(w, x, 0.2, 0.4, 9, he, aperture=1.5, m=3)
+    htu = sph.backproject(w, u, 0.2, 0.4, 9, he, aperture=1.5, m=3)
+    lhs, rhs = np.real(np.vdot(hx, u)), float(np.vdot(x, htu))
+    assert abs(lhs - rhs) <= 1e-12 * max(abs(lhs), abs(rhs))
+
+
+def test_row_and_point_evaluations_equal_the_full_operators():
+    """project_rows / backproject_points (used for sampled parity at the bench's sizes) are the same sums as project /
+    backproject."""
+    w = problem(n=5, q=4)
+    rng = np.random.default_rng(13)
+    x = rng.standard_normal((w.nz, w.ny, w.nx))
+    u = rng.standard_normal((w.n_trans, 7)) + 1j * rng.standard_normal((w.n_trans, 7))
+    full = sph.project(w, x, 0.1, 0.2, 7, aperture=1.0, m=2)
+    rows = sph.project_rows(w, x, [3, 1], 0.1, 0.2, 7, aperture=1.0, m=2, chunk=17)
+    assert np.allclose(rows, full[[3, 1]], rtol=1e-12, atol=1e-15)
+    xb = sph.backproject(w, u, 0.1, 0.2, 7, aperture=1.0, m=2)
+    from oracle.oat_fbp import node_positions
+    pts = node_positions(w)[[0, 4, 2], [1, 3, 2], [4, 0, 2]]
+    assert np.allclose(sph.backproject_points(w, u, pts, 0.1, 0.2, 7, aperture=1.0, m=2), xb[[0, 4, 2], [1, 3, 2], [4, 0, 2]], rtol=1e-12, atol=1e-15)
