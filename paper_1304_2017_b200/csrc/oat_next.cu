@@ -19,32 +19,64 @@ inline int grid_for(long long n, int block)
 
 // Row NEXT-1, EIR operator.  ADJ = 0: Eq. (14), out[q,k] = sum_m he[m] in[q, k-1-m]; ADJ = 1: Eq. (21),
 // out[q,k] = sum_m he[m] in[q, k+1+m]; he[m] given for m = 0..L-1, `in` zero outside [0, K) (reading G20).
-// One block = one transducer row x a tile of OAT_ET outputs; the taps and the input window of the tile sit in
-// shared memory; every output is one fixed-order fp32 FMA chain over the taps (deterministic).
-#define OAT_ET 256
+// Both are one correlation out[k0+o] = sum_m' h'[m'] win[o + m'] over a window of the row held in shared memory:
+//   ADJ = 1: h' = he,           window sample j <-> input k0 + 1 + j
+//   ADJ = 0: h'[m'] = he[Lp-1-m'] (taps reversed, Lp = L rounded up to 8 with zero taps), window sample j <-> k0 - Lp + j
+// One block = one transducer row x a tile of 2048 outputs; a thread owns 8 CONSECUTIVE outputs and slides a 16-sample
+// register window over the taps: per group of 8 taps 64 FMAs against 4 LDS.128 (the one-output-per-thread form needed
+// 2 shared-memory loads per FMA and ran at 5 % of the HBM rate).  Every output is one fixed-order fp32 FMA chain
+// (deterministic); algorithmic bytes = read + write of the data vector once, algorithmic work = L FMAs per output.
+#define OAT_ET 256          // threads per block
+#define OAT_ER 8            // outputs per thread
 template <int ADJ>
 __global__ void __launch_bounds__(OAT_ET)
-oat_eir_kernel(const float *__restrict__ in, float *__restrict__ out, const float *__restrict__ he, int L, int K)
+oat_eir_kernel(const float *__restrict__ in, float *__restrict__ out, const float *__restrict__ he, int L, int Lp, int K)
 {
-    extern __shared__ float sm[];
-    float *s_he = sm, *s_in = sm + L;                      // window: OAT_ET + L samples
-    const int q = blockIdx.y, k0 = blockIdx.x * OAT_ET, t = threadIdx.x;
+    extern __shared__ __align__(16) float sm[];
+    float *s_h = sm, *s_w = sm + Lp;                       // taps h'[0, Lp), window [0, T + Lp + 8)
+    constexpr int T = OAT_ET * OAT_ER;
+    const int q = blockIdx.y, k0 = blockIdx.x * T, t = threadIdx.x;
     const float *row = in + (size_t)q * K;
-    for (int m = t; m < L; m += OAT_ET) s_he[m] = he[m];
-    // ADJ = 0: window sample j <-> k0 - L + j  (inputs k-1-m, m < L, of outputs k0..k0+ET-1: k0-L .. k0+ET-2)
-    // ADJ = 1: window sample j <-> k0 + 1 + j  (inputs k+1+m: k0+1 .. k0+ET+L-1)
-    const int base = ADJ ? k0 + 1 : k0 - L;
-    for (int j = t; j < OAT_ET + L; j += OAT_ET) {
+    for (int m = t; m < Lp; m += OAT_ET) {
+        const int src = ADJ ? m : Lp - 1 - m;
+        s_h[m] = src < L ? he[src] : 0.f;
+    }
+    const int base = ADJ ? k0 + 1 : k0 - Lp;
+    for (int j = t; j < T + Lp + 8; j += OAT_ET) {
         const int kk = base + j;
-        s_in[j] = (kk >= 0 && kk < K) ? row[kk] : 0.f;
+        s_w[j] = (kk >= 0 && kk < K) ? row[kk] : 0.f;
     }
     __syncthreads();
-    const int k = k0 + t;
-    if (k >= K) return;
-    float acc = 0.f;
-    if (ADJ) { for (int m = 0; m < L; ++m) acc = fmaf(s_he[m], s_in[t + m], acc); }
-    else     { for (int m = 0; m < L; ++m) acc = fmaf(s_he[m], s_in[t + L - 1 - m], acc); }
-    out[(size_t)q * K + k] = acc;
+    float acc[OAT_ER], x[2 * OAT_ER];
+#pragma unroll
+    for (int r = 0; r < OAT_ER; ++r) acc[r] = 0.f;
+    const float4 *w4 = reinterpret_cast<const float4 *>(s_w + t * OAT_ER);
+    const float4 *h4 = reinterpret_cast<const float4 *>(s_h);
+    {
+        const float4 a = w4[0], b = w4[1];
+        x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = b.x; x[5] = b.y; x[6] = b.z; x[7] = b.w;
+    }
+    for (int m0 = 0; m0 < Lp; m0 += 8) {
+        const float4 a = w4[m0 / 4 + 2], b = w4[m0 / 4 + 3];
+        x[8] = a.x; x[9] = a.y; x[10] = a.z; x[11] = a.w; x[12] = b.x; x[13] = b.y; x[14] = b.z; x[15] = b.w;
+        const float4 ha = h4[m0 / 4], hb = h4[m0 / 4 + 1];           // same address for the whole block: a broadcast
+        const float h[8] = {ha.x, ha.y, ha.z, ha.w, hb.x, hb.y, hb.z, hb.w};
+#pragma unroll
+        for (int mm = 0; mm < 8; ++mm)
+#pragma unroll
+            for (int r = 0; r < OAT_ER; ++r) acc[r] = fmaf(h[mm], x[r + mm], acc[r]);
+#pragma unroll
+        for (int r = 0; r < OAT_ER; ++r) x[r] = x[r + 8];
+    }
+    const int k = k0 + t * OAT_ER;
+    float *o = out + (size_t)q * K + k;
+    if (k + OAT_ER <= K && (((size_t)q * K + k) & 3) == 0) {
+        reinterpret_cast<float4 *>(o)[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        reinterpret_cast<float4 *>(o)[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+    } else {
+#pragma unroll
+        for (int r = 0; r < OAT_ER; ++r) if (k + r < K) o[r] = acc[r];
+    }
 }
 
 // Row NEXT-1, smoothness penalty (Eq. 34, reading G21): out = beta out + alpha L x with R(x) = x^T L x,
@@ -291,14 +323,15 @@ oat_sph_bwd_kernel(const OatDev P, const OatSph S, const float2 *__restrict__ v,
 cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float *he, int L, int Q, int K, cudaStream_t st)
 {
     if (Q <= 0 || K <= 0) return cudaSuccess;
-    const size_t smem = sizeof(float) * (size_t)(OAT_ET + 2 * L);
+    const int Lp = ((L + 7) / 8) * 8, T = OAT_ET * OAT_ER;
+    const size_t smem = sizeof(float) * (size_t)(2 * Lp + T + 8);
     if (smem > 200 * 1024) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(oat_eir_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(oat_eir_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const dim3 grid((unsigned)((K + OAT_ET - 1) / OAT_ET), (unsigned)Q);
-    if (adjoint) oat_eir_kernel<1><<<grid, OAT_ET, smem, st>>>(in, out, he, L, K);
-    else oat_eir_kernel<0><<<grid, OAT_ET, smem, st>>>(in, out, he, L, K);
+    const dim3 grid((unsigned)((K + T - 1) / T), (unsigned)Q);
+    if (adjoint) oat_eir_kernel<1><<<grid, OAT_ET, smem, st>>>(in, out, he, L, Lp, K);
+    else oat_eir_kernel<0><<<grid, OAT_ET, smem, st>>>(in, out, he, L, Lp, K);
     return cudaGetLastError();
 }
 
