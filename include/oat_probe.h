@@ -14,11 +14,17 @@ extern "C" {
 #endif
 
 /* Kernel selection for tests and measurements.  key = "project" / "backproject": variant 4 = marching kernels (default,
- * used when the geometry allows: B = 32, records indexable with 32 bits, c dt <= spacing), 0 = the generic patch kernel
- * that otherwise serves as the fall-back.  key = "morton_shift": log2 of the cell size of the patch order (default 6).
+ * used when the geometry allows: B = 32, records indexable with 32 bits, c dt <= spacing), 5 = tile-stationary kernels
+ * (oat_tile.cu), 0 = the generic patch kernel that otherwise serves as the fall-back.  key = "tile_nq": transducers per
+ * work item of the tile kernels.  key = "morton_shift": log2 of the cell size of the patch order (default 6).
  * key = "record_limit_log2": pretend record indices have that many bits (tests of the automatic fall-back).
  * Unknown key or value => OAT_ERR_INVALID. */
 int oat_set_variant(oat_geometry *geom, const char *key, int variant);
+
+/* Enumeration counters of the tile-stationary kernels, accumulated over the calls since the last reset while
+ * oat_set_variant(geom, "tile_stats", 1) is in force: h_out[0] candidate rays, [1] candidates after the fp32 cull,
+ * [2] rays that own at least one chunk, [3] chunks (8 samples each) marched; h_out has room for 8 values. */
+int oat_tile_stats(oat_geometry *geom, unsigned long long *h_out, int reset);
 
 /* 1 if the next oat_project (backproject = 0) / oat_backproject (backproject = 1) on this handle runs the marching
  * kernel, 0 if it runs the generic patch kernel, negative on NULL. */

@@ -20,7 +20,7 @@ EXPORTS = [
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
     "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_fbp_weights", "oat_sph_set", "oat_sph_set_aperture", "oat_sph_project", "oat_sph_backproject", "oat_sph_pls_cg",
-    "oat_last_launch_count", "oat_uses_marching", "oat_last_kernel_ms", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_measure_gather_rate_ex", "oat_measure_red_rate_ex", "oat_last_error", "oat_version",
+    "oat_last_launch_count", "oat_uses_marching", "oat_last_kernel_ms", "oat_tile_stats", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_measure_gather_rate_ex", "oat_measure_red_rate_ex", "oat_last_error", "oat_version",
 ]
 
 
@@ -78,6 +78,8 @@ def load():
     lib.oat_last_launch_count.restype = ctypes.c_int
     lib.oat_uses_marching.argtypes = [vp, ctypes.c_int]
     lib.oat_uses_marching.restype = ctypes.c_int
+    lib.oat_tile_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong), ctypes.c_int]
+    lib.oat_tile_stats.restype = ctypes.c_int
     lib.oat_last_kernel_ms.argtypes = [vp]
     lib.oat_last_kernel_ms.restype = ctypes.c_float
     lib.oat_last_error.restype = ctypes.c_char_p
@@ -286,6 +288,13 @@ def oat_last_launch_count(g) -> int:
 
 def oat_last_kernel_ms(g) -> float:
     return float(load().oat_last_kernel_ms(g.handle))
+
+
+def oat_tile_stats(g, reset: bool = True):
+    """Enumeration counters of the tile-stationary kernels (candidates, after the fp32 cull, owning rays, chunks)."""
+    out = (ctypes.c_ulonglong * 8)()
+    _check(load().oat_tile_stats(g.handle, out, 1 if reset else 0))
+    return [int(v) for v in out[:8]]
 
 
 def oat_measure_red_rate(device: int = 0) -> float:

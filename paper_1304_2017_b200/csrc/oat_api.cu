@@ -80,6 +80,9 @@ struct oat_geometry {
     double *h_scal = nullptr;                 // pinned mirror of d_scal
     long long n_surface_samples = -1;
     int variant_project = 4, variant_backproject = 4;   // 4 = marching kernels, 0 = generic patch kernel (oat_probe.h)
+    int tile_tma = 1;                         // 0: the tile kernels stage the brick with plain loads instead of TMA (measurement aid)
+    int tile_nq = 1024;                       // transducers per (tile, transducer range) item of the tile-stationary kernels
+    unsigned long long *d_tile_stats = nullptr;   // enumeration counters of the tile kernels (oat_probe.h), NULL = off
     bool march_ok = false;                    // ray anchors fit the 10-bit packed offsets of the marching H^T queue, step <= 1
     size_t record_limit = (size_t)1 << 31;    // the marching kernels index records with 32 bits (lowered only by tests)
     int last_launches = 0;
@@ -98,7 +101,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
     cudaFree(g->d_y4); cudaFree(g->d_he); cudaFree(g->d_p0); cudaFree(g->d_sv); cudaFree(g->d_sd); cudaFree(g->d_sq);
-    cudaFree(g->d_counter); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done);
+    cudaFree(g->d_counter); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done); cudaFree(g->d_tile_stats);
     if (g->h_scal) cudaFreeHost(g->h_scal);
     if (g->ev0) cudaEventDestroy(g->ev0);
     if (g->ev1) cudaEventDestroy(g->ev1);
@@ -256,13 +259,14 @@ int build_geometry(oat_geometry *G)
         }
     }
     // direction table of the marching kernels: per band the leading rings any transducer can use
-    long long n_dir = 0;
+    long long n_dir = 0, max_band_dirs = 0;
     for (int b = 0; b < NB; ++b) {
         int mr = 0;
         for (int q = 0; q < Q; ++q) if (qb_rings[(size_t)q * NB + b] > mr) mr = qb_rings[(size_t)q * NB + b];
         bands[b].dir_rings = mr;
         bands[b].dir_ofs = n_dir;
         n_dir += rings[bands[b].ring_ofs + mr].cum;
+        if (rings[bands[b].ring_ofs + mr].cum > max_band_dirs) max_band_dirs = rings[bands[b].ring_ofs + mr].cum;
     }
 
     // ---- upload
@@ -286,6 +290,7 @@ int build_geometry(oat_geometry *G)
     P.rb_sectors = G->d_rb_sectors; P.patches = nullptr; P.n_patches = 0;
     P.q_count = nullptr; P.q_done = nullptr;
     P.dir = nullptr;
+    P.max_band_dirs = max_band_dirs;
     if (B == 32 && n_dir > 0 && n_dir < (1LL << 31)) {     // 16 B per direction; otherwise the generic kernel is used
         CUDA_TRY(cudaMalloc((void **)&G->d_dir, sizeof(double2) * (size_t)n_dir));
         P.dir = G->d_dir;
@@ -382,7 +387,16 @@ int project_impl(oat_geometry *G, const float *d_x, float *d_y, cudaStream_t st)
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    const bool march = G->variant_project == 4 && march_h_ok(G);   // else: B < 32 or a grid the marching kernel cannot index
+    if (G->variant_project == 5 && oat_tile_supported(P)) {           // tile-stationary kernel: no patch list, no record array
+        CUDA_TRY(cudaMemsetAsync(G->d_g, 0, sizeof(double) * (G->n_dat ? G->n_dat : 1), st));
+        CUDA_TRY(cudaEventRecord(G->ev0, st));
+        CUDA_TRY(oat_launch_tile_fwd(P, d_x, G->d_g, d_y, G->d_counter, G->d_tile_stats, G->tile_nq, G->tile_tma, st));
+        CUDA_TRY(cudaEventRecord(G->ev1, st));
+        G->ev_valid = true;
+        G->last_launches = 2;
+        return OAT_OK;
+    }
+    const bool march = G->variant_project >= 4 && march_h_ok(G);   // else: B < 32 or a grid the marching kernel cannot index
     int rc = ensure_patches(G); if (rc) return rc;
     if (march) {
         if (!G->d_cells) CUDA_TRY(cudaMalloc((void **)&G->d_cells, sizeof(float4) * 2 * G->n_cells));
@@ -884,7 +898,16 @@ int oat_fbp_weights(const oat_geometry *g, const double *h_areas, float *h_w)
 int oat_set_variant(oat_geometry *g, const char *key, int variant)
 {
     if (!g || !key) return fail(OAT_ERR_INVALID, "NULL argument");
-    if (!strcmp(key, "project")) { if (variant != 0 && variant != 4) return fail(OAT_ERR_INVALID, "unknown project variant %d (0 generic, 4 marching)", variant); g->variant_project = variant; return OAT_OK; }
+    if (!strcmp(key, "project")) { if (variant != 0 && variant != 4 && variant != 5) return fail(OAT_ERR_INVALID, "unknown project variant %d (0 generic, 4 marching, 5 tile-stationary)", variant); g->variant_project = variant; return OAT_OK; }
+    if (!strcmp(key, "tile_nq")) { if (variant < 1) return fail(OAT_ERR_INVALID, "tile_nq must be >= 1"); g->tile_nq = variant; return OAT_OK; }
+    if (!strcmp(key, "tile_tma")) { g->tile_tma = variant ? 1 : 0; return OAT_OK; }
+    if (!strcmp(key, "tile_stats")) {
+        if (variant && !g->d_tile_stats) {
+            CUDA_TRY(cudaMalloc((void **)&g->d_tile_stats, sizeof(unsigned long long) * 8));
+            CUDA_TRY(cudaMemset(g->d_tile_stats, 0, sizeof(unsigned long long) * 8));
+        } else if (!variant && g->d_tile_stats) { CUDA_TRY(cudaDeviceSynchronize()); cudaFree(g->d_tile_stats); g->d_tile_stats = nullptr; }
+        return OAT_OK;
+    }
     if (!strcmp(key, "backproject")) { if (variant != 0 && variant != 4) return fail(OAT_ERR_INVALID, "unknown backproject variant %d (0 generic, 4 marching)", variant); g->variant_backproject = variant; return OAT_OK; }
     if (!strcmp(key, "morton_shift")) {
         if (variant < 0 || variant > 10) return fail(OAT_ERR_INVALID, "morton_shift out of range");
@@ -902,6 +925,16 @@ int oat_uses_marching(const oat_geometry *g, int backproject)
 {
     if (!g) return -1;
     return backproject ? (g->variant_backproject == 4 && march_ht_ok(g)) : (g->variant_project == 4 && march_h_ok(g));
+}
+
+int oat_tile_stats(oat_geometry *g, unsigned long long *h_out, int reset)
+{
+    int rc = check_handle(g); if (rc) return rc;
+    if (!h_out || !g->d_tile_stats) return fail(OAT_ERR_INVALID, "tile statistics are off (oat_set_variant(g, \"tile_stats\", 1))");
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMemcpy(h_out, g->d_tile_stats, sizeof(unsigned long long) * 8, cudaMemcpyDeviceToHost));
+    if (reset) CUDA_TRY(cudaMemset(g->d_tile_stats, 0, sizeof(unsigned long long) * 8));
+    return OAT_OK;
 }
 
 int oat_last_launch_count(const oat_geometry *g) { return g ? g->last_launches : -1; }

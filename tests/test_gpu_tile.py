@@ -1,0 +1,133 @@
+"""GPU parity of the tile-stationary projection kernel (oat_tile.cu; `oat_set_variant(g, "project", 5)`, SURVEY 8(a)
+candidate V2: a brick of the volume staged in shared memory by a TMA box load, every sample evaluated from there)
+against the fp64 oracle, element by element, through the C ABI.  Same tolerance as the default kernels (1e-4).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from oracle import oat_oracle as orc
+    from paper_1304_2017_b200 import binding as oat, build, workloads as wl
+    build.build()
+    assert torch.cuda.is_available()
+    return torch, orc, oat, wl
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    nb = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / nb) if nb > 0 else float(np.linalg.norm(a))
+
+
+def tile_project(torch, oat, g, x, tma=True, nq=None):
+    oat.oat_set_variant(g, "project", 5)
+    oat.oat_set_variant(g, "tile_tma", 1 if tma else 0)
+    if nq:
+        oat.oat_set_variant(g, "tile_nq", nq)
+    y = oat.oat_project(g, torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).cuda())
+    torch.cuda.synchronize()
+    assert oat.oat_last_launch_count(g) == 2        # the tile kernel and the time difference: not the patch kernels
+    return y.cpu().numpy()
+
+
+@pytest.mark.parametrize("tma", [True, False])
+def test_config1_full_against_the_oracle(env, tma):
+    """BASELINE config 1 (32^3, h = spacing / 2): TMA staging and the plain-load staging give the same operator."""
+    torch, orc, oat, wl = env
+    w = wl.config(1)
+    x = w.phantom()
+    g = oat.oat_geometry_create(w)
+    hx = tile_project(torch, oat, g, x, tma=tma)
+    ref = orc.project(w, x.astype(np.float64))
+    assert rel_l2(hx, ref) <= TOL
+    assert np.max(np.abs(hx - ref)) <= 3 * TOL * np.max(np.abs(ref))
+    g.close()
+
+
+def test_chunk_ownership_visits_every_sample_once(env):
+    """The chunks (8 samples) owned over all tiles must add up to the rays' samples: with a constant volume that contains
+    whole shells, g = 4 pi rho^2 (pin P3) -- a chunk missed or marched twice shows up as a step in the data."""
+    torch, orc, oat, wl = env
+    w = wl.small(n=40, q=6, nt=160, kband=32, spacing=0.5, radius=30.0, dt=0.05)
+    x = np.random.default_rng(3).random((w.nz, w.ny, w.nx)).astype(np.float32)
+    g = oat.oat_geometry_create(w)
+    hx = tile_project(torch, oat, g, x, nq=2)       # several (tile, transducer range) items per tile
+    ref = orc.project(w, x.astype(np.float64))
+    assert rel_l2(hx, ref) <= TOL
+    oat.oat_set_variant(g, "tile_stats", 1)
+    tile_project(torch, oat, g, x)
+    cand, pre, rays, chunks = oat.oat_tile_stats(g)[:4]
+    oat.oat_set_variant(g, "tile_stats", 0)
+    n_in_box = oat.oat_num_surface_samples(g)
+    assert cand >= pre >= rays > 0
+    assert 8 * chunks >= n_in_box                   # every in-box sample lies in exactly one owned chunk
+    g.close()
+
+
+def test_non_cubic_grid_without_a_tensor_map(env):
+    """nx = 21 is not a multiple of 4 nodes: rows are not 16-byte aligned, no tensor map can be made, the kernel stages
+    the brick with plain loads; offset origin, transducers off the axes, gain != 1."""
+    torch, orc, oat, wl = env
+    tr = np.array([[25.0, 3.0, -4.0], [-6.0, -22.0, 9.0], [2.0, 5.0, 27.0], [-14.0, 11.0, -19.0]])
+    w = wl.Workload("noncubic", 21, 13, 9, 0.4, (-3.7, -2.1, -1.3), tr, c=1.5, t0=9.0, dt=0.06, nt=150,
+                    surf_step=0.3, kband=32, gain=0.5)
+    x = np.random.default_rng(4).random((w.nz, w.ny, w.nx)).astype(np.float32)
+    g = oat.oat_geometry_create(w)
+    hx = tile_project(torch, oat, g, x)
+    assert rel_l2(hx, orc.project(w, x.astype(np.float64))) <= TOL
+    g.close()
+
+
+def test_ragged_last_band_and_transducer_next_to_the_grid(env):
+    """nt = 70 (last band of 6 samples) and a transducer two cells from the grid (no azimuth window: the `nearq` path)."""
+    torch, orc, oat, wl = env
+    w = wl.small(n=14, q=5, nt=70, kband=32)
+    tr = np.array(w.trans_xyz)
+    tr[0] = np.array([0.5 * 14 * w.spacing + 2 * w.spacing, 0.3, -0.2])
+    w = wl.Workload("near", w.nx, w.ny, w.nz, w.spacing, w.origin, tr, c=w.c, t0=0.0, dt=w.dt, nt=70,
+                    surf_step=w.surf_step, kband=32)
+    x = np.random.default_rng(5).random((w.nz, w.ny, w.nx)).astype(np.float32)
+    g = oat.oat_geometry_create(w)
+    hx = tile_project(torch, oat, g, x)
+    assert rel_l2(hx, orc.project(w, x.astype(np.float64))) <= TOL
+    g.close()
+
+
+def test_unsupported_geometries_keep_the_default_kernels(env):
+    """7 c dt >= 3 spacing (a chunk could leave the brick's margin) or B < 32: variant 5 is ignored, the result is the
+    default path's."""
+    torch, orc, oat, wl = env
+    w = wl.small(n=14, q=4, nt=48, kband=8)
+    x = w.phantom()
+    g = oat.oat_geometry_create(w)
+    oat.oat_set_variant(g, "project", 5)
+    y = oat.oat_project(g, torch.from_numpy(x.astype(np.float32)).cuda())
+    torch.cuda.synchronize()
+    assert rel_l2(y.cpu().numpy(), orc.project(w, x.astype(np.float64))) <= TOL
+    g.close()
+
+
+def test_config3_sampled_rows_full_size_launch(env):
+    """Config 3 on a 96-transducer geometry (the launch shape of the bench's tile leg scaled down): 8 sampled rows against
+    the oracle, all rows against the default marching kernel."""
+    torch, orc, oat, wl = env
+    w = wl.config(3)
+    idx = np.arange(0, w.n_trans, w.n_trans // 96)[:96]
+    ws = w.subset(idx)
+    x = ws.phantom()
+    g = oat.oat_geometry_create(ws)
+    hx = tile_project(torch, oat, g, x)
+    oat.oat_set_variant(g, "project", 4)
+    h4 = oat.oat_project(g, torch.from_numpy(x.astype(np.float32)).cuda()).cpu().numpy()
+    assert rel_l2(hx, h4) <= 1e-5
+    rows = np.sort(np.random.default_rng(11).choice(96, 8, replace=False))
+    ref = orc.project(ws.subset(rows), x.astype(np.float64))
+    assert rel_l2(hx[rows], ref) <= TOL
+    g.close()
