@@ -119,6 +119,22 @@ __device__ __forceinline__ void red_add_v4_if(float4 *addr, float a, float b, fl
                  ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d), "r"((int)pred) : "memory");
 }
 
+// The two reductions of one marching step of H^T: quad L into record `cur` when `fl`, quad H into record `cur + sa` when `fh`
+// (records of 16 bytes from `base`).  One 32 x 32 -> 64 bit multiply-add per address instead of 64-bit index arithmetic.
+__device__ __forceinline__ void red_quads(unsigned long long base, unsigned cur, unsigned sa, bool fl, bool fh,
+                                          float L0, float L1, float L2, float L3, float H0, float H1, float H2, float H3)
+{
+    asm volatile("{\n\t.reg .pred p, q;\n\t.reg .b64 a, b;\n\t.reg .b32 c2;\n\t"
+                 "setp.ne.b32 p, %3, 0;\n\tsetp.ne.b32 q, %4, 0;\n\t"
+                 "mad.wide.u32 a, %1, 16, %0;\n\t"
+                 "add.u32 c2, %1, %2;\n\t"
+                 "mad.wide.u32 b, c2, 16, %0;\n\t"
+                 "@p red.global.add.v4.f32 [a], {%5,%6,%7,%8};\n\t"
+                 "@q red.global.add.v4.f32 [b], {%9,%10,%11,%12};\n\t}"
+                 ::"l"(base), "r"(cur), "r"(sa), "r"((int)fl), "r"((int)fh),
+                   "f"(L0), "f"(L1), "f"(L2), "f"(L3), "f"(H0), "f"(H1), "f"(H2), "f"(H3) : "memory");
+}
+
 // sum acc[i] over the 16 lanes of each half-warp; lane l returns the total of acc[l & 15] of its half (15 shuffles)
 __device__ __forceinline__ float half_warp_transpose_sum(float (&acc)[16], int lane)
 {
@@ -401,7 +417,7 @@ oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__
                                    n2 = o == 0 ? P.nz : o == 1 ? P.nx : P.ny;
                     const int nb = o == 0 ? P.f_nb[0] : o == 1 ? P.f_nb[1] : P.f_nb[2];
                     const int nc = o == 0 ? P.f_nc[0] : o == 1 ? P.f_nc[1] : P.f_nc[2];
-                    float4 *const qb = faces + (o == 0 ? P.f_base[0] : o == 1 ? P.f_base[1] : P.f_base[2]);
+                    const unsigned long long qb = (unsigned long long)(faces + (o == 0 ? P.f_base[0] : o == 1 ? P.f_base[1] : P.f_base[2]));
                     const int sa = nb * nc;                            // records per plane
                     const bool flip = u0 < 0.f;
                     const float s0 = flip ? -u0 : u0, s1 = flip ? -u1 : u1, s2 = flip ? -u2 : u2;   // s0 >= 0: the ray advances along local axis 0
@@ -425,8 +441,7 @@ oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__
                             const unsigned dcur = nxt - cur;
                             const bool chg = dcur != 0u;
                             const bool carry = dcur == (unsigned)sa;       // one cell forward along the dominant axis only
-                            red_add_v4_if(qb + cur, L0, L1, L2, L3, valid & chg);
-                            red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid & chg & !carry);
+                            red_quads(qb, cur, (unsigned)sa, valid & chg, valid & chg & !carry, L0, L1, L2, L3, H0, H1, H2, H3);
                             L0 = chg ? (carry ? H0 : 0.f) : L0; L1 = chg ? (carry ? H1 : 0.f) : L1;
                             L2 = chg ? (carry ? H2 : 0.f) : L2; L3 = chg ? (carry ? H3 : 0.f) : L3;
                             H0 = chg ? 0.f : H0; H1 = chg ? 0.f : H1; H2 = chg ? 0.f : H2; H3 = chg ? 0.f : H3;
@@ -442,8 +457,7 @@ oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__
                             H0 = fmaf(q0, wh, H0); H1 = fmaf(q1, wh, H1); H2 = fmaf(q2, wh, H2); H3 = fmaf(q3, wh, H3);
                         }
                     }
-                    red_add_v4_if(qb + cur, L0, L1, L2, L3, valid);
-                    red_add_v4_if(qb + (cur + (unsigned)sa), H0, H1, H2, H3, valid);
+                    red_quads(qb, cur, (unsigned)sa, valid, valid, L0, L1, L2, L3, H0, H1, H2, H3);
                 }
                 if (last) break;
             }
