@@ -467,6 +467,23 @@ def run_ours(args):
                 cgls = {"iterations": 20, "ms_total": dt_cg, "ms_per_iteration": dt_cg / 20.0, "residual_first_last": [float(res[0]), float(res[-1])]}
             except Exception as ex:
                 cgls = {"error": str(ex)}
+        # ---- measured alternative (SURVEY 8(a) candidate V2, north_star (1)): the tile-stationary projection kernel -- bricks of the
+        # volume staged in shared memory by TMA box loads -- on the same workload and input, after the timed region
+        tile = None
+        if not args.no_next and world == 1:
+            try:
+                y_ref = oat.oat_project(g, x).clone()
+                oat.oat_set_variant(g, "project", 5)
+                y5 = torch.empty_like(y)
+                oat.oat_project(g, x, y5); torch.cuda.synchronize()
+                ms5 = float(oat.oat_last_kernel_ms(g))
+                oat.oat_set_variant(g, "project", 4)
+                d = (y5.double() - y_ref.double()).norm() / y_ref.double().norm()
+                tile = {"kernel": "oat_tile_fwd_kernel (project variant 5, not the default)", "ms_H_tile": ms5, "ms_H_default": k_h,
+                        "rel_l2_vs_default": float(d.item()),
+                        "note": "16^3-cell cores + 3-cell margin per block, 3-D TMA box loads with zero fill, chunk ownership; DESIGN.md section 5.8"}
+            except Exception as ex:
+                tile = {"error": str(ex)}
         cpu = None
         if not args.no_cpu_baseline and world == 1:       # rank 0 at N=1 only
             try:
@@ -497,7 +514,7 @@ def run_ours(args):
                 "ms_H": ms_h, "ms_HT": ms_t,
                 "samples_per_operator": int(n_samples), "samples_per_s": 2.0 * float(tot_samples.item()) / (ms_step * 1e-3),
                 "samples_per_s_H": float(tot_samples.item()) / (ms_h * 1e-3), "samples_per_s_HT": float(tot_samples.item()) / (ms_t * 1e-3),
-                "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "next1": next1, "next2": next2, "next3": next3, "cgls": cgls, "cpu_baseline": cpu,
+                "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "next1": next1, "next2": next2, "next3": next3, "tile_variant": tile, "cgls": cgls, "cpu_baseline": cpu,
                 "paper_context": "PAPER.md Table I: PLS-Int 20-137 min/iteration on a Tesla C2050 for 1,440-11,520 transducers on 210x210x440 voxels (another workload and machine)"}
         print(json.dumps(line), flush=True)
     g.close()
