@@ -236,6 +236,9 @@ def run_ours(args):
     elif world > 1:                                         # weak: N-times denser view sampling, per-GPU work fixed
         w = replace(w_all, trans_xyz=shard.weak_replica_transducers(w_all.trans_xyz, rank, world, 144))
     g = oat.oat_geometry_create(w, local)
+    if args.project_variant != 4:                           # measurement aid: 5 = the tile-stationary projection kernel (not the default)
+        oat.oat_set_variant(g, "project", args.project_variant)
+        note = ((note + "; ") if note else "") + f"NON-DEFAULT projection kernel variant {args.project_variant} (include/oat_probe.h)"
     x = torch.from_numpy(w.phantom()).cuda()
     y = torch.empty((w.n_trans, w.nt), dtype=torch.float32, device="cuda")
     ynoise = torch.from_numpy(dense_data(w)).cuda()
@@ -536,6 +539,8 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=64, help="transducers in the oracle's timed sample (SURVEY 8(d): 64)")
     ap.add_argument("--ref-sample", type=int, default=8, help="transducers per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--project-variant", type=int, default=4, choices=[0, 4, 5],
+                    help="measurement aid: 4 = default kernels, 5 = tile-stationary projection kernel, 0 = generic patch kernel")
     ap.add_argument("--no-next", action="store_true", help="skip the NEXT-row legs after the timed region")
     args = ap.parse_args()
     if args.impl == "reference":
