@@ -463,6 +463,33 @@ int dot_sync(oat_geometry *G, const float *a, const float *b, size_t n, double *
     return OAT_OK;
 }
 
+// dot product into slot `i` of the device scalars (asynchronous: the CG loops read it back on the device)
+int dot_dev(oat_geometry *G, const float *a, const float *b, size_t n, int i, cudaStream_t st)
+{
+    CUDA_TRY(cudaMemsetAsync(G->d_scal + i, 0, sizeof(double), st));
+    oat_launch_dot(a, b, (long long)n, G->d_scal + i, st);
+    return OAT_OK;
+}
+
+// pinned curves of a CG run (written by the scalar kernel through UVA), copied to the caller's arrays at the end
+struct CgCurves {
+    double *a = nullptr, *b = nullptr;
+    int n = 0;
+    int init(int n_iter, bool want_a, bool want_b)
+    {
+        n = n_iter + 1;
+        if (want_a) CUDA_TRY(cudaMallocHost((void **)&a, sizeof(double) * (size_t)n));
+        if (want_b) CUDA_TRY(cudaMallocHost((void **)&b, sizeof(double) * (size_t)n));
+        return OAT_OK;
+    }
+    void finish(double *ha, double *hb)
+    {
+        if (a && ha) memcpy(ha, a, sizeof(double) * (size_t)n);
+        if (b && hb) memcpy(hb, b, sizeof(double) * (size_t)n);
+    }
+    ~CgCurves() { if (a) cudaFreeHost(a); if (b) cudaFreeHost(b); }
+};
+
 // H = H^e D G (Eq. 11) and H^T = G^T D^T H^e† (L168); without taps the EIR is left out
 int project_full(oat_geometry *G, const float *d_x, float *d_u, cudaStream_t st)
 {
@@ -630,38 +657,33 @@ int oat_cgls(oat_geometry *g, const float *d_y, float *d_x, int n_iter, double *
     if ((rc = ensure(&g->d_x3, g->n_vox))) return rc;     // s
     if ((rc = ensure(&g->d_x4, g->n_vox))) return rc;     // p
     float *r = g->d_y2, *qv = g->d_y3, *s = g->d_x3, *p = g->d_x4;
+    // scalars stay on the device (slots: oat_kernels.cu, oat_cg_scalar_kernel); ONE synchronisation, at the end
+    CgCurves cv;
+    if ((rc = cv.init(n_iter, h_res != nullptr, h_grad != nullptr))) return rc;
+    double *sc = g->d_scal;
     CUDA_TRY(cudaMemsetAsync(d_x, 0, sizeof(float) * g->n_vox, st));
     CUDA_TRY(cudaMemcpyAsync(r, d_y, sizeof(float) * g->n_dat, cudaMemcpyDeviceToDevice, st));
     if ((rc = backproject_impl(g, r, s, st))) return rc;
     CUDA_TRY(cudaMemcpyAsync(p, s, sizeof(float) * g->n_vox, cudaMemcpyDeviceToDevice, st));
-    double gamma, ynorm2, rr;
-    if ((rc = dot_sync(g, s, s, g->n_vox, &gamma, st))) return rc;
-    if ((rc = dot_sync(g, d_y, d_y, g->n_dat, &ynorm2, st))) return rc;
-    const double ynorm = sqrt(ynorm2);
-    if (h_res) h_res[0] = ynorm > 0 ? 1.0 : 0.0;
-    if (h_grad) h_grad[0] = sqrt(gamma);
+    if ((rc = dot_dev(g, s, s, g->n_vox, 0, st))) return rc;               // gamma
+    if ((rc = dot_dev(g, d_y, d_y, g->n_dat, 6, st))) return rc;           // |y|^2
+    oat_launch_cg_scalar(sc, 0, 0, 0.0, cv.a, cv.b, st);
     for (int it = 0; it < n_iter; ++it) {
-        double qq;
         if ((rc = project_impl(g, p, qv, st))) return rc;
-        if ((rc = dot_sync(g, qv, qv, g->n_dat, &qq, st))) return rc;
-        if (qq > 0 && gamma > 0) {
-            const double alpha = gamma / qq;
-            oat_launch_axpy((float)alpha, p, d_x, (long long)g->n_vox, st);
-            oat_launch_axpy((float)-alpha, qv, r, (long long)g->n_dat, st);
-            if ((rc = backproject_impl(g, r, s, st))) return rc;
-            double gamma_new;
-            if ((rc = dot_sync(g, s, s, g->n_vox, &gamma_new, st))) return rc;
-            const double beta = gamma_new / gamma;
-            gamma = gamma_new;
-            oat_launch_xpay(s, (float)beta, p, (long long)g->n_vox, st);
-        }
-        if (h_res) {
-            if ((rc = dot_sync(g, r, r, g->n_dat, &rr, st))) return rc;
-            h_res[it + 1] = ynorm > 0 ? sqrt(rr) / ynorm : 0.0;
-        }
-        if (h_grad) h_grad[it + 1] = sqrt(gamma);
+        if ((rc = dot_dev(g, qv, qv, g->n_dat, 1, st))) return rc;
+        oat_launch_cg_scalar(sc, 1, it, 0.0, nullptr, nullptr, st);         // alpha = gamma / |q|^2 (flag 0: leave everything as it is)
+        oat_launch_axpy_dev(sc, 3, 7, 1.f, p, d_x, (long long)g->n_vox, st);
+        oat_launch_axpy_dev(sc, 3, 7, -1.f, qv, r, (long long)g->n_dat, st);
+        if ((rc = backproject_impl(g, r, s, st))) return rc;
+        if ((rc = dot_dev(g, s, s, g->n_vox, 2, st))) return rc;
+        oat_launch_cg_scalar(sc, 2, it, 0.0, nullptr, nullptr, st);         // beta, gamma
+        oat_launch_xpay_dev(s, sc, 4, 7, p, (long long)g->n_vox, st);
+        if (h_res && (rc = dot_dev(g, r, r, g->n_dat, 5, st))) return rc;
+        oat_launch_cg_scalar(sc, 3, it, 0.0, cv.a, cv.b, st);
     }
+    CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaStreamSynchronize(st));
+    cv.finish(h_res, h_grad);
     return OAT_OK;
 }
 
@@ -750,48 +772,41 @@ static int pls_cg_impl(oat_geometry *g, const float *d_u, float *d_x, int n_iter
                            reinterpret_cast<const float2 *>(u), g->d_p0, g->d_sv, x, st);
         return OAT_OK;
     };
+    CgCurves cv;
+    if ((rc = cv.init(n_iter, h_obj != nullptr, h_grad != nullptr))) return rc;
+    double *sc = g->d_scal;
     CUDA_TRY(cudaMemsetAsync(d_x, 0, sizeof(float) * g->n_vox, st));
     CUDA_TRY(cudaMemcpyAsync(d, d_u, sizeof(float) * n_dat, cudaMemcpyDeviceToDevice, st));
     if ((rc = bwd(d_u, r))) return rc;
     CUDA_TRY(cudaMemcpyAsync(p, r, sizeof(float) * g->n_vox, cudaMemcpyDeviceToDevice, st));
-    double rr, dd;
-    if ((rc = dot_sync(g, r, r, g->n_vox, &rr, st))) return rc;
-    if ((rc = dot_sync(g, d, d, n_dat, &dd, st))) return rc;
-    if (h_obj) h_obj[0] = dd;
-    if (h_grad) h_grad[0] = sqrt(rr);
+    if ((rc = dot_dev(g, r, r, g->n_vox, 0, st))) return rc;               // |r|^2
+    if ((rc = dot_dev(g, d, d, n_dat, 5, st))) return rc;                  // |u|^2
+    oat_launch_cg_scalar(sc, 4, 0, mu, cv.a, cv.b, st);
     for (int it = 0; it < n_iter; ++it) {
-        double pw;
         if ((rc = fwd(p, q))) return rc;
         if ((rc = bwd(q, w))) return rc;
         if (mu > 0) oat_launch_penalty(g->dev, p, w, (float)mu, 1.f, st);          // w += mu L p
-        if ((rc = dot_sync(g, p, w, g->n_vox, &pw, st))) return rc;
-        if (!(pw > 0) || rr == 0) {
-            if (h_obj) h_obj[it + 1] = h_obj[it];
-            if (h_grad) h_grad[it + 1] = h_grad[it];
-            continue;
-        }
-        const double alpha = rr / pw;
-        oat_launch_axpy((float)alpha, p, d_x, (long long)g->n_vox, st);
-        oat_launch_axpy((float)-alpha, q, d, (long long)n_dat, st);
-        oat_launch_axpy((float)-alpha, w, r, (long long)g->n_vox, st);
-        double rr_new;
-        if ((rc = dot_sync(g, r, r, g->n_vox, &rr_new, st))) return rc;
-        const double beta = rr_new / rr;
-        rr = rr_new;
-        oat_launch_xpay(r, (float)beta, p, (long long)g->n_vox, st);
+        if ((rc = dot_dev(g, p, w, g->n_vox, 1, st))) return rc;
+        oat_launch_cg_scalar(sc, 1, it, mu, nullptr, nullptr, st);         // alpha = |r|^2 / <p, w> (flag 0: a degenerate step changes nothing)
+        oat_launch_axpy_dev(sc, 3, 7, 1.f, p, d_x, (long long)g->n_vox, st);
+        oat_launch_axpy_dev(sc, 3, 7, -1.f, q, d, (long long)n_dat, st);
+        oat_launch_axpy_dev(sc, 3, 7, -1.f, w, r, (long long)g->n_vox, st);
+        if ((rc = dot_dev(g, r, r, g->n_vox, 2, st))) return rc;
+        oat_launch_cg_scalar(sc, 2, it, mu, nullptr, nullptr, st);         // beta, |r|^2
+        oat_launch_xpay_dev(r, sc, 4, 7, p, (long long)g->n_vox, st);
         if (h_obj) {
-            double pen = 0.0;
-            if ((rc = dot_sync(g, d, d, n_dat, &dd, st))) return rc;
+            if ((rc = dot_dev(g, d, d, n_dat, 5, st))) return rc;
+            CUDA_TRY(cudaMemsetAsync(sc + 6, 0, sizeof(double), st));
             if (mu > 0) {
                 oat_launch_penalty(g->dev, d_x, w, 1.f, 0.f, st);
-                if ((rc = dot_sync(g, d_x, w, g->n_vox, &pen, st))) return rc;
+                oat_launch_dot(d_x, w, (long long)g->n_vox, sc + 6, st);
             }
-            h_obj[it + 1] = dd + mu * pen;
         }
-        if (h_grad) h_grad[it + 1] = sqrt(rr);
+        oat_launch_cg_scalar(sc, 5, it, mu, cv.a, cv.b, st);
     }
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaStreamSynchronize(st));
+    cv.finish(h_obj, h_grad);
     return OAT_OK;
 }
 

@@ -109,6 +109,11 @@ cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift
 void oat_launch_dot(const float *a, const float *b, long long n, double *out, cudaStream_t st);
 void oat_launch_axpy(float alpha, const float *x, float *y, long long n, cudaStream_t st);   // y += alpha x
 void oat_launch_xpay(const float *x, float beta, float *y, long long n, cudaStream_t st);    // y = x + beta y
+// device-scalar forms for the CG loops: y += sign * scal[idx] x, y = x + scal[idx] y (both no-ops when scal[flag] == 0), and the
+// one-thread scalar steps (op codes in oat_kernels.cu); curves point to pinned host memory
+void oat_launch_axpy_dev(const double *scal, int idx, int flag, float sign, const float *x, float *y, long long n, cudaStream_t st);
+void oat_launch_xpay_dev(const float *x, const double *scal, int idx, int flag, float *y, long long n, cudaStream_t st);
+void oat_launch_cg_scalar(double *scal, int op, int it, double mu, double *curve_a, double *curve_b, cudaStream_t st);
 // row NEXT-1 (oat_next.cu): EIR convolution / correlation along time (Eq. 14 / Eq. 21) and the penalty stencil (Eq. 34)
 cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float *he, int L, int Q, int K, cudaStream_t st);
 void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha, float beta, cudaStream_t st);   // out = beta out + alpha L x

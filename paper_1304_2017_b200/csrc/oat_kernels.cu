@@ -480,6 +480,57 @@ __global__ void oat_xpay_kernel(const float *__restrict__ x, float beta, float *
         y[i] = fmaf(beta, y[i], x[i]);
 }
 
+// The CG loops keep their scalars on the device (no host round trip per iteration): the vector updates read the step from
+// scal[idx] and do nothing when scal[flag] == 0 (a degenerate step: the loop leaves the vectors as they are).
+__global__ void oat_axpy_dev_kernel(const double *__restrict__ scal, int idx, int flag, float sign, const float *__restrict__ x,
+                                    float *__restrict__ y, long long n)
+{
+    if (scal[flag] == 0.0) return;
+    const float alpha = sign * (float)scal[idx];
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        y[i] = fmaf(alpha, x[i], y[i]);
+}
+
+__global__ void oat_xpay_dev_kernel(const float *__restrict__ x, const double *__restrict__ scal, int idx, int flag, float *__restrict__ y, long long n)
+{
+    if (scal[flag] == 0.0) return;
+    const float beta = (float)scal[idx];
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        y[i] = fmaf(beta, y[i], x[i]);
+}
+
+// Scalar steps of the CG loops, one thread.  s: [0] gamma = |s|^2 (CGLS) or |r|^2 (PLS), [1] |q|^2 or <p, w>, [2] the new gamma,
+// [3] alpha, [4] beta, [5] |r|^2 or |d|^2 (data residual), [6] |y|^2 or the penalty x^T L x, [7] flag: 0 = degenerate step.
+// curves (pinned host memory, written through UVA): a[it], b[it].
+__global__ void oat_cg_scalar_kernel(double *s, int op, int it, double mu, double *curve_a, double *curve_b)
+{
+    switch (op) {
+    case 0:                                                // CGLS start: curves[0] = (1 or 0, |s|)
+        if (curve_a) curve_a[0] = s[6] > 0.0 ? 1.0 : 0.0;
+        if (curve_b) curve_b[0] = sqrt(s[0]);
+        break;
+    case 1:                                                // alpha = gamma / [1]
+        s[7] = (s[1] > 0.0 && s[0] > 0.0) ? 1.0 : 0.0;
+        s[3] = s[7] != 0.0 ? s[0] / s[1] : 0.0;
+        break;
+    case 2:                                                // beta = gamma_new / gamma; gamma = gamma_new
+        if (s[7] != 0.0) { s[4] = s[2] / s[0]; s[0] = s[2]; }
+        break;
+    case 3:                                                // CGLS curves of iteration it (after the update)
+        if (curve_a) curve_a[it + 1] = s[6] > 0.0 ? sqrt(s[5]) / sqrt(s[6]) : 0.0;
+        if (curve_b) curve_b[it + 1] = sqrt(s[0]);
+        break;
+    case 4:                                                // PLS start: objective |u|^2, gradient |r|
+        if (curve_a) curve_a[0] = s[5];
+        if (curve_b) curve_b[0] = sqrt(s[0]);
+        break;
+    case 5:                                                // PLS curves: |d|^2 + mu x^T L x, |r|; a degenerate step repeats the last values
+        if (curve_a) curve_a[it + 1] = s[7] != 0.0 ? s[5] + mu * s[6] : curve_a[it];
+        if (curve_b) curve_b[it + 1] = s[7] != 0.0 ? sqrt(s[0]) : curve_b[it];
+        break;
+    }
+}
+
 inline int grid_for(long long n, int block)
 {
     long long g = (n + block - 1) / block;
@@ -607,6 +658,21 @@ void oat_launch_dot(const float *a, const float *b, long long n, double *out, cu
 void oat_launch_axpy(float alpha, const float *x, float *y, long long n, cudaStream_t st)
 {
     if (n > 0) oat_axpy_kernel<<<grid_for(n, 256), 256, 0, st>>>(alpha, x, y, n);
+}
+
+void oat_launch_axpy_dev(const double *scal, int idx, int flag, float sign, const float *x, float *y, long long n, cudaStream_t st)
+{
+    if (n > 0) oat_axpy_dev_kernel<<<grid_for(n, 256), 256, 0, st>>>(scal, idx, flag, sign, x, y, n);
+}
+
+void oat_launch_xpay_dev(const float *x, const double *scal, int idx, int flag, float *y, long long n, cudaStream_t st)
+{
+    if (n > 0) oat_xpay_dev_kernel<<<grid_for(n, 256), 256, 0, st>>>(x, scal, idx, flag, y, n);
+}
+
+void oat_launch_cg_scalar(double *scal, int op, int it, double mu, double *curve_a, double *curve_b, cudaStream_t st)
+{
+    oat_cg_scalar_kernel<<<1, 1, 0, st>>>(scal, op, it, mu, curve_a, curve_b);
 }
 
 void oat_launch_xpay(const float *x, float beta, float *y, long long n, cudaStream_t st)
