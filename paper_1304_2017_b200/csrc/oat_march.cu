@@ -188,7 +188,6 @@ oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__
     __shared__ double s_frame[16];
     __shared__ RingRow s_ring[OAT_RI];
     __shared__ float4 s_qa[OAT_MT / 32][OAT_QNH], s_qs[OAT_MT / 32][OAT_QNH];
-    __shared__ float s_red[OAT_MT / 32][32];
     __shared__ int s_flag;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -264,7 +263,7 @@ oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__
                 head += n; if (head >= OAT_QNH) head -= OAT_QNH;
                 cnt -= n;
 #pragma unroll
-                for (int k = 0; k < 16; ++k) {
+                for (int k = 15; k >= 0; --k) {            // from the middle of the ray outwards: both halves start in (nearly) the same cell, one sector request
                     const float kk = (float)k - 15.5f;
                     float tx[OAT_NRH], ty[OAT_NRH], tz[OAT_NRH], rx[OAT_NRH], ry[OAT_NRH], rz[OAT_NRH];
 #pragma unroll
@@ -290,12 +289,14 @@ oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__
         }
         // S5: half-warp sums -> fp64 cross-warp combine -> one fp64 atomic per time sample
         const float tot = half_warp_transpose_sum(acc, lane);
-        s_red[warp][lane < 16 ? lane : 47 - lane] = tot;           // lane l >= 16 holds sample 31 - (l - 16)
+        // the warps' partial sums go through the (now empty) ray queues
+        float *const s_red = reinterpret_cast<float *>(s_qa);       // [warp][32] at a stride of OAT_QNH float4
+        s_red[warp * (OAT_QNH * 4) + (lane < 16 ? lane : 47 - lane)] = tot;   // lane l >= 16 holds sample 31 - (l - 16)
         __syncthreads();
         if (warp == 0) {
             double sum = 0.0;
 #pragma unroll
-            for (int w = 0; w < OAT_MT / 32; ++w) sum += (double)s_red[w][lane];
+            for (int w = 0; w < OAT_MT / 32; ++w) sum += (double)s_red[w * (OAT_QNH * 4) + lane];
             const int k = band.k0 + lane;
             const double rho = P.c * (P.t0 + (double)k * P.dt);
             if (lane < band.nk && rho > 0.0 && sum != 0.0) atomicAdd(&g[(size_t)q * P.K + k], rho * rho * sum);
