@@ -180,7 +180,7 @@ __device__ __forceinline__ float half_warp_transpose_sum(float (&acc)[16], int l
 #endif
 #define OAT_QNH (16 * OAT_NRH + 32)    // queue entries per warp: at most 16 NRH - 1 left over + 32 new
 #ifndef OAT_MBLKH
-#define OAT_MBLKH (OAT_NRH == 1 ? 1024 / OAT_MT : 768 / OAT_MT)
+#define OAT_MBLKH (OAT_NRH == 1 ? 1152 / OAT_MT : 768 / OAT_MT)   // 9 blocks = 36 warps at 56 registers, no spills (8 blocks: 57.5 ms, 9: 54.6, 10: spills, 57.3)
 #endif
 __global__ void __launch_bounds__(OAT_MT, OAT_MBLKH)
 oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__restrict__ y_out, double *__restrict__ g)
