@@ -25,7 +25,7 @@
 #ifndef OAT_MT
 #define OAT_MT 128         // threads per block of the marching kernels
 #endif
-#define OAT_BU 8           // steps per trip of the (rolled) backprojection marching loop
+#define OAT_BU 4           // steps per trip of the (rolled) backprojection marching loop
 
 struct OatBand {
     double s_mid;      // radius of the band's anchor (k0 + (B-1)/2) in voxel units: rho/ds
