@@ -427,7 +427,7 @@ oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__
                     float L0 = 0.f, L1 = 0.f, L2 = 0.f, L3 = 0.f, H0 = 0.f, H1 = 0.f, H2 = 0.f, H3 = 0.f;
                     unsigned cur = 0;                                  // record index within orientation o (32-bit: one IMAD.WIDE per reduction)
                     bool valid = false;
-                    // 8 steps per trip of a rolled loop: the fully unrolled body missed the instruction cache
+                    // OAT_BU (4) steps per trip of a rolled loop: the fully unrolled body misses the instruction cache
 #pragma unroll 1
                     for (int kb = 0; kb < 32; kb += OAT_BU) {
                         const float kbase = (float)kb - 15.5f;
