@@ -169,7 +169,7 @@ __device__ __forceinline__ float half_warp_transpose_sum(float (&acc)[16], int l
 // lanes 16..31 samples 31..16 of the same ray walked BACKWARDS with the direction negated -- fma(-s, -kk, a) ==
 // fma(s, kk, a), so both halves run the same instruction stream with the same immediates kk = k' - 15.5 and the
 // positions are bit-identical to a forward walk.  16 accumulators per lane (sample k' of the lower half, 31 - k' of the
-// upper) fit the 64-register budget of 8 resident blocks per SM.
+// upper) fit the 56-register budget of 9 resident blocks per SM.
 // Per step: 3 FFMA (position), 3 FADD.RM (floor), 1 IADD + 2 IMAD (record index), 1 ISETP (new cell?), 1 IMAD.WIDE,
 // 1 predicated 256-bit load of the cell's polynomial record -- only when the ray has entered a new cell, ~2.2 samples
 // share one load --, 6 FADD (fractions), 7 FFMA (Horner in fx, fy, fz) + 1 FFMA (quadrature weight): 26 instructions.
