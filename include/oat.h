@@ -125,6 +125,38 @@ int oat_backproject_eir(oat_geometry *geom, const float *d_u, float *d_x, void *
 int oat_penalty_apply(oat_geometry *geom, const float *d_x, float *d_lx, void *cuda_stream);
 int oat_penalty_value(oat_geometry *geom, const float *d_x, double *value, void *cuda_stream);
 
+/* ---- Penalty value without any allocation, for callers that cannot call cudaMalloc.
+ *
+ * Such callers exist: an application that has given all free GPU memory to its own pool (a further cudaMalloc fails or
+ * eats into the pool), and a real-time acquisition / reconstruction loop that may not tolerate the device-wide
+ * synchronisation every cudaMalloc and cudaFree brings.  oat_penalty_value does not work for them: it needs a geometry
+ * handle (creating one allocates) and allocates a volume-sized scratch buffer the first time it runs.
+ *
+ * oat_penalty_value_noalloc computes the same R(x) = x^T L x (Eq. 34, reading G21) with no handle and no
+ * allocation of any kind (no cudaMalloc / cudaFree / cudaMallocHost, no allocating library routine): its scratch -- the
+ * fp32 volume L x plus one fp64 accumulator -- is a fixed array inside liboat.so's device image.
+ *
+ *   nx, ny, nz  nodes per axis, each >= 1, with nx*ny*nz <= OAT_NOALLOC_MAX_VOXELS; a larger volume is refused with
+ *               OAT_ERR_INVALID and a message that names the limit (nothing is launched).
+ *   d_x         DEVICE, nz*ny*nx fp32, x fastest, owned by the caller, read only; must live on the calling thread's
+ *               CURRENT device (checked; host pointers are refused too).
+ *   h_value     HOST, one double, owned by the caller; written before the call returns.
+ *   cuda_stream a stream of the current device (NULL = legacy default stream).  The work is enqueued there and the call
+ *               waits for that stream before returning.
+ *
+ * Cost of the limit: the array is 8 MiB + 256 B (OAT_NOALLOC_MAX_VOXELS = 2^21 voxels, e.g. 128^3) and every GPU on which
+ * this process uses liboat.so carries it until the process exits, whether or not this function is ever called.
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress; cached per device afterwards).
+ * Make that first call at start-up, before any stream capture begins.
+ * Sharing: all calls on one device use the same array, and it keeps what the previous call left.  The function zeroes
+ * the accumulator itself and overwrites every element of L x it reads, so back-to-back calls are independent -- but two
+ * calls whose GPU work can overlap (different streams, or different host threads) race on the array and return garbage.
+ * Serialise them.
+ * Result: identical arithmetic to oat_penalty_value (fp32 stencil, fp64 sum); the two agree to the rounding of the
+ * fp64 atomic summation order (~1e-15 relative). */
+#define OAT_NOALLOC_MAX_VOXELS (1 << 21)
+int oat_penalty_value_noalloc(int32_t nx, int32_t ny, int32_t nz, const float *d_x, double *h_value, void *cuda_stream);
+
 /* PLS-Int (Eq. 29; reading G22): n_iter steps of linear CG on (H^T H + mu L) x = H^T u from x = 0 with
  * H = H^e D G (the EIR set by oat_eir_set, if any); one H and one H^T per iteration (L273); fp32 vectors, fp64 dot
  * products.  d_u: Q*K (read), d_x: nz*ny*nx (OVERWRITTEN with the iterate after n_iter steps), mu >= 0.

@@ -14,12 +14,13 @@ _LIB_PATH = Path(__file__).resolve().parent / "csrc" / "liboat.so"
 _lib = None
 
 OAT_OK, OAT_ERR_INVALID, OAT_ERR_ALLOC, OAT_ERR_CUDA = 0, -1, -2, -3
+OAT_NOALLOC_MAX_VOXELS = 1 << 21     # include/oat.h: largest volume oat_penalty_value_noalloc accepts
 
 EXPORTS = [
     "oat_geometry_create", "oat_geometry_destroy", "oat_num_voxels", "oat_num_samples",
     "oat_num_surface_samples", "oat_project", "oat_backproject", "oat_adjoint_check",
     "oat_project_host", "oat_backproject_host", "oat_cgls", "oat_set_variant",
-    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_pls_cg", "oat_fbp", "oat_fbp_weights", "oat_sph_set", "oat_sph_set_aperture", "oat_sph_project", "oat_sph_backproject", "oat_sph_pls_cg",
+    "oat_eir_set", "oat_eir_apply", "oat_project_eir", "oat_backproject_eir", "oat_penalty_apply", "oat_penalty_value", "oat_penalty_value_noalloc", "oat_pls_cg", "oat_fbp", "oat_fbp_weights", "oat_sph_set", "oat_sph_set_aperture", "oat_sph_project", "oat_sph_backproject", "oat_sph_pls_cg",
     "oat_last_launch_count", "oat_uses_marching", "oat_last_kernel_ms", "oat_tile_stats", "oat_measure_red_rate", "oat_measure_gather_rate", "oat_measure_gather_rate_ex", "oat_measure_red_rate_ex", "oat_last_error", "oat_version",
 ]
 
@@ -98,6 +99,8 @@ def load():
     lib.oat_backproject_eir.argtypes = [vp, fp, fp, vp]
     lib.oat_penalty_apply.argtypes = [vp, fp, fp, vp]
     lib.oat_penalty_value.argtypes = [vp, fp, dp, vp]
+    lib.oat_penalty_value_noalloc.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, fp, dp, vp]
+    lib.oat_penalty_value_noalloc.restype = ctypes.c_int
     lib.oat_pls_cg.argtypes = [vp, fp, fp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
     lib.oat_sph_set.argtypes = [vp, ctypes.c_int32, ctypes.c_double, ctypes.c_double, fp]
     lib.oat_sph_project.argtypes = [vp, fp, fp, vp]
@@ -354,6 +357,25 @@ def oat_penalty_apply(g, x, lx=None, stream=None):
 def oat_penalty_value(g, x, stream=None) -> float:
     v = ctypes.c_double(0.0)
     _check(load().oat_penalty_value(g.handle, _dev_ptr(x, oat_num_voxels(g), "x", g), ctypes.byref(v), _stream(stream)))
+    return float(v.value)
+
+
+def oat_penalty_value_noalloc(x, stream=None) -> float:
+    """R(x) = x^T L x for a (nz, ny, nx) float32 CUDA tensor of at most OAT_NOALLOC_MAX_VOXELS elements, through the
+    library entry point that needs no geometry handle and allocates nothing (its scratch is a fixed array inside
+    liboat.so).  It exists for programs that may not call cudaMalloc once they are running -- all GPU memory already
+    belongs to their own pool, or the device-wide stall of an allocation is not tolerable in their acquisition loop.
+    Larger volumes raise OatError (OAT_ERR_INVALID) naming the limit; use oat_penalty_value for those.  Calls share the
+    library's one scratch array per GPU: do not run two of them concurrently on the same device.  This wrapper itself
+    only marshals arguments; it makes x's device current for the call, as the entry point works on the current device."""
+    import torch
+    if not isinstance(x, torch.Tensor) or not x.is_cuda or x.dtype != torch.float32 or not x.is_contiguous() or x.dim() != 3:
+        raise OatError(OAT_ERR_INVALID, "x must be a contiguous float32 CUDA tensor of shape (nz, ny, nx)")
+    nz, ny, nx = (int(v) for v in x.shape)
+    v = ctypes.c_double(0.0)
+    with torch.cuda.device(x.device):
+        _check(load().oat_penalty_value_noalloc(ctypes.c_int32(nx), ctypes.c_int32(ny), ctypes.c_int32(nz),
+                                                ctypes.c_void_p(x.data_ptr()), ctypes.byref(v), _stream(stream)))
     return float(v.value)
 
 

@@ -18,7 +18,7 @@ from pathlib import Path
 
 CSRC = Path(__file__).resolve().parent / "csrc"
 LIB = CSRC / "liboat.so"
-SOURCES = ["oat_api.cu", "oat_march.cu", "oat_tile.cu", "oat_kernels.cu", "oat_next.cu", "oat_probe.cu"]
+SOURCES = ["oat_api.cu", "oat_march.cu", "oat_tile.cu", "oat_kernels.cu", "oat_next.cu", "oat_probe.cu", "oat_noalloc.cu"]
 HEADERS = ["oat_internal.h", "../../include/oat.h", "../../include/oat_probe.h"]
 
 NVCC_FLAGS = [
