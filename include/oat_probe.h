@@ -14,12 +14,12 @@ extern "C" {
 #endif
 
 /* Kernel selection for tests and measurements.  key = "project" / "backproject": variant 4 = marching kernels (default,
- * used when the geometry allows: B = 32, records indexable with 32 bits, c dt <= spacing), 5 = tile-stationary kernels
- * (oat_tile.cu), 0 = the generic patch kernel that otherwise serves as the fall-back.  key = "tile_nq": transducers per
- * work item of the tile-stationary projection; "tile_nq_bwd": of the tile-stationary backprojection (default 16; its
- * accumulators are 32-bit fixed point in shared memory, flushed per item: rel-L2 8e-5 .. 6e-4 on the BASELINE configs, i.e.
- * NOT within the product tolerance of 1e-4 -- a measured experiment); "tile_tma": 0 stages the bricks
- * with plain loads; "tile_stats": 1 collects the counters of oat_tile_stats.  key = "morton_shift": log2 of the cell size of the patch order (default 6).
+ * used when the geometry allows: B = 32, records indexable with 32 bits, c dt <= spacing), 0 = the generic patch kernel that
+ * otherwise serves as the fall-back; "project" also takes 5 = the tile-stationary projection kernel (oat_tile.cu), which
+ * holds the product tolerance.  Every selectable kernel is within 1e-4 of the oracle: "backproject" 5 (the round-2
+ * tile-stationary H^T with 32-bit fixed-point accumulators, 8e-5 .. 6e-4, no overflow guard) has been removed from the
+ * library and is refused; its measurement is profiles/r2_tile_bwd.md.  key = "tile_nq": transducers
+ * per work item of the tile-stationary projection; "tile_tma": 0 stages the bricks with plain loads; "tile_stats": 1 collects the counters of oat_tile_stats.  key = "morton_shift": log2 of the cell size of the patch order (default 6).
  * key = "record_limit_log2": pretend record indices have that many bits (tests of the automatic fall-back).
  * Unknown key or value => OAT_ERR_INVALID. */
 int oat_set_variant(oat_geometry *geom, const char *key, int variant);

@@ -81,8 +81,7 @@ struct oat_geometry {
     long long n_surface_samples = -1;
     int variant_project = 4, variant_backproject = 4;   // 4 = marching kernels, 0 = generic patch kernel (oat_probe.h)
     int tile_tma = 1;                         // 0: the tile kernels stage the brick with plain loads instead of TMA (measurement aid)
-    int tile_nq_bwd = 16;                     // ... of the tile-stationary H^T (its fixed-point accumulators are flushed per item)
-    int tile_nq = 1024;                       // transducers per (tile, transducer range) item of the tile-stationary kernels
+    int tile_nq = 1024;                       // transducers per (tile, transducer range) item of the tile-stationary projection
     unsigned long long *d_tile_stats = nullptr;   // enumeration counters of the tile kernels (oat_probe.h), NULL = off
     bool march_ok = false;                    // ray anchors fit the 10-bit packed offsets of the marching H^T queue, step <= 1
     size_t record_limit = (size_t)1 << 31;    // the marching kernels index records with 32 bits (lowered only by tests)
@@ -292,8 +291,6 @@ int build_geometry(oat_geometry *G)
     P.q_count = nullptr; P.q_done = nullptr;
     P.dir = nullptr;
     P.max_band_dirs = max_band_dirs;
-    { float om = 0.f; for (const OatRing &r : rings) if (r.omega > om) om = r.omega; P.omega_max = om; }
-    P.samples_per_cell = (ds / h) * (ds / h) / P.step;
     if (B == 32 && n_dir > 0 && n_dir < (1LL << 31)) {     // 16 B per direction; otherwise the generic kernel is used
         CUDA_TRY(cudaMalloc((void **)&G->d_dir, sizeof(double2) * (size_t)n_dir));
         P.dir = G->d_dir;
@@ -328,7 +325,7 @@ int build_geometry(oat_geometry *G)
     G->n_pad = (size_t)P.pz * P.pxy;
     if (G->n_pad >= (1ULL << 31)) return fail(OAT_ERR_INVALID, "padded grid has more than 2^31 nodes");
     CUDA_TRY(cudaMalloc((void **)&G->d_g, sizeof(double) * (G->n_dat ? G->n_dat : 1)));
-    CUDA_TRY(cudaMalloc((void **)&G->d_scal, sizeof(double) * 16));   // [0..7] CG scalars, [8] max |coef| of the tile-stationary H^T
+    CUDA_TRY(cudaMalloc((void **)&G->d_scal, sizeof(double) * 16));   // [0..7] CG scalars, rest spare
     CUDA_TRY(cudaMalloc((void **)&G->d_counter, sizeof(unsigned long long)));
     CUDA_TRY(cudaMallocHost((void **)&G->h_scal, sizeof(double) * 8));
     CUDA_TRY(cudaEventCreate(&G->ev0));
@@ -429,16 +426,6 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
 {
     const OatDev &P = G->dev;
     G->last_launches = 0;
-    if (G->variant_backproject == 5 && oat_tile_supported(P)) {       // tile-stationary kernel (measured alternative)
-        int rc0 = ensure(&G->d_coef, G->n_dat); if (rc0) return rc0;
-        oat_launch_coef(P, d_y, G->d_coef, st);
-        CUDA_TRY(cudaEventRecord(G->ev0, st));
-        CUDA_TRY(oat_launch_tile_bwd(P, G->d_coef, reinterpret_cast<float *>(G->d_scal + 8), d_x, G->d_counter, G->tile_nq_bwd, st));
-        CUDA_TRY(cudaEventRecord(G->ev1, st));
-        G->ev_valid = true;
-        G->last_launches = 3;
-        return OAT_OK;
-    }
     const bool march = G->variant_backproject >= 4 && march_ht_ok(G);
     int rc = ensure_patches(G); if (rc) return rc;
     if (march) {
@@ -936,8 +923,13 @@ int oat_set_variant(oat_geometry *g, const char *key, int variant)
         } else if (!variant && g->d_tile_stats) { CUDA_TRY(cudaDeviceSynchronize()); cudaFree(g->d_tile_stats); g->d_tile_stats = nullptr; }
         return OAT_OK;
     }
-    if (!strcmp(key, "backproject")) { if (variant != 0 && variant != 4 && variant != 5) return fail(OAT_ERR_INVALID, "unknown backproject variant %d (0 generic, 4 marching, 5 tile-stationary)", variant); g->variant_backproject = variant; return OAT_OK; }
-    if (!strcmp(key, "tile_nq_bwd")) { if (variant < 1 || variant > 4096) return fail(OAT_ERR_INVALID, "tile_nq_bwd must be in 1..4096"); g->tile_nq_bwd = variant; return OAT_OK; }
+    if (!strcmp(key, "backproject")) {
+        // variant 5 (tile-stationary H^T, int32 fixed-point accumulators in shared memory) was measured in round 2 and removed:
+        // 2.05x slower and 8e-5 .. 5.7e-4 from the oracle, with no overflow guard.  A handle cannot be switched onto it.
+        if (variant == 5) return fail(OAT_ERR_INVALID, "backproject variant 5 (tile-stationary H^T) is not part of the library: it missed the 1e-4 tolerance (profiles/r2_tile_bwd.md)");
+        if (variant != 0 && variant != 4) return fail(OAT_ERR_INVALID, "unknown backproject variant %d (0 generic, 4 marching)", variant);
+        g->variant_backproject = variant; return OAT_OK;
+    }
     if (!strcmp(key, "morton_shift")) {
         if (variant < 0 || variant > 10) return fail(OAT_ERR_INVALID, "morton_shift out of range");
         if (g->morton_shift != variant) { cudaFree(g->d_patches); g->d_patches = nullptr; g->dev.patches = nullptr; g->dev.n_patches = 0; }

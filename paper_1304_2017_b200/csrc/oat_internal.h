@@ -63,8 +63,6 @@ struct OatDev {
     long long n_patches;
     const double2 *dir;                  // direction table (marching kernels): (sin th cos phi, sin th sin phi) of ring r,
                                          // azimuth j of band b at band.dir_ofs + ring.cum + j, fp64 (S2, S3)
-    float omega_max;                     // largest solid-angle weight of any ring (H^T tile kernel: fixed-point scale)
-    double samples_per_cell;             // (spacing / h)^2 spacing / (c dt): quadrature samples per cell and transducer
     long long max_band_dirs;             // largest number of table directions of one band (the tile kernels pack it into 27 bits)
     const int *q_count;                  // patches per transducer
     int *q_done;                         // patches finished in the running projection (zeroed per call)
@@ -98,13 +96,11 @@ void oat_launch_unface(const OatDev &P, const float4 *faces, float *x, cudaStrea
 // mode 1 scatters coef[q,k] = g'_k rho_k^2 into the face-quad accumulators
 cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, float4 *faces, float *y_out,
                              const float *coef, double *g, cudaStream_t st);
-// tile-stationary kernels (oat_tile.cu): a block keeps a brick of the volume in shared memory (TMA box load) and evaluates every
+// tile-stationary projection kernel (oat_tile.cu): a block keeps a brick of the volume in shared memory (TMA box load) and evaluates every
 // sample that falls into it; needs B = 32, the direction table and 7 c dt < 3 spacing
 bool oat_tile_supported(const OatDev &P);
 cudaError_t oat_launch_tile_fwd(const OatDev &P, const float *x, double *g, float *y, unsigned long long *counter,
                                 unsigned long long *stats, int nq_per_item, int allow_tma, cudaStream_t st);
-cudaError_t oat_launch_tile_bwd(const OatDev &P, const float *coef, float *coef_max, float *x, unsigned long long *counter,
-                                int nq_per_item, cudaStream_t st);
 void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream_t st);
 // coef[q,k] = kappa (y[k-1] - y[k+1]) / (2 dt t_k) * rho_k^2   (Eq. 22 L172 with the rho^2 of S8; 0 where t_k <= 0)
 void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st);

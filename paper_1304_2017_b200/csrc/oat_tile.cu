@@ -48,9 +48,6 @@ namespace {
 #define TT_BZ 12                       // 12 planes per round
 #define TT_STAGE_BYTES (TT_BX * TT_BY * TT_BZ * 4)
 #define TT_QUEUE_BYTES (TT_WARPS * TT_QN * 32)
-#define TT_NN (TT_R + 1)                // H^T: 23 nodes per axis of the brick, int32 accumulators with pitches 23 and 529 (both odd)
-#define TT_NPY TT_NN
-#define TT_NPZ (TT_NN * TT_NN)
 static_assert(TT_C % 4 == 0 && (2 * TT_M + 2) % 4 == 0 && TT_R + 2 <= TT_BX, "the staged box must start on a multiple of 4 nodes in x");
 
 struct TileParams {
@@ -58,7 +55,6 @@ struct TileParams {
     int n_qc, nq;                      // transducer ranges per tile, transducers per range
     long long n_items;
     int use_tma;
-    float fix_num;                     // H^T: fixed-point scale = fix_num / max|coef| (2^30 / (transducers per item x samples per node x max omega))
 };
 
 struct SmemLayout {
@@ -70,7 +66,6 @@ struct SmemLayout {
     unsigned char qc[TT_WARPS][TT_QN];
     unsigned cq[TT_WARPS][TT_QN];      // candidate queue: ring slot << 27 | index into the band's direction table
     double frame[TT_WARPS][16];        // e_x, e_y, e_z, base', then the band's s_mid, s_lo, s_hi
-    float coef[TT_WARPS][32];          // H^T: the band's coefficients g'_k rho_k^2 (step B1)
     float framef[TT_WARPS][12];
     unsigned long long mbar;
     long long item;
@@ -218,56 +213,6 @@ __device__ __forceinline__ void march_group_fwd(const float4 *qa, const float4 *
 }
 
 // ------------------------------------------------------------------------------------------------
-// H^T: march one group of <= 32 queued chunks and ADD the 8 corner weights of every sample into the brick's node accumulators
-// in shared memory.  fp32 shared atomics are compare-and-swap loops on sm_100a (ATOMS.CAST.SPIN), only the 32-bit integer add
-// is native (ATOMS.ADD), so the accumulators are fixed point: a weight is scaled by `oms` = omega x scale, rounded to an
-// integer by the add of 1.5 * 2^23, and added with one ATOMS.ADD per corner (8 per sample, addresses = base + immediates).
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void atoms_add(unsigned addr, int v)
-{
-    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
-}
-
-__device__ __forceinline__ void march_group_bwd(const float4 *qa, const float4 *qs, const unsigned char *qc, int &head, int &cnt,
-                                                const float *s_coef, int lane, unsigned node_base, float scale)
-{
-    const int n = min(cnt, 32);
-    const int slot = (head + lane) & (TT_QN - 1);
-    float4 ea = make_float4(0.f, 0.f, 0.f, 0.f);
-    float4 es = make_float4(0.f, 0.f, 0.f, __uint_as_float(node_base - 4u * OAT_MAGIC_BITS * (1u + TT_NPY + TT_NPZ)));   // idle lane: node 0, weight 0
-    int cc = 0;
-    if (lane < n) { ea = qa[slot]; es = qs[slot]; cc = qc[slot]; }
-    __syncwarp();
-    head = (head + n) & (TT_QN - 1);
-    cnt -= n;
-    const unsigned Kr = __float_as_uint(es.w);
-    const float kk0 = 8.f * (float)cc - 15.5f;
-    const float oms = ea.w * scale;
-    const float *cf = s_coef + 8 * cc;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const float kk = kk0 + (float)i;
-        const float tx = fmaf(es.x, kk, ea.x), ty = fmaf(es.y, kk, ea.y), tz = fmaf(es.z, kk, ea.z);
-        const float rx = __fadd_rd(tx, OAT_MAGIC), ry = __fadd_rd(ty, OAT_MAGIC), rz = __fadd_rd(tz, OAT_MAGIC);
-        const unsigned adr = __float_as_uint(rz) * (4u * TT_NPZ) + (__float_as_uint(ry) * (4u * TT_NPY) + (__float_as_uint(rx) * 4u + Kr));
-        const float fx = tx - (rx - OAT_MAGIC), fy = ty - (ry - OAT_MAGIC), fz = tz - (rz - OAT_MAGIC);
-        const float cw = cf[i] * oms;
-        const float ex = 1.f - fx, ey = 1.f - fy;
-        const float w0 = cw - cw * fz, w1 = cw * fz;                                  // planes z, z + 1
-        const float a00 = w0 * ey, a01 = w0 * fy, a10 = w1 * ey, a11 = w1 * fy;      // [plane][row]
-        // round(a * e) as the low mantissa bits of a * e + 1.5 * 2^23 (|.| < 2^22 by the choice of the scale)
-        atoms_add(adr,                                  (int)(__float_as_uint(fmaf(a00, ex, OAT_MAGIC)) - OAT_MAGIC_BITS));
-        atoms_add(adr + 4u,                             (int)(__float_as_uint(fmaf(a00, fx, OAT_MAGIC)) - OAT_MAGIC_BITS));
-        atoms_add(adr + 4u * TT_NPY,                    (int)(__float_as_uint(fmaf(a01, ex, OAT_MAGIC)) - OAT_MAGIC_BITS));
-        atoms_add(adr + 4u * TT_NPY + 4u,               (int)(__float_as_uint(fmaf(a01, fx, OAT_MAGIC)) - OAT_MAGIC_BITS));
-        atoms_add(adr + 4u * TT_NPZ,                    (int)(__float_as_uint(fmaf(a10, ex, OAT_MAGIC)) - OAT_MAGIC_BITS));
-        atoms_add(adr + 4u * TT_NPZ + 4u,               (int)(__float_as_uint(fmaf(a10, fx, OAT_MAGIC)) - OAT_MAGIC_BITS));
-        atoms_add(adr + 4u * (TT_NPZ + TT_NPY),         (int)(__float_as_uint(fmaf(a11, ex, OAT_MAGIC)) - OAT_MAGIC_BITS));
-        atoms_add(adr + 4u * (TT_NPZ + TT_NPY) + 4u,    (int)(__float_as_uint(fmaf(a11, fx, OAT_MAGIC)) - OAT_MAGIC_BITS));
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
 // brick load: raw nodes by TMA (or plain loads when the volume's row pitch / address does not fit a tensor map), two rounds of
 // 12 node planes through the staging buffer, bilinear plane records into `rec`
 // ------------------------------------------------------------------------------------------------
@@ -330,12 +275,13 @@ __device__ __forceinline__ void clip_arc(float &xl, float &xh, float c0, float a
     xl = nl; xh = nh;
 }
 
-// MODE 0: H (x -> g; records from the brick).  MODE 1: H^T (coef -> xout; node accumulators in the brick, flushed per item).
-template <int MODE, bool STATS>
+// H: x -> g, records from the brick.  (A tile-stationary H^T on the same enumeration, with fixed-point node accumulators in
+// shared memory, was measured in round 2 -- profiles/r2_tile_bwd.md, DESIGN.md 5.9 -- and is no longer part of the library:
+// 2.05x slower than the marching H^T and outside the 1e-4 product tolerance.)
+template <bool STATS>
 __global__ void __launch_bounds__(TT_THREADS, 1)
 oat_tile_kernel(const __grid_constant__ CUtensorMap tmap, const OatDev P, const TileParams T, const float *__restrict__ x,
-                double *__restrict__ g, unsigned long long *__restrict__ counter, unsigned long long *__restrict__ stats,
-                const float *__restrict__ coef, const float *__restrict__ coef_max, float *__restrict__ xout)
+                double *__restrict__ g, unsigned long long *__restrict__ counter, unsigned long long *__restrict__ stats)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     SmemLayout &S = *reinterpret_cast<SmemLayout *>(smem_raw);
@@ -349,11 +295,7 @@ oat_tile_kernel(const __grid_constant__ CUtensorMap tmap, const OatDev P, const 
     unsigned *const cq = S.cq[warp];
     double *const s_frame = S.frame[warp];
     float *const s_ff = S.framef[warp];
-    const unsigned rec_base = smem_u32(S.rec);       // MODE 1: the node accumulators (int32) live in the same memory
-    int *const nodes = reinterpret_cast<int *>(S.rec);
-    float *const s_coef = S.coef[warp];
-    float scale = 0.f;
-    if (MODE == 1) { const float cm = coef_max[0]; if (!(cm > 0.f)) return; scale = T.fix_num / cm; }   // all data zero: x stays zero
+    const unsigned rec_base = smem_u32(S.rec);
     unsigned phase = 0;
     long long cur_tile = -1;
     unsigned st_cand = 0, st_pre = 0, st_ray = 0, st_chunk = 0;         // STATS: candidates, after the fp32 cull, rays / chunks owned
@@ -371,11 +313,7 @@ oat_tile_kernel(const __grid_constant__ CUtensorMap tmap, const OatDev P, const 
         const int tz = (int)(tile / ((long long)T.ntx * T.nty)), ty = (int)((tile / T.ntx) % T.nty), tx = (int)(tile % T.ntx);
         const int clo[3] = {-TT_M + TT_C * tx, -TT_M + TT_C * ty, -TT_M + TT_C * tz};
         const int rlo[3] = {clo[0] - TT_M, clo[1] - TT_M, clo[2] - TT_M};
-        if (MODE == 0) {
-            if (tile != cur_tile) { load_brick(S, P, &tmap, x, T.use_tma, rlo, phase, tid); cur_tile = tile; }
-        } else {
-            for (int i = tid; i < TT_NN * TT_NPZ; i += TT_THREADS) nodes[i] = 0;
-        }
+        if (tile != cur_tile) { load_brick(S, P, &tmap, x, T.use_tma, rlo, phase, tid); cur_tile = tile; }
         if (tid == 0) S.nextq = 0;
         __syncthreads();
         const int q_begin = qc_i * T.nq, q_end = min(P.Q, q_begin + T.nq);
@@ -415,13 +353,6 @@ oat_tile_kernel(const __grid_constant__ CUtensorMap tmap, const OatDev P, const 
                 __syncwarp();
                 const OatRing *__restrict__ ring = P.ring + band.ring_ofs;
                 const double2 *__restrict__ dir = P.dir + band.dir_ofs;
-                if (MODE == 1) {                           // B1: the band's 32 coefficients; a band of zeros contributes exactly nothing
-                    const float cfv = lane < band.nk ? coef[(size_t)q * P.K + band.k0 + lane] : 0.f;
-                    if (!__any_sync(0xffffffffu, cfv != 0.f)) continue;
-                    __syncwarp();
-                    s_coef[lane] = cfv;
-                    __syncwarp();
-                }
                 // ---- window of rings and azimuths that covers the core's projection: 27 lattice points of the core
                 float th, ph, rp;
                 {
@@ -473,8 +404,7 @@ oat_tile_kernel(const __grid_constant__ CUtensorMap tmap, const OatDev P, const 
 #pragma unroll 1
                 for (;;) {
                     if (cnt >= 32 || (all_done && cnt > 0)) {
-                        if (MODE == 0) march_group_fwd(qa, qs, qc, head, cnt, acc, lane, rec_base);
-                        else march_group_bwd(qa, qs, qc, head, cnt, s_coef, lane, rec_base, scale);
+                        march_group_fwd(qa, qs, qc, head, cnt, acc, lane, rec_base);
                         continue;
                     }
                     if (all_done) break;
@@ -521,12 +451,8 @@ oat_tile_kernel(const __grid_constant__ CUtensorMap tmap, const OatDev P, const 
                             }
                         }
                         if (STATS) { st_ray += own ? 1 : 0; st_chunk += __popc(own); }
-                        if (MODE == 0)
-                            Kc = rec_base + 16u * (((unsigned)(e.ix - rlo[0]) - OAT_MAGIC_BITS) + (unsigned)TT_PY * ((unsigned)(e.iy - rlo[1]) - OAT_MAGIC_BITS)
-                                                   + (unsigned)TT_PZ * ((unsigned)(e.iz - rlo[2]) - OAT_MAGIC_BITS));
-                        else                               // node (lx, ly, lz) of the brick = lower corner of cell (lx, ly, lz)
-                            Kc = rec_base + 4u * (((unsigned)(e.ix - rlo[0]) - OAT_MAGIC_BITS) + (unsigned)TT_NPY * ((unsigned)(e.iy - rlo[1]) - OAT_MAGIC_BITS)
-                                                  + (unsigned)TT_NPZ * ((unsigned)(e.iz - rlo[2]) - OAT_MAGIC_BITS));
+                        Kc = rec_base + 16u * (((unsigned)(e.ix - rlo[0]) - OAT_MAGIC_BITS) + (unsigned)TT_PY * ((unsigned)(e.iy - rlo[1]) - OAT_MAGIC_BITS)
+                                               + (unsigned)TT_PZ * ((unsigned)(e.iz - rlo[2]) - OAT_MAGIC_BITS));
                         if (__any_sync(0xffffffffu, own != 0u)) pend = 0;
                         continue;
                     }
@@ -614,7 +540,6 @@ oat_tile_kernel(const __grid_constant__ CUtensorMap tmap, const OatDev P, const 
                     n_rows = nmax == 0 ? 0 : ((nb + (32 >> wsh) - 1) >> (5 - wsh)) * nseg;
                     row = 0;
                 }
-                if (MODE == 1) continue;
                 // S5: sum the accumulators over the lanes (lane l collects sample l of the band), one fp64 atomic per time sample
                 float accK = 0.f;
 #pragma unroll
@@ -625,21 +550,6 @@ oat_tile_kernel(const __grid_constant__ CUtensorMap tmap, const OatDev P, const 
                 const int k = band.k0 + lane;
                 const double rho = P.c * (P.t0 + (double)k * P.dt);
                 if (lane < band.nk && rho > 0.0 && accK != 0.f) atomicAdd(&g[(size_t)q * P.K + k], rho * rho * (double)accK);
-            }
-        }
-        if (MODE == 1) {
-            // flush: every accumulated node of the brick that exists in the grid goes to x with one fp32 reduction (B3)
-            __syncthreads();
-            const float inv = 1.f / scale;
-            for (int c = tid; c < TT_NPZ; c += TT_THREADS) {
-                const int ly = c / TT_NN, lx = c - ly * TT_NN;
-                const int X = rlo[0] - 1 + lx, Y = rlo[1] - 1 + ly;
-                if (X < 0 || X >= P.nx || Y < 0 || Y >= P.ny) continue;
-                for (int lz = 0; lz < TT_NN; ++lz) {
-                    const int Z = rlo[2] - 1 + lz;
-                    const int v = nodes[lz * TT_NPZ + c];
-                    if (v != 0 && Z >= 0 && Z < P.nz) atomicAdd(&xout[((size_t)Z * P.ny + Y) * P.nx + X], (float)v * inv);
-                }
             }
         }
         // all warps meet at the barrier at the top of the loop before the brick or the staging buffer is touched again
@@ -661,19 +571,6 @@ __global__ void oat_tile_diff_kernel(const OatDev P, const double *__restrict__ 
         if (k - 1 >= 0) { const double t = P.t0 + (double)(k - 1) * P.dt; if (t > 0.0) sm = g[i - 1] / t; }
         y[i] = (float)(P.kappa * (sp - sm) / (2.0 * P.dt));
     }
-}
-
-// max |v| of a vector: non-negative floats order like their bit patterns (H^T: the fixed-point scale needs max |coef|)
-__global__ void oat_absmax_kernel(const float *__restrict__ v, long long n, unsigned *__restrict__ out)
-{
-    unsigned m = 0u;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const float a = fabsf(v[i]);
-        if (a == a && a < 3.0e38f) m = max(m, __float_as_uint(a));                 // NaN / inf are left out of the scale
-    }
-#pragma unroll
-    for (int s = 16; s >= 1; s >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, s));
-    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -729,9 +626,9 @@ cudaError_t oat_launch_tile_fwd(const OatDev &P, const float *x, double *g, floa
     cudaGetDevice(&dev);
     const int smem = (int)sizeof(SmemLayout);
     if (dev < 0 || dev >= 64 || !attr_set[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(oat_tile_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(oat_tile_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(oat_tile_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        e = cudaFuncSetAttribute(oat_tile_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
@@ -740,60 +637,13 @@ cudaError_t oat_launch_tile_fwd(const OatDev &P, const float *x, double *g, floa
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     const long long grid = T.n_items < n_sm ? T.n_items : n_sm;
-    if (stats) oat_tile_kernel<0, true><<<(unsigned)grid, TT_THREADS, smem, st>>>(map, P, T, x, g, counter, stats, nullptr, nullptr, nullptr);
-    else oat_tile_kernel<0, false><<<(unsigned)grid, TT_THREADS, smem, st>>>(map, P, T, x, g, counter, stats, nullptr, nullptr, nullptr);
+    if (stats) oat_tile_kernel<true><<<(unsigned)grid, TT_THREADS, smem, st>>>(map, P, T, x, g, counter, stats);
+    else oat_tile_kernel<false><<<(unsigned)grid, TT_THREADS, smem, st>>>(map, P, T, x, g, counter, stats);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     const long long n = (long long)P.Q * P.K;
     long long gsz = (n + 255) / 256;
     if (gsz > 148LL * 16) gsz = 148LL * 16;
     oat_tile_diff_kernel<<<(unsigned)gsz, 256, 0, st>>>(P, g, y);
-    return cudaGetLastError();
-}
-
-// H^T by the tile-stationary kernel: x is zeroed, every (tile, transducer range) item accumulates its samples into the brick's
-// fixed-point node accumulators in shared memory and adds them to x with one fp32 reduction per touched node.
-cudaError_t oat_launch_tile_bwd(const OatDev &P, const float *coef, float *coef_max, float *x, unsigned long long *counter,
-                                int nq_per_item, cudaStream_t st)
-{
-    TileParams T;
-    T.ntx = (P.nx + 1 + 2 * TT_M + TT_C - 1) / TT_C;
-    T.nty = (P.ny + 1 + 2 * TT_M + TT_C - 1) / TT_C;
-    T.ntz = (P.nz + 1 + 2 * TT_M + TT_C - 1) / TT_C;
-    T.nq = nq_per_item > 0 ? nq_per_item : 16;
-    T.n_qc = (P.Q + T.nq - 1) / T.nq;
-    T.n_items = (long long)T.ntx * T.nty * T.ntz * T.n_qc;
-    T.use_tma = 0;
-    // Fixed-point scale.  The weights a node receives from one transducer sum to about samples_per_cell = 1 / (h^2 c dt) in voxel
-    // units (the hat function integrates to one cell); closed rings and the band rule (rho_ref / rho)^2 raise the density by a few
-    // per cent.  |sum of one node over an item| <= transducers x 4 ceil(samples_per_cell) x max |coef| omega is taken as < 2^30; a
-    // single sample's weight then stays far below 2^22, which the rounding add needs.
-    T.fix_num = (float)(1073741824.0 / ((double)T.nq * 4.0 * ceil(P.samples_per_cell) * (double)P.omega_max));
-    T.fix_num = fminf(T.fix_num, (float)(4194000.0 / (double)P.omega_max));      // one weight < 2^22 whatever the item size
-    CUtensorMap map;
-    memset(&map, 0, sizeof(map));
-    static bool attr_set[64] = {false};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    const int smem = (int)sizeof(SmemLayout);
-    if (dev < 0 || dev >= 64 || !attr_set[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(oat_tile_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) attr_set[dev] = true;
-    }
-    int n_sm = 148;
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(coef_max, 0, sizeof(float), st);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(x, 0, sizeof(float) * (size_t)P.nx * P.ny * P.nz, st);
-    if (e != cudaSuccess) return e;
-    const long long n = (long long)P.Q * P.K;
-    long long gsz = (n + 255) / 256;
-    if (gsz > 148LL * 16) gsz = 148LL * 16;
-    oat_absmax_kernel<<<(unsigned)gsz, 256, 0, st>>>(coef, n, reinterpret_cast<unsigned *>(coef_max));
-    const long long grid = T.n_items < n_sm ? T.n_items : n_sm;
-    oat_tile_kernel<1, false><<<(unsigned)grid, TT_THREADS, smem, st>>>(map, P, T, nullptr, nullptr, counter, nullptr, coef, coef_max, x);
     return cudaGetLastError();
 }
