@@ -763,13 +763,14 @@ static int pls_cg_impl(oat_geometry *g, const float *d_u, float *d_x, int n_iter
     auto fwd = [&](const float *x, float *u) -> int {
         if (!sph) return project_full(g, x, u, st);
         CUDA_TRY(cudaMemsetAsync(u, 0, sizeof(float) * n_dat, st));
-        oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m, x, g->d_p0, u, st);
+        CUDA_TRY(oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m, x, g->d_p0, u, st));
         return OAT_OK;
     };
     auto bwd = [&](const float *u, float *x) -> int {
         if (!sph) return backproject_full(g, u, x, st);
         oat_launch_sph_bwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m,
                            reinterpret_cast<const float2 *>(u), g->d_p0, g->d_sv, x, st);
+        CUDA_TRY(cudaGetLastError());                      // a bad launch surfaces here, not after the whole loop has been enqueued
         return OAT_OK;
     };
     CgCurves cv;
@@ -875,8 +876,7 @@ int oat_sph_project(oat_geometry *g, const float *d_x, float *d_u, void *stream)
     if (!d_x || (!d_u && g->dev.Q)) return fail(OAT_ERR_INVALID, "d_x / d_u must not be NULL");
     cudaStream_t st = (cudaStream_t)stream;
     if (g->dev.Q > 0) CUDA_TRY(cudaMemsetAsync(d_u, 0, sizeof(float2) * (size_t)g->sph_nf * (size_t)g->dev.Q, st));
-    oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m, d_x, g->d_p0, d_u, st);
-    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(oat_launch_sph_fwd(g->dev, g->sph_nf, g->sph_f0, g->sph_df, g->desc.spacing, g->desc.c, g->sph_aperture, g->sph_m, d_x, g->d_p0, d_u, st));
     return OAT_OK;
 }
 

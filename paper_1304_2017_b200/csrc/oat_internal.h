@@ -121,5 +121,5 @@ void oat_launch_penalty(const OatDev &P, const float *x, float *out, float alpha
 void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, cudaStream_t st);
 // row NEXT-3: spherical-voxel model (Eq. 17-19, 24); point-like transducers or square apertures of side `aperture` (mm)
 // integrated with m x m sub-elements (Eq. 18, reading G30); u, v: Q x nf complex (float2), p0: nf complex
-void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float *x, const float2 *p0, float *u, cudaStream_t st);
+cudaError_t oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float *x, const float2 *p0, float *u, cudaStream_t st);
 void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st);

@@ -35,7 +35,7 @@ oat_eir_kernel(const float *__restrict__ in, float *__restrict__ out, const floa
     extern __shared__ __align__(16) float sm[];
     float *s_h = sm, *s_w = sm + Lp;                       // taps h'[0, Lp), window [0, T + Lp + 8)
     constexpr int T = OAT_ET * OAT_ER;
-    const int q = blockIdx.y, k0 = blockIdx.x * T, t = threadIdx.x;
+    const int q = blockIdx.x, k0 = blockIdx.y * T, t = threadIdx.x;      // transducers on grid.x (no 65535 limit on Q)
     const float *row = in + (size_t)q * K;
     for (int m = t; m < Lp; m += OAT_ET) {
         const int src = ADJ ? m : Lp - 1 - m;
@@ -167,12 +167,12 @@ oat_sph_fwd_kernel(const OatDev P, const OatSph S, const float *__restrict__ x, 
 {
     __shared__ float s_x[OAT_SV];
     const long long n_vox = (long long)P.nx * P.ny * P.nz;
-    const long long v0 = (long long)blockIdx.y * OAT_SV;
+    const long long v0 = (long long)blockIdx.x * OAT_SV;                 // voxel chunks on grid.x: up to 2^31 - 1 of them (the handle allows 2^40 voxels)
     const int nv = (int)min((long long)OAT_SV, n_vox - v0);
     int any = 0;
     for (int i = threadIdx.x; i < nv; i += blockDim.x) { const float v = x[v0 + i]; s_x[i] = v; any |= (v != 0.f); }
     if (!__syncthreads_or(any)) return;                    // an all-zero chunk contributes nothing
-    const long long wi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long wi = (long long)blockIdx.y * blockDim.x + threadIdx.x;
     if (wi >= (long long)P.Q * S.n_lg) return;
     const int q = (int)(wi / S.n_lg), lg = (int)(wi % S.n_lg);
     const int l0 = lg * OAT_SG;
@@ -329,7 +329,8 @@ cudaError_t oat_launch_eir(int adjoint, const float *in, float *out, const float
     cudaError_t e = cudaFuncSetAttribute(oat_eir_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(oat_eir_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const dim3 grid((unsigned)((K + T - 1) / T), (unsigned)Q);
+    const dim3 grid((unsigned)Q, (unsigned)((K + T - 1) / T));            // grid.y <= 65535 holds for K < 1.3e8 (K is an int32 count of 2048-sample chunks)
+    if (grid.y > 65535u) return cudaErrorInvalidValue;
     if (adjoint) oat_eir_kernel<1><<<grid, OAT_ET, smem, st>>>(in, out, he, L, Lp, K);
     else oat_eir_kernel<0><<<grid, OAT_ET, smem, st>>>(in, out, he, L, Lp, K);
     return cudaGetLastError();
@@ -341,14 +342,17 @@ void oat_launch_fbp(const OatDev &P, const float *p, const float *wq, float *x, 
     oat_fbp_kernel<<<grid, 256, 0, st>>>(P, p, wq, x);
 }
 
-void oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float *x, const float2 *p0, float *u, cudaStream_t st)
+cudaError_t oat_launch_sph_fwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float *x, const float2 *p0, float *u, cudaStream_t st)
 {
     OatSph S; S.nf = nf; S.n_lg = (nf + OAT_SG - 1) / OAT_SG; S.f0 = f0; S.df = df; S.ds = ds; S.ds_over_c = ds / c;
     S.m = (aperture > 0.0 && m > 1) ? m : 1; S.a_nodes = S.m > 1 ? aperture / ds : 0.0;
     const long long n_vox = (long long)P.nx * P.ny * P.nz, work = (long long)P.Q * S.n_lg;
-    if (n_vox <= 0 || work <= 0) return;
-    const dim3 grid((unsigned)((work + 127) / 128), (unsigned)((n_vox + OAT_SV - 1) / OAT_SV));
+    if (n_vox <= 0 || work <= 0) return cudaSuccess;
+    const long long gx = (n_vox + OAT_SV - 1) / OAT_SV, gy = (work + 127) / 128;
+    if (gx > 2147483647LL || gy > 65535LL) return cudaErrorInvalidValue;          // > 8.4e6 (transducer, frequency group) pairs
+    const dim3 grid((unsigned)gx, (unsigned)gy);
     oat_sph_fwd_kernel<<<grid, 128, 0, st>>>(P, S, x, p0, u);
+    return cudaGetLastError();
 }
 
 void oat_launch_sph_bwd(const OatDev &P, int nf, double f0, double df, double ds, double c, double aperture, int m, const float2 *u, const float2 *p0, float2 *v, float *x, cudaStream_t st)

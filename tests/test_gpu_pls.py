@@ -32,9 +32,10 @@ def eir_taps(n, dt, seed=0):
     return (dt * np.exp(-t / (0.15 * n * dt)) * np.sin(2 * np.pi * 2.5 * t + 0.3 * seed)).astype(np.float32)
 
 
-@pytest.mark.parametrize("K,L,Q", [(300, 37, 5), (256, 256, 3), (1000, 300, 2), (40, 64, 4), (513, 1, 2)])
+@pytest.mark.parametrize("K,L,Q", [(300, 37, 5), (256, 256, 3), (1000, 300, 2), (40, 64, 4), (513, 1, 2), (40, 5, 70000)])
 def test_eir_forward_and_adjoint_match_the_oracle(env, K, L, Q):
-    """Eq. (14) / Eq. (21) on ragged tiles (K not a multiple of the 256-output tile), L > K, L = 1."""
+    """Eq. (14) / Eq. (21) on ragged tiles (K not a multiple of the 256-output tile), L > K, L = 1, and more transducers
+    than a grid's y dimension can hold (Q = 70 000 > 65 535: the rows are on grid.x)."""
     torch, orc, pls, oat, wl = env
     w = wl.small(n=8, q=Q, nt=K, kband=32)
     rng = np.random.default_rng(K + L)
