@@ -8,7 +8,9 @@ complete transducer set on the GPU), checked on sampled outputs the oracle can c
         (b) DENSE: y ~ N(0,1) in every row.  By linearity H^T y - H^T (y with the subset's rows zeroed) is the subset's
         contribution; both terms are dense full-size launches (no skipped band, every reduction contended), and their
         difference is compared with the oracle's H^T of the subset's rows.  The difference carries the rounding of the
-        two dense sums (~ sqrt(Q / n_sub) x 3e-7 ~ 1e-5), still inside the tolerance.
+        two dense sums (~ sqrt(Q / n_sub) x 3e-7 ~ 1e-5), still inside the tolerance;
+        (c) the adjoint identity with dense y and a dense x ~ U(0,1) (H of that x checked on the sampled rows), so that
+        H^T y is weighed on every voxel.
 Tolerance: rel-L2 <= 1e-4 (north_star).
 """
 import numpy as np
@@ -60,7 +62,17 @@ def test_fullsize_sampled_rows(cfg, nsub):
     e_td = rel_l2((x_all - x_rest).cpu().numpy(), ref_xb)
     # adjoint identity at full size with dense y (a property that holds at any size)
     lhs, rhs, rel = oat.oat_adjoint_check(g, xd, ydense)
+    # (c) the same identity with a DENSE x ~ U(0,1): <H x, y> = <x, H^T y> then weighs H^T y on EVERY voxel, not only on the
+    # 0.7 % the vessel phantom touches -- an error of the dense H^T anywhere in the volume, including one that (b)'s
+    # difference of two launches would cancel, breaks it.  Its left side is anchored by the oracle: H of the dense x on the
+    # sampled rows.
+    xdense = rng.random(x.shape, dtype=np.float32)
+    xdd = torch.from_numpy(xdense).cuda()
+    yd_rows = oat.oat_project(g, xdd)[didx].cpu().numpy()
+    e_hd = rel_l2(yd_rows, orc.project(ws, xdense.astype(np.float64)))
+    lhs_d, rhs_d, rel_d = oat.oat_adjoint_check(g, xdd, ydense)
     print(f"config {cfg}: H rows[{nsub}] {e_h:.2e}, H^T sparse {e_t:.2e}, H^T dense-by-linearity {e_td:.2e}, adjoint {rel:.2e}, "
-          f"samples/op {oat.oat_num_surface_samples(g):.4g}")
+          f"dense x: H rows {e_hd:.2e}, adjoint {rel_d:.2e}, samples/op {oat.oat_num_surface_samples(g):.4g}")
     g.close()
     assert e_h <= TOL and e_t <= TOL and e_td <= TOL and rel <= TOL
+    assert e_hd <= TOL and rel_d <= TOL
