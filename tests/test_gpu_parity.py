@@ -352,3 +352,33 @@ def test_generic_kernel_on_config1(env):
     assert rel_l2(gpu_project(torch, oat, w, x, g), orc.project(w, x.astype(np.float64))) <= TOL
     assert rel_l2(gpu_backproject(torch, oat, w, y, g), orc.backproject(w, y.astype(np.float64))) <= TOL
     g.close()
+
+
+@pytest.mark.parametrize("variant", [4, 0, 5])
+def test_repeated_launches_agree(env, variant):
+    """Race check that needs no tool (compute-sanitizer is closed on the GPU pool, profiles/r3_sanitizer.md): the same
+    operator launched five times on the same input, with other work on the device in between, must give the same result
+    up to the order of its atomic additions (fp64 atomics then one rounding for H, fp32 reductions for H^T).  A lost
+    update, a queue slot read before it is written or an epilogue that runs before the last patch has landed shows up as
+    a difference orders of magnitude above that.  Variants: 4 marching kernels, 0 generic patch kernel, 5 tile-stationary
+    projection (TMA + mbarrier staging; H only)."""
+    torch, orc, oat, wl = env
+    w = wl.config(1)
+    x = torch.from_numpy(w.phantom()).cuda()
+    y = torch.from_numpy(w.data_noise()).cuda()
+    g = oat.oat_geometry_create(w)
+    oat.oat_set_variant(g, "project", variant)
+    if variant != 5:
+        oat.oat_set_variant(g, "backproject", variant)
+    busy = torch.empty(64 << 20, dtype=torch.uint8, device="cuda")
+    hx, hty = [], []
+    for i in range(5):
+        hx.append(oat.oat_project(g, x).double().clone())
+        busy.fill_(i)                                    # evicts L2, changes what is resident next to the kernels
+        hty.append(oat.oat_backproject(g, y).double().clone())
+    torch.cuda.synchronize()
+    g.close()
+    for a in hx[1:]:
+        assert float((a - hx[0]).norm() / hx[0].norm()) <= 1e-6
+    for a in hty[1:]:
+        assert float((a - hty[0]).norm() / hty[0].norm()) <= 2e-6
