@@ -58,7 +58,6 @@ struct oat_geometry {
     // scratch
     float *d_xpad = nullptr;                  // padded volume (generic kernel: gather source / scatter target; lazy)
     double2 *d_dir = nullptr;                 // direction table of the marching kernels
-    float *d_coef = nullptr;                  // Q*K adjoint coefficients g'_k rho_k^2 (marching H^T, lazy)
     float4 *d_faces = nullptr;                // face-quad accumulators of the 3 orientations (marching H^T, lazy)
     size_t n_faces = 0;                       // float4 records, 0 = marching H^T unavailable for this grid
     float4 *d_cells = nullptr;                // per-cell polynomial records (marching H, lazy)
@@ -101,7 +100,7 @@ void free_all(oat_geometry *g)
     cudaFree(g->d_xpad); cudaFree(g->d_g); cudaFree(g->d_y2);
     cudaFree(g->d_x2); cudaFree(g->d_x3); cudaFree(g->d_y3); cudaFree(g->d_x4); cudaFree(g->d_scal);
     cudaFree(g->d_y4); cudaFree(g->d_he); cudaFree(g->d_p0); cudaFree(g->d_sv); cudaFree(g->d_sd); cudaFree(g->d_sq);
-    cudaFree(g->d_counter); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_coef); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done); cudaFree(g->d_tile_stats);
+    cudaFree(g->d_counter); cudaFree(g->d_cells); cudaFree(g->d_faces); cudaFree(g->d_dir); cudaFree(g->d_rb_sectors); cudaFree(g->d_patches); cudaFree(g->d_q_count); cudaFree(g->d_q_done); cudaFree(g->d_tile_stats);
     if (g->h_scal) cudaFreeHost(g->h_scal);
     if (g->ev0) cudaEventDestroy(g->ev0);
     if (g->ev1) cudaEventDestroy(g->ev1);
@@ -431,8 +430,6 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
     if (march) {
         if (!G->d_faces) CUDA_TRY(cudaMalloc((void **)&G->d_faces, sizeof(float4) * G->n_faces));
         CUDA_TRY(cudaMemsetAsync(G->d_faces, 0, sizeof(float4) * G->n_faces, st));
-        if ((rc = ensure(&G->d_coef, G->n_dat))) return rc;
-        oat_launch_coef(P, d_y, G->d_coef, st); ++G->last_launches;
     } else {
         if ((rc = ensure_xpad(G))) return rc;
         CUDA_TRY(cudaMemsetAsync(G->d_xpad, 0, sizeof(float) * G->n_pad, st));
@@ -441,7 +438,7 @@ int backproject_impl(oat_geometry *G, const float *d_y, float *d_x, cudaStream_t
     bool launched;
     if (march) {
         launched = G->dev.n_patches > 0;
-        CUDA_TRY(oat_launch_march(1, G->dev, nullptr, G->d_faces, nullptr, G->d_coef, nullptr, st));
+        CUDA_TRY(oat_launch_march(1, G->dev, nullptr, G->d_faces, nullptr, d_y, nullptr, st));
     } else if ((rc = launch_traversal(G, 1, nullptr, G->d_xpad, d_y, nullptr, nullptr, st, &launched))) return rc;
     if (launched) ++G->last_launches;
     CUDA_TRY(cudaEventRecord(G->ev1, st));

@@ -22,9 +22,7 @@
 #define OAT_NW (OAT_NT / 32)
 #define OAT_RI 32          // rings per patch
 #define OAT_RJ 32          // max azimuth samples per ring of a patch
-#ifndef OAT_MT
 #define OAT_MT 128         // threads per block of the marching kernels
-#endif
 #define OAT_BU 4           // steps per trip of the (rolled) backprojection marching loop
 
 struct OatBand {
@@ -93,17 +91,15 @@ void oat_launch_pad_cells(const OatDev &P, const float *x, float4 *cells, cudaSt
 // x[n] = sum of the 12 face-quad components that are node n (marching H^T)
 void oat_launch_unface(const OatDev &P, const float4 *faces, float *x, cudaStream_t st);
 // marching kernels (oat_march.cu, B = 32): mode 0 gathers from cell records into g (and writes y rows, step A4),
-// mode 1 scatters coef[q,k] = g'_k rho_k^2 into the face-quad accumulators
+// mode 1 reads the data y_in, forms g'_k rho_k^2 per band at load (step B1) and scatters it into the face-quad accumulators
 cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, float4 *faces, float *y_out,
-                             const float *coef, double *g, cudaStream_t st);
+                             const float *y_in, double *g, cudaStream_t st);
 // tile-stationary projection kernel (oat_tile.cu): a block keeps a brick of the volume in shared memory (TMA box load) and evaluates every
 // sample that falls into it; needs B = 32, the direction table and 7 c dt < 3 spacing
 bool oat_tile_supported(const OatDev &P);
 cudaError_t oat_launch_tile_fwd(const OatDev &P, const float *x, double *g, float *y, unsigned long long *counter,
                                 unsigned long long *stats, int nq_per_item, int allow_tma, cudaStream_t st);
 void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream_t st);
-// coef[q,k] = kappa (y[k-1] - y[k+1]) / (2 dt t_k) * rho_k^2   (Eq. 22 L172 with the rho^2 of S8; 0 where t_k <= 0)
-void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st);
 cudaError_t oat_build_patches(const OatDev &P, unsigned long long cap, int shift, int *q_count, unsigned long long **patches_out, long long *n_patches);
 // vector kernels (row C1 and the adjoint check); dots accumulate in fp64 into *out (pre-zeroed)
 void oat_launch_dot(const float *a, const float *b, long long n, double *out, cudaStream_t st);

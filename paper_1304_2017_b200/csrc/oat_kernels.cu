@@ -314,20 +314,6 @@ __global__ void oat_dir_table_kernel(const OatDev P, double2 *__restrict__ dir)
     }
 }
 
-// S7 with the rho^2 of S8 folded in: coef[q,k] = kappa (y[k-1] - y[k+1]) / (2 dt) / t_k * rho_k^2, 0 where t_k <= 0
-__global__ void oat_coef_kernel(const OatDev P, const float *__restrict__ y, float *__restrict__ coef)
-{
-    const long long n = (long long)P.Q * P.K;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const int k = (int)(i % P.K);
-        const double tk = P.t0 + (double)k * P.dt, rho = P.c * tk;
-        const float ym = (k - 1 >= 0) ? y[i - 1] : 0.f;
-        const float yp = (k + 1 < P.K) ? y[i + 1] : 0.f;
-        const double sp = P.kappa * ((double)ym - (double)yp) / (2.0 * P.dt);   // Eq. 22
-        coef[i] = rho > 0.0 ? (float)(sp / tk * rho * rho) : 0.f;
-    }
-}
-
 // number of patches per transducer (for the fused time-difference epilogue)
 __global__ void oat_count_patches_kernel(const unsigned long long *__restrict__ patches, long long n, int *__restrict__ q_count)
 {
@@ -579,12 +565,6 @@ static cudaError_t launch_patch_t(const OatDev &P, const float *xpad, float *xac
 void oat_launch_dir_table(const OatDev &P, int n_bands, double2 *dir, cudaStream_t st)
 {
     if (n_bands > 0) oat_dir_table_kernel<<<dim3(256, (unsigned)n_bands), 128, 0, st>>>(P, dir);
-}
-
-void oat_launch_coef(const OatDev &P, const float *y, float *coef, cudaStream_t st)
-{
-    const long long n = (long long)P.Q * P.K;
-    if (n > 0) oat_coef_kernel<<<grid_for(n, 256), 256, 0, st>>>(P, y, coef);
 }
 
 cudaError_t oat_launch_patch(int mode, const OatDev &P, const float *xpad, float *xacc, const float *y,

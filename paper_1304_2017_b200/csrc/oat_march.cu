@@ -102,21 +102,13 @@ __device__ __forceinline__ void fill_ring_rows(const OatRing *__restrict__ ring,
 
 __device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
-#ifndef OAT_LDHINT
 #define OAT_LDHINT ".L1::no_allocate"
-#endif
 __device__ __forceinline__ void ldg256_if(float (&c)[8], const float4 *p, bool pred)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
         "@p ld.global.nc" OAT_LDHINT ".v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"   // a record is used by one ray only
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]), "+f"(c[4]), "+f"(c[5]), "+f"(c[6]), "+f"(c[7])
         : "l"(p), "r"((int)pred));
-}
-
-__device__ __forceinline__ void red_add_v4_if(float4 *addr, float a, float b, float c, float d, bool pred)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t@p red.global.add.v4.f32 [%0], {%1,%2,%3,%4};\n\t}"
-                 ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d), "r"((int)pred) : "memory");
 }
 
 // The two reductions of one marching step of H^T: quad L into record `cur` when `fl`, quad H into record `cur + sa` when `fh`
@@ -175,13 +167,9 @@ __device__ __forceinline__ float half_warp_transpose_sum(float (&acc)[16], int l
 // share one load --, 6 FADD (fractions), 7 FFMA (Horner in fx, fy, fz) + 1 FFMA (quadrature weight): 26 instructions.
 // The records carry a zero margin of P.cm cells around the padded box, so no sample needs a bounds test.
 // ------------------------------------------------------------------------------------------------
-#ifndef OAT_NRH
-#define OAT_NRH 1     // rays marched together by one lane: their record loads are in flight at the same time
-#endif
+#define OAT_NRH 1     // rays marched together by one lane (2 was measured: 92 registers, 24 warps per SM, slower)
 #define OAT_QNH (16 * OAT_NRH + 32)    // queue entries per warp: at most 16 NRH - 1 left over + 32 new
-#ifndef OAT_MBLKH
-#define OAT_MBLKH (OAT_NRH == 1 ? 1152 / OAT_MT : 768 / OAT_MT)   // 9 blocks = 36 warps at 56 registers, no spills (8 blocks: 57.5 ms, 9: 54.6, 10: spills, 57.3)
-#endif
+#define OAT_MBLKH (1152 / OAT_MT)   // 9 blocks = 36 warps at 56 registers, no spills (8 blocks: 57.5 ms, 9: 54.6, 10: spills, 57.3)
 __global__ void __launch_bounds__(OAT_MT, OAT_MBLKH)
 oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__restrict__ y_out, double *__restrict__ g)
 {
@@ -332,12 +320,10 @@ oat_march_fwd_kernel(const OatDev P, const float4 *__restrict__ cells, float *__
 //   * when the ray steps to the next cell along a only (record index + one plane), the finished quad L is retired with
 //     ONE reduction and H is carried over as the new L; any other cell change flushes both quads.
 // ------------------------------------------------------------------------------------------------
-#ifndef OAT_MBLKT
 #define OAT_MBLKT 9     // 55 registers, no spills; with 4 steps per loop trip: 77.7 -> 77.0 ms on the 512-transducer subset
-#endif
 #define OAT_QNT 64    // queue entries per warp: at most 31 left over + 32 new
 __global__ void __launch_bounds__(OAT_MT, OAT_MBLKT)
-oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__restrict__ coef)
+oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__restrict__ y)
 {
     __shared__ double s_frame[16];
     __shared__ RingRow s_ring[OAT_RI];
@@ -359,8 +345,20 @@ oat_march_bwd_kernel(const OatDev P, float4 *__restrict__ faces, const float *__
         const int r0 = rb * OAT_RI;
         const int r1 = min(r0 + OAT_RI, P.qb_rings[(size_t)q * P.NB + b]);
         if (warp == 0) fill_ring_rows(P.ring + band.ring_ofs, band.dir_ofs, r0, r1, sec, P.rb_sectors[band.rb_ofs + rb], lane, s_ring);
-        if (warp == 1) {                                   // B1: the band's 32 coefficients g'_k rho_k^2, forward and reversed
-            const float cf = lane < band.nk ? coef[(size_t)q * P.K + band.k0 + lane] : 0.f;
+        if (warp == 1) {
+            // B1 fused at load (Eq. 22, S7 with the rho^2 of S8): the band's 32 coefficients
+            // g'_k rho_k^2 = kappa (y[k-1] - y[k+1]) / (2 dt) / t_k * rho_k^2 straight from the data row (zero extension at both
+            // ends, 0 where t_k <= 0), in fp64 with one rounding; stored forward and reversed
+            float cf = 0.f;
+            if (lane < band.nk) {
+                const int k = band.k0 + lane;
+                const float *__restrict__ row = y + (size_t)q * P.K;
+                const double tk = P.t0 + (double)k * P.dt, rho = P.c * tk;
+                const float ym = (k - 1 >= 0) ? row[k - 1] : 0.f;
+                const float yp = (k + 1 < P.K) ? row[k + 1] : 0.f;
+                const double sp = P.kappa * ((double)ym - (double)yp) / (2.0 * P.dt);
+                cf = rho > 0.0 ? (float)(sp / tk * rho * rho) : 0.f;
+            }
             s_coef[lane] = cf;
             s_coef[63 - lane] = cf;
             const bool any = __any_sync(0xffffffffu, cf != 0.f);
@@ -510,12 +508,12 @@ void oat_launch_pad_cells(const OatDev &P, const float *x, float4 *cells, cudaSt
 }
 
 cudaError_t oat_launch_march(int mode, const OatDev &P, const float4 *cells, float4 *faces, float *y_out,
-                             const float *coef, double *g, cudaStream_t st)
+                             const float *y_in, double *g, cudaStream_t st)
 {
     if (P.n_patches <= 0) return cudaSuccess;
     const long long cap = 0x7fffffffLL;
     const unsigned grid = (unsigned)(P.n_patches < cap ? P.n_patches : cap);
     if (mode == 0) oat_march_fwd_kernel<<<grid, OAT_MT, 0, st>>>(P, cells, y_out, g);
-    else oat_march_bwd_kernel<<<grid, OAT_MT, 0, st>>>(P, faces, coef);
+    else oat_march_bwd_kernel<<<grid, OAT_MT, 0, st>>>(P, faces, y_in);
     return cudaGetLastError();
 }
