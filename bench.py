@@ -137,6 +137,11 @@ def workload(args):
     if args.subset and args.subset < w.n_trans:
         _, w = w.seeded_subset(args.subset)
         note = f"DEBUG subset of {args.subset} transducers: not the BASELINE workload"
+    if args.kband:
+        from dataclasses import replace
+        w = replace(w, kband=args.kband)
+        note = ((note + "; ") if note else "") + (f"NON-BASELINE angular rule: B = {args.kband} time samples per rule (B = 1 is the paper's literal per-sample "
+                                                  "Eq. 37; any B < 32 runs on the generic patch kernel, not the marching kernels)")
     return w, note
 
 
@@ -572,6 +577,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number (1-5); 3 is the metric's")
     ap.add_argument("--subset", type=int, default=0, help="debug only: use a seeded subset of transducers")
+    ap.add_argument("--kband", type=int, default=0,
+                    help="measurement aid: time samples sharing one angular rule (default: the config's B = 32); 1 = the paper's per-sample Eq. 37")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank a rotated copy of the array (per-GPU work fixed), strong = rows of H partitioned")
     ap.add_argument("--e2e-steps", type=int, default=5)

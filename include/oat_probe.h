@@ -53,7 +53,10 @@ int oat_measure_gather_rate(int device, double *sectors_per_s);
  * 8 blocks of 128 threads per SM each holding `smem_kb_per_block` KB of (unused) shared memory -- what is carved out
  * for shared memory is taken from L1.
  * oat_measure_red_rate_ex: RED.128 with an address pattern within the warp: 0 every lane its own record, 1 32 consecutive
- * records (16 sectors), 2 one record per 128-byte line, 3 lane pairs sharing a sector, 4 four scattered lines of 8 records. */
+ * records (16 sectors), 2 one record per 128-byte line, 3 lane pairs sharing a sector (regular stride), 4 four scattered lines
+ * of 8 records; the sector-packing cases of a scattered accumulator (round 3): 5 every lane its own scattered sector, both
+ * 16-byte halves by two back-to-back reductions of the same thread, 6 lanes l and l + 16 fill one scattered sector, 7 lanes
+ * 2m and 2m + 1 fill one scattered sector.  The rate counts 16-byte reduction lanes in every pattern. */
 int oat_measure_gather_rate_ex(int device, int lanes_active, int smem_kb_per_block, double *sectors_per_s);
 int oat_measure_red_rate_ex(int device, int pattern, double *lanes_per_s);
 

@@ -88,8 +88,18 @@ __global__ void oat_red_probe_ex_kernel(float4 *__restrict__ buf, unsigned n16, 
         else if (pattern == 1) r = wbase + lane;                           // 32 consecutive records = 16 sectors in 4 lines
         else if (pattern == 2) r = wbase + lane * 8;                       // one record per 128-byte line, 32 lines
         else if (pattern == 3) r = wbase + (lane >> 1) * 64 + (lane & 1);  // lane pairs share a sector, pairs 1 KB apart
-        else r = wbase + (lane >> 3) * 1024 + (lane & 7);                  // 4 scattered lines of 8 records
-        red_add_v4(buf + (r % n16), 1.f, 1.f, 1.f, 1.f);
+        else if (pattern == 4) r = wbase + (lane >> 3) * 1024 + (lane & 7);  // 4 scattered lines of 8 records
+        else if (pattern == 5) { const unsigned h = (s >> 4) + lane * 2654435761u; r = ((h ^ (h >> 13)) * 0x9E3779B1u) & ~1u; }   // own sector, both halves (below)
+        else if (pattern == 6) { const unsigned h = (s >> 4) + (lane & 15) * 2654435761u; r = (((h ^ (h >> 13)) * 0x9E3779B1u) & ~1u) + (lane >> 4); }   // lanes l, l + 16 fill one scattered sector
+        else { const unsigned h = (s >> 4) + (lane >> 1) * 2654435761u; r = (((h ^ (h >> 13)) * 0x9E3779B1u) & ~1u) + (lane & 1); }      // lanes 2m, 2m + 1 fill one scattered sector
+        if (pattern == 5) {
+            // the face-quad case "flush L and H of one cell": one thread, two back-to-back reductions into the two
+            // 16-byte halves of ONE scattered 32-byte sector (n16 is even, so r + 1 stays inside the buffer)
+            float4 *p = buf + (r % n16);
+            red_add_v4(p, 1.f, 1.f, 1.f, 1.f);
+            red_add_v4(p + 1, 1.f, 1.f, 1.f, 1.f);
+        } else
+            red_add_v4(buf + (r % n16), 1.f, 1.f, 1.f, 1.f);
     }
 }
 
@@ -223,7 +233,7 @@ int oat_measure_gather_rate_ex(int device, int lanes_active, int smem_kb_per_blo
 
 int oat_measure_red_rate_ex(int device, int pattern, double *lanes_per_s)
 {
-    if (!lanes_per_s || pattern < 0 || pattern > 4) return fail(OAT_ERR_INVALID, "bad argument (pattern 0..4)");
+    if (!lanes_per_s || pattern < 0 || pattern > 7) return fail(OAT_ERR_INVALID, "bad argument (pattern 0..7)");
     CUDA_TRY(cudaSetDevice(device));
     const size_t bytes = 64u << 20;
     const int blocks = 148 * 8, iters = 2000;
@@ -246,7 +256,7 @@ int oat_measure_red_rate_ex(int device, int pattern, double *lanes_per_s)
     if (b) cudaEventDestroy(b);
     cudaFree(buf);
     if (e != cudaSuccess || !(ms > 0.f)) return fail(OAT_ERR_CUDA, "reduction-rate probe failed: %s", cudaGetErrorString(e));
-    *lanes_per_s = (double)blocks * 256.0 * iters / (ms * 1e-3);
+    *lanes_per_s = (double)blocks * 256.0 * iters * (pattern == 5 ? 2.0 : 1.0) / (ms * 1e-3);    // pattern 5 issues two reductions per step
     return OAT_OK;
 }
 
