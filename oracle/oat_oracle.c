@@ -225,7 +225,11 @@ int oat_ref_srt(const oat_ref_desc *d, const double *x, double *g)
     for (int q = 0; q < d->n_trans; ++q) {
         const double *rq = d->trans_xyz + 3 * (size_t)q;
         double ex[3], ey[3], ez[3], L;
-        if (ref_frame(&kc, rq, ex, ey, ez, &L)) { bad = 1; continue; }
+        if (ref_frame(&kc, rq, ex, ey, ez, &L)) {
+            _Pragma("omp atomic write")
+            bad = 1;
+            continue;
+        }
         for (int k = 0; k < d->nt; ++k) {
             const double rho = d->c * (d->t0 + k * d->dt);
             const double s = ref_shell(d, &kc, rq, ex, ey, ez, L, k, 0, x, NULL, 0.0, NULL);
@@ -264,7 +268,11 @@ int oat_ref_srt_adjoint(const oat_ref_desc *d, const double *gp, double *x)
         for (int q = 0; q < d->n_trans; ++q) {
             const double *rq = d->trans_xyz + 3 * (size_t)q;
             double ex[3], ey[3], ez[3], L;
-            if (ref_frame(&kc, rq, ex, ey, ez, &L)) { bad = 1; continue; }
+            if (ref_frame(&kc, rq, ex, ey, ez, &L)) {
+            _Pragma("omp atomic write")
+            bad = 1;
+            continue;
+        }
             for (int k = 0; k < d->nt; ++k) {
                 const double gv = gp[(size_t)q * d->nt + k];
                 if (gv == 0.0) continue;                           /* contributes exactly zero */
@@ -355,7 +363,11 @@ int oat_ref_count_samples(const oat_ref_desc *d, int64_t *per_qk, int64_t *total
     for (int q = 0; q < d->n_trans; ++q) {
         const double *rq = d->trans_xyz + 3 * (size_t)q;
         double ex[3], ey[3], ez[3], L;
-        if (ref_frame(&kc, rq, ex, ey, ez, &L)) { bad = 1; continue; }
+        if (ref_frame(&kc, rq, ex, ey, ez, &L)) {
+            _Pragma("omp atomic write")
+            bad = 1;
+            continue;
+        }
         for (int k = 0; k < d->nt; ++k) {
             int64_t cnt = 0;
             ref_shell(d, &kc, rq, ex, ey, ez, L, k, 2, NULL, NULL, 0.0, &cnt);
